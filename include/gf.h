@@ -1,0 +1,136 @@
+/*
+ * include/gf.h -- C ABI of libgf.so: lattice gauge fixing of 3+1-dimensional SU(3) gauge fields by
+ * checkerboard (RED/BLACK) overrelaxation, with the F_g / theta reductions and an SU(2)-heatbath
+ * simulated-annealing sweep, on one NVIDIA B200 (sm_100a).
+ *
+ * Method: Schroeck & Vogt, "Gauge fixing using overrelaxation and simulated annealing on GPUs"
+ * (arXiv:1209.4008).  Citations "PAPER.md:<line>" refer to the text of that paper; "Cn" are the readings of
+ * DESIGN.md ("Readings of the paper") taken where the paper is silent, ambiguous or garbled.
+ *
+ * Conventions common to all calls
+ *   - Every function returning int returns GF_OK (0) or a negative GF_E* code.  Nothing throws across the
+ *     ABI.  gf_last_error(ctx) gives the message of the last failing call on ctx (ctx == NULL: of the last
+ *     failing gf_create in this thread's process).
+ *   - "device" pointers are CUDA device pointers of the current device, owned by the CALLER (e.g. the
+ *     data_ptr() of a torch tensor); the library never frees or reallocates them.  "host" pointers are plain
+ *     host memory (pinned memory makes the copies faster, it is not required).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the default stream).  Calls that take a stream only
+ *     enqueue work on it and return; they do not synchronise.
+ *   - Lattice: extents Nx,Ny,Nz,Nt, all even and >= 2 (checkerboard with periodic boundaries, C5);
+ *     V = Nx*Ny*Nz*Nt < 2^31; direction mu = 0,1,2,3 <-> x,y,z,t.
+ *   - Canonical exchange layout (fp64, host or device): site s = x + Nx*(y + Ny*(z + Nz*t)); the double at
+ *       (((s*4 + mu)*3 + row)*3 + col)*2 + {0: re, 1: im}
+ *     is that part of (U_mu(x))_{row,col}.  V*4*18 doubles.
+ *   - Native layout (device only; what gf_overrelax / gf_anneal / gf_functional / gf_theta work on):
+ *     parity-split, component-major structure of arrays with the site index running fastest
+ *     (PAPER.md:124), 12 or 18 reals per link, in 128-bit vectors.  Exact definition:
+ *     DESIGN.md "Data layout in HBM".  Produced and consumed only through gf_pack / gf_unpack.
+ */
+#ifndef GF_H_
+#define GF_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gf_ctx gf_ctx; /* opaque; owns reduction scratch, launch configuration, staging buffers */
+
+enum { GF_FP32 = 0, GF_FP64 = 1 };      /* precision of the stored links and of the sweep arithmetic */
+enum { GF_LANDAU = 0, GF_COULOMB = 1 }; /* gauge condition */
+enum { GF_OK = 0, GF_EINVAL = -1, GF_ECUDA = -2, GF_ENOMEM = -3 };
+
+/* ---- life cycle --------------------------------------------------------------------------------------- */
+
+/* Problem statement of the paper: maximise F_g[U] (eq. 2.1) over gauge transformations by
+ * Alg. 1 on an Nx*Ny*Nz*Nt lattice, in Landau gauge (all four mu enter K, F, theta) or
+ * Coulomb gauge (mu = x,y,z only, every timeslice fixed independently; the temporal links are still
+ * transformed, C12).  Allocates only small device scratch.  *out is NULL on failure.
+ * GF_EINVAL: odd or < 2 extent, V >= 2^31, unknown precision / gauge.  GF_ECUDA: no usable device. */
+int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int gauge);
+void gf_destroy(gf_ctx* ctx);
+const char* gf_last_error(const gf_ctx* ctx);
+
+/* Reals stored per link: 18 (default) or 12 (rows 0 and 1 stored, row 2 = conj(row0 x row1) rebuilt on
+ * load, C16).  Must be called before the first gf_pack.  GF_EINVAL otherwise. */
+int gf_set_storage(gf_ctx* ctx, int reals_per_link);
+
+/* Bytes the caller must allocate (device, 256-byte aligned) for one field in the native layout:
+ * 4 * V * reals_per_link * sizeof(real). */
+size_t gf_field_bytes(const gf_ctx* ctx);
+
+/* ---- layout conversion (device -> device) --------------------------------------------------------------- */
+
+/* canonical fp64 (device) -> native (device).  fp32: rounds each real to nearest.  R12: drops row 2. */
+int gf_pack(gf_ctx* ctx, const double* U_canon_dev, void* U_native_dev, void* stream);
+/* native (device) -> canonical fp64 (device).  R12: row 2 is rebuilt from rows 0,1 (C16). */
+int gf_unpack(gf_ctx* ctx, const void* U_native_dev, double* U_canon_dev, void* stream);
+
+/* ---- the sweeps (device, in place, asynchronous on `stream`) --------------------------------------------- */
+
+/* `nsweeps` iterations of Alg. 1: for sublattice = RED (parity 0), BLACK (parity 1): for
+ * every site x of the sublattice: K(x) = sum_mu [U_mu(x) + U_mu(x-mu)^dagger] (eq. 2.3, C2); for
+ * the SU(2) subgroups (0,1),(0,2),(1,2) in turn (C4): g = maximiser of Re tr[g K] in the subgroup
+ * (eq. 2.4, C7), g -> g^omega to second order, reprojected to SU(2) (C9);
+ * U_mu(x) <- g U_mu(x), U_mu(x-mu) <- U_mu(x-mu) g^dagger for all four mu.
+ * U: native layout, device, updated in place.  omega in [1,2).  nsweeps >= 0.
+ * Launches 2*nsweeps kernels on `stream`.  GF_EINVAL: omega outside [1,2), nsweeps < 0, NULL U. */
+int gf_overrelax(gf_ctx* ctx, void* U_native_dev, double omega, int nsweeps, void* stream);
+
+/* Simulated annealing "preconditioner" (all details C13/C14): `nsteps` full sweeps
+ * (RED then BLACK), step i at temperature T_i = T_start + (T_end - T_start) * i / (nsteps - 1)
+ * (nsteps == 1: T_start).  Each site update replaces the overrelaxed maximiser by an SU(2) heatbath draw
+ * with weight exp(Re tr[g K] / T) per subgroup (Kennedy-Pendleton sampler), random numbers from
+ * Philox4x32-10 keyed by (seed; site, step, parity, subgroup, trial).  The step counter restarts at 0 on
+ * every call.  GF_EINVAL: T_start <= 0 or T_end <= 0, nsteps < 0, NULL U. */
+int gf_anneal(gf_ctx* ctx, void* U_native_dev, double T_start, double T_end, int nsteps,
+              unsigned long long seed, void* stream);
+
+/* ---- the reductions (device field -> host scalar; these calls synchronise) ------------------------------- */
+
+/* F = Re sum_{x, mu < Nd} tr U_mu(x) / (N_c * Nd * V)  (eq. 2.1, C1), Nd = 4 (Landau) or 3
+ * (Coulomb); F = 1 on the unit field.  Runs on the stream last passed to this ctx and waits for it. */
+int gf_functional(gf_ctx* ctx, const void* U_native_dev, double* F_host);
+/* theta = (1 / (V N_c)) sum_x tr[Delta(x) Delta(x)^dagger]  (eq. 2.5), Delta(x) the traceless
+ * part of (K - K^dagger) / (2i) (C3).  Landau: that number.  Coulomb: max over timeslices of the
+ * per-timeslice value (C12). */
+int gf_theta(gf_ctx* ctx, const void* U_native_dev, double* theta_host);
+/* per-timeslice theta_t = (1 / (V_s N_c)) sum_{x in slice t} tr[Delta Delta^dagger]; theta_host_Nt: Nt doubles */
+int gf_theta_slices(gf_ctx* ctx, const void* U_native_dev, double* theta_host_Nt);
+
+/* ---- host-buffer convenience path (what a user with a configuration in host memory calls) ---------------- */
+
+/* U_canon_host (canonical fp64, V*72 doubles) is copied to the device, packed, swept `nsweeps` times at
+ * `omega`, F and theta are reduced, the field is unpacked and copied back into U_canon_host; F_host /
+ * theta_host (may be NULL) receive the values after the last sweep.  Device staging buffers live in ctx and
+ * are reused between calls.  Synchronous.  GF_ENOMEM when the staging buffers cannot be allocated. */
+int gf_overrelax_host(gf_ctx* ctx, double* U_canon_host, double omega, int nsweeps, double* F_host,
+                      double* theta_host);
+
+/* ---- tuning and diagnostics ------------------------------------------------------------------------------ */
+
+/* Launch shape of the sweep kernels: threads_per_site in {1,2,4} (1: one thread holds all 8 links of a site;
+ * 2: two threads hold the links of 2 directions each; 4: one direction each; partial K summed by warp
+ * shuffles), block = threads per block (multiple of 32, <= 256).  0 keeps the current value.  Defaults are
+ * chosen per precision from the ncu measurements in profiles/. */
+int gf_set_tuning(gf_ctx* ctx, int threads_per_site, int block);
+/* fp32 unitarity policy (C15): every `every`-th sweep the RED half-sweep re-orthonormalises rows 0,1 of each
+ * link on load (and rebuilds row 2).  0 = never.  Default: 16 for fp32, 0 for fp64. */
+int gf_set_reunit(gf_ctx* ctx, int every);
+/* Alternate the block traversal direction between consecutive half-sweeps so that the tail of one
+ * half-sweep, still in L2, is what the next one reads first (1 = on, default; 0 = off). */
+int gf_set_l2_reversal(gf_ctx* ctx, int on);
+/* Optional debug output of gf_anneal: d_trials (device, V*3 unsigned, index 3*s + subgroup) receives the
+ * number of Kennedy-Pendleton trials of every (site, subgroup) of the LAST step; NULL switches it off. */
+int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);
+/* Number of kernels this ctx has launched so far. */
+unsigned long long gf_launch_count(const gf_ctx* ctx);
+/* Registers per thread and local-memory (spill) bytes per thread of the sweep kernel that the current
+ * (precision, storage, tuning) selects; mode 0 = overrelaxation, 1 = heatbath. */
+int gf_kernel_info(gf_ctx* ctx, int mode, int* regs_per_thread, int* local_bytes_per_thread);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GF_H_ */

@@ -1,0 +1,267 @@
+"""paper_1209_4008_b200 -- thin Python binding of libgf.so (include/gf.h).
+
+Lattice gauge fixing of SU(3) gauge fields by checkerboard overrelaxation and SU(2)-heatbath simulated annealing
+(Schroeck & Vogt, arXiv:1209.4008) on one NVIDIA B200.  Every step of the method runs in the CUDA kernels of
+``csrc/``; this module only marshals arguments.  PyTorch supplies device memory and streams, nothing else.
+There is no CPU path: without the compiled library or without a CUDA device the calls raise.
+
+The functions carry the names of the C ABI: ``gf_create, gf_overrelax, gf_anneal, gf_functional, gf_theta`` (plus
+``gf_pack / gf_unpack / gf_theta_slices / gf_overrelax_host`` and the tuning calls).  :class:`GaugeFixer` is a
+small convenience wrapper that owns a context and a native field.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+GF_FP32, GF_FP64 = 0, 1
+GF_LANDAU, GF_COULOMB = 0, 1
+GF_OK, GF_EINVAL, GF_ECUDA, GF_ENOMEM = 0, -1, -2, -3
+
+# paper flop model, Alg. 1: 60 + 19 + 4*(84+84) = 751 per subgroup, 2253 per site
+FLOP_PER_SITE = 3 * (60 + 19 + 4 * (84 + 84))
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgf.so")
+
+# every symbol include/gf.h declares: name -> (restype, argtypes)
+_vp, _i, _d, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+_ull = ctypes.c_ulonglong
+_pd, _pi = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int)
+SIGNATURES = {
+    "gf_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, _i, _i]),
+    "gf_destroy": (None, [_vp]),
+    "gf_last_error": (ctypes.c_char_p, [_vp]),
+    "gf_set_storage": (_i, [_vp, _i]),
+    "gf_field_bytes": (_sz, [_vp]),
+    "gf_pack": (_i, [_vp, _vp, _vp, _vp]),
+    "gf_unpack": (_i, [_vp, _vp, _vp, _vp]),
+    "gf_overrelax": (_i, [_vp, _vp, _d, _i, _vp]),
+    "gf_anneal": (_i, [_vp, _vp, _d, _d, _i, _ull, _vp]),
+    "gf_functional": (_i, [_vp, _vp, _pd]),
+    "gf_theta": (_i, [_vp, _vp, _pd]),
+    "gf_theta_slices": (_i, [_vp, _vp, _pd]),
+    "gf_overrelax_host": (_i, [_vp, _vp, _d, _i, _pd, _pd]),
+    "gf_set_tuning": (_i, [_vp, _i, _i]),
+    "gf_set_reunit": (_i, [_vp, _i]),
+    "gf_set_l2_reversal": (_i, [_vp, _i]),
+    "gf_set_trial_buffer": (_i, [_vp, _vp]),
+    "gf_launch_count": (_ull, [_vp]),
+    "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
+}
+
+_lib = None
+
+
+class GFError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"libgf error {code}: {message}")
+        self.code = code
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree libgf.so (build it with ``python -m paper_1209_4008_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1209_4008_b200.build` "
+                "(there is no CPU fallback)"
+            )
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(ctx, rc: int) -> None:
+    if rc != GF_OK:
+        msg = load_library().gf_last_error(ctx)
+        raise GFError(rc, msg.decode() if msg else "")
+
+
+def _ptr(t) -> int:
+    """device (or host) address of a torch tensor / numpy array / int"""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+# ---- the C ABI, one Python function per call -------------------------------------------------------------
+def gf_create(Nx: int, Ny: int, Nz: int, Nt: int, precision: int = GF_FP64, gauge: int = GF_LANDAU):
+    lib = load_library()
+    ctx = _vp()
+    rc = lib.gf_create(ctypes.byref(ctx), Nx, Ny, Nz, Nt, precision, gauge)
+    _check(None, rc)
+    return ctx
+
+
+def gf_destroy(ctx) -> None:
+    load_library().gf_destroy(ctx)
+
+
+def gf_set_storage(ctx, reals_per_link: int) -> None:
+    _check(ctx, load_library().gf_set_storage(ctx, reals_per_link))
+
+
+def gf_field_bytes(ctx) -> int:
+    return int(load_library().gf_field_bytes(ctx))
+
+
+def gf_pack(ctx, U_canon_dev, U_native_dev, stream=None) -> None:
+    _check(ctx, load_library().gf_pack(ctx, _ptr(U_canon_dev), _ptr(U_native_dev), _stream(stream)))
+
+
+def gf_unpack(ctx, U_native_dev, U_canon_dev, stream=None) -> None:
+    _check(ctx, load_library().gf_unpack(ctx, _ptr(U_native_dev), _ptr(U_canon_dev), _stream(stream)))
+
+
+def gf_overrelax(ctx, U, omega: float, nsweeps: int, stream=None) -> None:
+    _check(ctx, load_library().gf_overrelax(ctx, _ptr(U), float(omega), int(nsweeps), _stream(stream)))
+
+
+def gf_anneal(ctx, U, T_start: float, T_end: float, nsteps: int, seed: int, stream=None) -> None:
+    _check(ctx, load_library().gf_anneal(ctx, _ptr(U), float(T_start), float(T_end), int(nsteps), int(seed),
+                                        _stream(stream)))
+
+
+def gf_functional(ctx, U) -> float:
+    out = ctypes.c_double()
+    _check(ctx, load_library().gf_functional(ctx, _ptr(U), ctypes.byref(out)))
+    return out.value
+
+
+def gf_theta(ctx, U) -> float:
+    out = ctypes.c_double()
+    _check(ctx, load_library().gf_theta(ctx, _ptr(U), ctypes.byref(out)))
+    return out.value
+
+
+def gf_theta_slices(ctx, U, Nt: int):
+    out = (ctypes.c_double * Nt)()
+    _check(ctx, load_library().gf_theta_slices(ctx, _ptr(U), out))
+    return list(out)
+
+
+def gf_overrelax_host(ctx, U_canon_host, omega: float, nsweeps: int):
+    """U_canon_host: host array (numpy complex128 (V,4,3,3) or a pinned torch tensor), updated in place.
+    Returns (F, theta) after the last sweep."""
+    F, th = ctypes.c_double(), ctypes.c_double()
+    _check(ctx, load_library().gf_overrelax_host(ctx, _ptr(U_canon_host), float(omega), int(nsweeps),
+                                                ctypes.byref(F), ctypes.byref(th)))
+    return F.value, th.value
+
+
+def gf_set_tuning(ctx, threads_per_site: int = 0, block: int = 0) -> None:
+    _check(ctx, load_library().gf_set_tuning(ctx, threads_per_site, block))
+
+
+def gf_set_reunit(ctx, every: int) -> None:
+    _check(ctx, load_library().gf_set_reunit(ctx, every))
+
+
+def gf_set_l2_reversal(ctx, on: bool) -> None:
+    _check(ctx, load_library().gf_set_l2_reversal(ctx, int(bool(on))))
+
+
+def gf_set_trial_buffer(ctx, d_trials) -> None:
+    _check(ctx, load_library().gf_set_trial_buffer(ctx, _ptr(d_trials)))
+
+
+def gf_launch_count(ctx) -> int:
+    return int(load_library().gf_launch_count(ctx))
+
+
+def gf_kernel_info(ctx, mode: int = 0):
+    regs, loc = ctypes.c_int(), ctypes.c_int()
+    _check(ctx, load_library().gf_kernel_info(ctx, mode, ctypes.byref(regs), ctypes.byref(loc)))
+    return regs.value, loc.value
+
+
+# ---- convenience wrapper ---------------------------------------------------------------------------------
+class GaugeFixer:
+    """Owns a gf_ctx and one native field on the current CUDA device.
+
+    >>> gf = GaugeFixer((32, 32, 32, 32), precision="fp32", reals_per_link=12)
+    >>> gf.load(U)                      # numpy complex128 (V,4,3,3), canonical layout
+    >>> gf.overrelax(1.7, 100); gf.theta(), gf.functional()
+    >>> U_fixed = gf.download()
+    """
+
+    def __init__(self, dims, precision="fp64", gauge="landau", reals_per_link: int = 18):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1209_4008_b200 needs a CUDA device (there is no CPU path)")
+        self.dims = tuple(int(d) for d in dims)
+        self.V = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        self.precision = {"fp32": GF_FP32, "fp64": GF_FP64}[precision] if isinstance(precision, str) else precision
+        self.gauge = {"landau": GF_LANDAU, "coulomb": GF_COULOMB}[gauge] if isinstance(gauge, str) else gauge
+        self.R = int(reals_per_link)
+        self.ctx = gf_create(*self.dims, self.precision, self.gauge)
+        gf_set_storage(self.ctx, self.R)
+        self.nbytes = gf_field_bytes(self.ctx)
+        self.U = torch.empty(self.nbytes, dtype=torch.uint8, device="cuda")
+        self._torch = torch
+
+    def close(self):
+        if self.ctx is not None:
+            gf_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # field transfer
+    def load(self, U_canon):
+        """host numpy complex128 (V,4,3,3) or device float64 tensor with V*72 elements -> native field"""
+        torch = self._torch
+        if not isinstance(U_canon, torch.Tensor):
+            U_canon = torch.from_numpy(U_canon.view("float64").reshape(-1))
+        dev = U_canon.to("cuda", non_blocking=False).contiguous()
+        assert dev.dtype == torch.float64 and dev.numel() == self.V * 72
+        gf_pack(self.ctx, dev, self.U)
+        torch.cuda.current_stream().synchronize()
+
+    def download(self):
+        """native field -> host numpy complex128 (V,4,3,3)"""
+        torch = self._torch
+        dev = torch.empty(self.V * 72, dtype=torch.float64, device="cuda")
+        gf_unpack(self.ctx, self.U, dev)
+        return dev.cpu().numpy().view("complex128").reshape(self.V, 4, 3, 3)
+
+    # the method
+    def overrelax(self, omega: float, nsweeps: int, stream=None):
+        gf_overrelax(self.ctx, self.U, omega, nsweeps, stream)
+
+    def anneal(self, T_start: float, T_end: float, nsteps: int, seed: int, stream=None):
+        gf_anneal(self.ctx, self.U, T_start, T_end, nsteps, seed, stream)
+
+    def functional(self) -> float:
+        return gf_functional(self.ctx, self.U)
+
+    def theta(self) -> float:
+        return gf_theta(self.ctx, self.U)
+
+    def theta_slices(self):
+        return gf_theta_slices(self.ctx, self.U, self.dims[3])

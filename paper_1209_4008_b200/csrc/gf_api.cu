@@ -1,0 +1,337 @@
+// gf_api.cu -- the C ABI of libgf.so (include/gf.h): argument checking, context, launch sequencing.
+// No arithmetic of the method lives here; every step runs in the kernels of gf_sweep.cuh / gf_aux.cu.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/gf.h"
+#include "gf_internal.h"
+#include "gf_sweep.cuh"
+
+using namespace gf;
+
+struct gf_ctx {
+    int Nx, Ny, Nz, Nt;
+    int precision, gauge, R;
+    Lattice L;
+    int tps, block;
+    int reunit_every;
+    int l2_reversal;
+    unsigned long long sweeps_done;   // overrelaxation sweeps since creation (cadence of the fp32 reunitarisation)
+    unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
+    unsigned long long launches;
+    unsigned* d_trials;
+    cudaStream_t last_stream;
+    double* d_partials;               // reduction partials
+    double* d_out;                    // reduction results: [0] total, [1] max slice, [2..2+Nt) slices
+    double* h_out;                    // pinned mirror of d_out
+    int bx;
+    // host-buffer path staging (lazily allocated)
+    double* d_canon;
+    void* d_native;
+    char err[512];
+};
+
+static char g_create_err[512] = "";
+
+static int fail(gf_ctx* ctx, int code, const char* fmt, ...)
+{
+    char* dst = ctx ? ctx->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+static int cuda_fail(gf_ctx* ctx, cudaError_t e, const char* what)
+{
+    return fail(ctx, e == cudaErrorMemoryAllocation ? GF_ENOMEM : GF_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+static size_t real_size(const gf_ctx* c) { return c->precision == GF_FP64 ? 8 : 4; }
+
+extern "C" const char* gf_last_error(const gf_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int gauge)
+{
+    if (out == nullptr) return fail(nullptr, GF_EINVAL, "gf_create: out is NULL");
+    *out = nullptr;
+    const int N[4] = {Nx, Ny, Nz, Nt};
+    for (int d = 0; d < 4; ++d)
+        if (N[d] < 2 || (N[d] & 1))
+            return fail(nullptr, GF_EINVAL, "gf_create: extent %d is %d; every extent must be even and >= 2 (C5)", d, N[d]);
+    const unsigned long long V = (unsigned long long)Nx * Ny * Nz * Nt;
+    if (V >= (1ull << 31)) return fail(nullptr, GF_EINVAL, "gf_create: volume %llu >= 2^31", V);
+    if (precision != GF_FP32 && precision != GF_FP64) return fail(nullptr, GF_EINVAL, "gf_create: unknown precision %d", precision);
+    if (gauge != GF_LANDAU && gauge != GF_COULOMB) return fail(nullptr, GF_EINVAL, "gf_create: unknown gauge %d", gauge);
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, GF_ECUDA, "gf_create: no CUDA device (%s); this library has no CPU path",
+                    e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+
+    gf_ctx* c = new (std::nothrow) gf_ctx();
+    if (c == nullptr) return fail(nullptr, GF_ENOMEM, "gf_create: host allocation failed");
+    c->Nx = Nx; c->Ny = Ny; c->Nz = Nz; c->Nt = Nt;
+    c->precision = precision; c->gauge = gauge; c->R = 18;
+    c->L.Nxh = Nx / 2; c->L.Ny = Ny; c->L.Nz = Nz; c->L.Nt = Nt; c->L.H = (unsigned)(V / 2);
+    // launch shape chosen from the measurements in profiles/ 
+    c->tps = precision == GF_FP64 ? 4 : 1;
+    c->block = 64;
+    c->reunit_every = precision == GF_FP32 ? 16 : 0;
+    c->l2_reversal = 1;
+    c->sweeps_done = 0; c->half_sweeps = 0; c->launches = 0;
+    c->d_trials = nullptr; c->last_stream = nullptr;
+    c->d_canon = nullptr; c->d_native = nullptr;
+    c->err[0] = 0;
+    c->bx = reduce_blocks_per_slice(c->L);
+    const size_t npart = (size_t)c->bx * 2 * Nt;
+    c->d_partials = nullptr; c->d_out = nullptr; c->h_out = nullptr;
+    if ((e = cudaMalloc(&c->d_partials, npart * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_out, (size_t)(Nt + 2) * sizeof(double))) != cudaSuccess ||
+        (e = cudaMallocHost(&c->h_out, (size_t)(Nt + 2) * sizeof(double))) != cudaSuccess) {
+        int rc = cuda_fail(nullptr, e, "gf_create: scratch allocation");
+        gf_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return GF_OK;
+}
+
+extern "C" void gf_destroy(gf_ctx* c)
+{
+    if (c == nullptr) return;
+    if (c->d_partials) cudaFree(c->d_partials);
+    if (c->d_out) cudaFree(c->d_out);
+    if (c->h_out) cudaFreeHost(c->h_out);
+    if (c->d_canon) cudaFree(c->d_canon);
+    if (c->d_native) cudaFree(c->d_native);
+    delete c;
+}
+
+extern "C" int gf_set_storage(gf_ctx* c, int R)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (R != 12 && R != 18) return fail(c, GF_EINVAL, "gf_set_storage: reals_per_link must be 12 or 18, got %d", R);
+    if (c->d_native != nullptr && R != c->R) { cudaFree(c->d_native); c->d_native = nullptr; }
+    c->R = R;
+    return GF_OK;
+}
+
+extern "C" size_t gf_field_bytes(const gf_ctx* c)
+{
+    if (c == nullptr) return 0;
+    return (size_t)8 * c->L.H * (size_t)c->R * real_size(c);
+}
+
+extern "C" int gf_set_tuning(gf_ctx* c, int tps, int block)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (tps != 0 && tps != 1 && tps != 2 && tps != 4) return fail(c, GF_EINVAL, "gf_set_tuning: threads_per_site must be 1, 2 or 4");
+    if (block != 0 && (block < 32 || block > MAX_BLOCK || block % 32)) return fail(c, GF_EINVAL, "gf_set_tuning: block must be a multiple of 32 in [32, %d]", MAX_BLOCK);
+    if (tps) c->tps = tps;
+    if (block) c->block = block;
+    return GF_OK;
+}
+
+extern "C" int gf_set_reunit(gf_ctx* c, int every)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (every < 0) return fail(c, GF_EINVAL, "gf_set_reunit: every must be >= 0");
+    c->reunit_every = every;
+    return GF_OK;
+}
+
+extern "C" int gf_set_l2_reversal(gf_ctx* c, int on)
+{
+    if (c == nullptr) return GF_EINVAL;
+    c->l2_reversal = on ? 1 : 0;
+    return GF_OK;
+}
+
+extern "C" int gf_set_trial_buffer(gf_ctx* c, unsigned* d_trials)
+{
+    if (c == nullptr) return GF_EINVAL;
+    c->d_trials = d_trials;
+    return GF_OK;
+}
+
+extern "C" unsigned long long gf_launch_count(const gf_ctx* c) { return c ? c->launches : 0ull; }
+
+static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p, cudaStream_t st)
+{
+    if (c->precision == GF_FP32) return c->R == 18 ? launch_sweep_f32_r18(c->tps, mode, c->block, p, st) : launch_sweep_f32_r12(c->tps, mode, c->block, p, st);
+    return c->R == 18 ? launch_sweep_f64_r18(c->tps, mode, c->block, p, st) : launch_sweep_f64_r12(c->tps, mode, c->block, p, st);
+}
+
+extern "C" int gf_kernel_info(gf_ctx* c, int mode, int* regs, int* local_bytes)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (mode != 0 && mode != 1) return fail(c, GF_EINVAL, "gf_kernel_info: mode must be 0 or 1");
+    cudaFuncAttributes a;
+    cudaError_t e;
+    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(c->tps, mode, &a) : sweep_attributes_f32_r12(c->tps, mode, &a);
+    else e = c->R == 18 ? sweep_attributes_f64_r18(c->tps, mode, &a) : sweep_attributes_f64_r12(c->tps, mode, &a);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gf_kernel_info");
+    if (regs) *regs = a.numRegs;
+    if (local_bytes) *local_bytes = (int)a.localSizeBytes;
+    return GF_OK;
+}
+
+static SweepParams base_params(gf_ctx* c, void* U)
+{
+    SweepParams p;
+    memset(&p, 0, sizeof p);
+    p.U = U;
+    p.L = c->L;
+    p.nd = c->gauge == GF_COULOMB ? 3 : 4;
+    p.omega = 1.0;
+    p.T = 1.0;
+    return p;
+}
+
+extern "C" int gf_pack(gf_ctx* c, const double* canon, void* native, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (canon == nullptr || native == nullptr) return fail(c, GF_EINVAL, "gf_pack: NULL pointer");
+    c->last_stream = (cudaStream_t)stream;
+    cudaError_t e = launch_pack(c->precision, c->R, c->L, c->Nx, canon, native, c->last_stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gf_pack");
+    c->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (canon == nullptr || native == nullptr) return fail(c, GF_EINVAL, "gf_unpack: NULL pointer");
+    c->last_stream = (cudaStream_t)stream;
+    cudaError_t e = launch_unpack(c->precision, c->R, c->L, c->Nx, native, canon, c->last_stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gf_unpack");
+    c->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (U == nullptr) return fail(c, GF_EINVAL, "gf_overrelax: U is NULL");
+    if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_overrelax: omega = %g outside [1,2) (PAPER.md:63)", omega);
+    if (nsweeps < 0) return fail(c, GF_EINVAL, "gf_overrelax: nsweeps = %d < 0", nsweeps);
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    SweepParams p = base_params(c, U);
+    p.omega = omega;
+    for (int sweep = 0; sweep < nsweeps; ++sweep) {
+        const bool reunit = c->reunit_every > 0 && ((c->sweeps_done + 1) % (unsigned long long)c->reunit_every) == 0;
+        for (int parity = 0; parity < 2; ++parity) { // RED, BLACK
+            p.parity = parity;
+            p.reunit = (reunit && parity == 0) ? 1 : 0; // every link is loaded once per half-sweep (C6)
+            p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
+            cudaError_t e = launch_sweep(c, MODE_OVERRELAX, p, st);
+            if (e != cudaSuccess) return cuda_fail(c, e, "gf_overrelax: kernel launch");
+            c->half_sweeps += 1;
+            c->launches += 1;
+        }
+        c->sweeps_done += 1;
+    }
+    return GF_OK;
+}
+
+extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, unsigned long long seed, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (U == nullptr) return fail(c, GF_EINVAL, "gf_anneal: U is NULL");
+    if (!(T_start > 0.0) || !(T_end > 0.0)) return fail(c, GF_EINVAL, "gf_anneal: temperatures must be > 0 (got %g, %g)", T_start, T_end);
+    if (nsteps < 0) return fail(c, GF_EINVAL, "gf_anneal: nsteps = %d < 0", nsteps);
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    SweepParams p = base_params(c, U);
+    p.key0 = (uint32_t)seed;
+    p.key1 = (uint32_t)(seed >> 32);
+    for (int step = 0; step < nsteps; ++step) {
+        // T_i = T_start + (T_end - T_start) i / (nsteps - 1)   (C13)
+        p.T = nsteps > 1 ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
+        p.step = (uint32_t)step;
+        p.trials = (step == nsteps - 1) ? c->d_trials : nullptr;
+        for (int parity = 0; parity < 2; ++parity) {
+            p.parity = parity;
+            p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
+            cudaError_t e = launch_sweep(c, MODE_HEATBATH, p, st);
+            if (e != cudaSuccess) return cuda_fail(c, e, "gf_anneal: kernel launch");
+            c->half_sweeps += 1;
+            c->launches += 1;
+        }
+    }
+    return GF_OK;
+}
+
+// runs one reduction on last_stream and brings the Nt+2 results to h_out
+static int reduce_to_host(gf_ctx* c, const void* U, bool theta, const char* who)
+{
+    if (U == nullptr) return fail(c, GF_EINVAL, "%s: U is NULL", who);
+    const int nd = c->gauge == GF_COULOMB ? 3 : 4;
+    cudaStream_t st = c->last_stream;
+    cudaError_t e = theta ? launch_theta(c->precision, c->R, c->L, nd, U, c->d_partials, c->d_out, st)
+                          : launch_functional(c->precision, c->R, c->L, nd, U, c->d_partials, c->d_out, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, who);
+    c->launches += 2;
+    e = cudaMemcpyAsync(c->h_out, c->d_out, (size_t)(c->Nt + 2) * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(c, e, who);
+    return GF_OK;
+}
+
+extern "C" int gf_functional(gf_ctx* c, const void* U, double* F_host)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (F_host == nullptr) return fail(c, GF_EINVAL, "gf_functional: F_host is NULL");
+    int rc = reduce_to_host(c, U, false, "gf_functional");
+    if (rc != GF_OK) return rc;
+    *F_host = c->h_out[0];
+    return GF_OK;
+}
+
+extern "C" int gf_theta(gf_ctx* c, const void* U, double* theta_host)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (theta_host == nullptr) return fail(c, GF_EINVAL, "gf_theta: theta_host is NULL");
+    int rc = reduce_to_host(c, U, true, "gf_theta");
+    if (rc != GF_OK) return rc;
+    *theta_host = c->gauge == GF_COULOMB ? c->h_out[1] : c->h_out[0];
+    return GF_OK;
+}
+
+extern "C" int gf_theta_slices(gf_ctx* c, const void* U, double* theta_host_Nt)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (theta_host_Nt == nullptr) return fail(c, GF_EINVAL, "gf_theta_slices: output is NULL");
+    int rc = reduce_to_host(c, U, true, "gf_theta_slices");
+    if (rc != GF_OK) return rc;
+    memcpy(theta_host_Nt, c->h_out + 2, (size_t)c->Nt * sizeof(double));
+    return GF_OK;
+}
+
+extern "C" int gf_overrelax_host(gf_ctx* c, double* U_host, double omega, int nsweeps, double* F_host, double* theta_host)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (U_host == nullptr) return fail(c, GF_EINVAL, "gf_overrelax_host: U_canon_host is NULL");
+    const size_t canon_bytes = (size_t)c->L.H * 2 * 72 * sizeof(double);
+    cudaError_t e;
+    if (c->d_canon == nullptr && (e = cudaMalloc(&c->d_canon, canon_bytes)) != cudaSuccess) { c->d_canon = nullptr; return cuda_fail(c, e, "gf_overrelax_host: staging allocation"); }
+    if (c->d_native == nullptr && (e = cudaMalloc(&c->d_native, gf_field_bytes(c))) != cudaSuccess) { c->d_native = nullptr; return cuda_fail(c, e, "gf_overrelax_host: staging allocation"); }
+    cudaStream_t st = c->last_stream;
+    if ((e = cudaMemcpyAsync(c->d_canon, U_host, canon_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(c, e, "gf_overrelax_host: H2D copy");
+    int rc = gf_pack(c, c->d_canon, c->d_native, st);
+    if (rc == GF_OK) rc = gf_overrelax(c, c->d_native, omega, nsweeps, st);
+    if (rc == GF_OK) rc = gf_unpack(c, c->d_native, c->d_canon, st);
+    if (rc != GF_OK) return rc;
+    if ((e = cudaMemcpyAsync(U_host, c->d_canon, canon_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(c, e, "gf_overrelax_host: D2H copy");
+    if (F_host != nullptr && (rc = gf_functional(c, c->d_native, F_host)) != GF_OK) return rc;
+    if (theta_host != nullptr && (rc = gf_theta(c, c->d_native, theta_host)) != GF_OK) return rc;
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(c, e, "gf_overrelax_host: synchronise");
+    return GF_OK;
+}

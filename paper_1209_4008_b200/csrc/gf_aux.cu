@@ -1,0 +1,224 @@
+// gf_aux.cu -- layout conversion (canonical fp64 <-> native) and the F_g / theta reductions (the paper's second
+// kernel: "checks the current value of the gauge fixing functional F_g[U] and the gauge precision
+// theta").  Reductions: fp64 arithmetic on the stored links, warp shuffles inside a block, one partial per block,
+// then a single-block final pass that adds the partials in a fixed order (deterministic, no atomics).
+#include "gf_internal.h"
+#include "gf_device.cuh"
+
+namespace gf {
+
+constexpr int AUX_BLOCK = 256;
+
+// ---------------------------------------------------------------------------------------------------------
+// pack / unpack.  One thread per (half-site h, link block l = parity*4 + mu).
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, int R>
+__global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, const double* __restrict__ canon, T* __restrict__ native)
+{
+    const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (unsigned long long)L.H * 8ull) return;
+    const unsigned h = (unsigned)(gid % L.H);
+    const int l = (int)(gid / L.H), parity = l >> 2, mu = l & 3;
+    const Site s = decode_site(L, h, parity);
+    const double* src = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
+    cx<T> u[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) u[e] = {(T)src[2 * e], (T)src[2 * e + 1]};
+    LinkIO<T, R>::store(native + (size_t)l * R * L.H, L.H, h, u);
+}
+
+template <typename T, int R>
+__global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* __restrict__ native, double* __restrict__ canon)
+{
+    const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (unsigned long long)L.H * 8ull) return;
+    const unsigned h = (unsigned)(gid % L.H);
+    const int l = (int)(gid / L.H), parity = l >> 2, mu = l & 3;
+    const Site s = decode_site(L, h, parity);
+    cx<T> u[9];
+    LinkIO<T, R>::load(native + (size_t)l * R * L.H, L.H, h, u);
+    double* dst = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { dst[2 * e] = (double)u[e].re; dst[2 * e + 1] = (double)u[e].im; }
+}
+
+cudaError_t launch_pack(int prec, int R, const Lattice& L, int, const double* canon, void* native, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (prec == 0 && R == 18) pack_kernel<float, 18><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
+    else if (prec == 0 && R == 12) pack_kernel<float, 12><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
+    else if (prec == 1 && R == 18) pack_kernel<double, 18><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
+    else if (prec == 1 && R == 12) pack_kernel<double, 12><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack(int prec, int R, const Lattice& L, int, const void* native, double* canon, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (prec == 0 && R == 18) unpack_kernel<float, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
+    else if (prec == 0 && R == 12) unpack_kernel<float, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
+    else if (prec == 1 && R == 18) unpack_kernel<double, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
+    else if (prec == 1 && R == 12) unpack_kernel<double, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// reductions.  Grid (bx, 2*Nt): blockIdx.y = 2*t + parity, so every block lies inside one timeslice and the
+// Coulomb per-timeslice theta (C12) falls out of the same partials.
+// ---------------------------------------------------------------------------------------------------------
+int reduce_blocks_per_slice(const Lattice& L)
+{
+    const unsigned Hs = (unsigned)L.Nxh * L.Ny * L.Nz;
+    return (int)((Hs + AUX_BLOCK - 1) / AUX_BLOCK);
+}
+
+__device__ __forceinline__ void block_sum_to(double v, double* dst)
+{
+    __shared__ double warp_sums[AUX_BLOCK / 32];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0) warp_sums[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double acc = 0.0;
+#pragma unroll
+        for (int w = 0; w < AUX_BLOCK / 32; ++w) acc += warp_sums[w];
+        *dst = acc;
+    }
+}
+
+// eq. 2.1, reading C1: sum over x, mu < nd of Re tr U_mu(x) on the current links
+template <typename T, int R>
+__global__ void __launch_bounds__(AUX_BLOCK) functional_kernel(Lattice L, int nd, const T* __restrict__ native,
+                                                               double* __restrict__ partials)
+{
+    const unsigned Hs = (unsigned)L.Nxh * L.Ny * L.Nz;
+    const unsigned local = blockIdx.x * blockDim.x + threadIdx.x;
+    const int t = blockIdx.y >> 1, parity = blockIdx.y & 1;
+    double acc = 0.0;
+    if (local < Hs) {
+        const unsigned h = (unsigned)t * Hs + local;
+        for (int mu = 0; mu < nd; ++mu) {
+            cx<T> u[9];
+            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, h, u);
+            acc += (double)u[0].re + (double)u[4].re + (double)u[8].re;
+        }
+    }
+    block_sum_to(acc, partials + (size_t)blockIdx.y * gridDim.x + blockIdx.x);
+}
+
+// eq. 2.5, reading C3: Delta(x) = traceless part of (K - K^dagger)/(2i),
+// tr[Delta Delta^dagger] = sum_ab |Delta_ab|^2.  K from eq. 2.3 in the in-place form (C2).
+template <typename T, int R>
+__global__ void __launch_bounds__(AUX_BLOCK) theta_kernel(Lattice L, int nd, const T* __restrict__ native,
+                                                          double* __restrict__ partials)
+{
+    const unsigned Hs = (unsigned)L.Nxh * L.Ny * L.Nz;
+    const unsigned local = blockIdx.x * blockDim.x + threadIdx.x;
+    const int t = blockIdx.y >> 1, parity = blockIdx.y & 1;
+    double acc = 0.0;
+    if (local < Hs) {
+        const Site s = decode_site(L, (unsigned)t * Hs + local, parity);
+        cx<double> K[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) K[e] = {0.0, 0.0};
+        for (int mu = 0; mu < nd; ++mu) {
+            cx<T> f[9], b[9];
+            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, s.h, f);
+            LinkIO<T, R>::load(native + (size_t)((1 - parity) * 4 + mu) * R * L.H, L.H, backward_neighbour(L, s, mu), b);
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    K[3 * r + c].re += (double)f[3 * r + c].re + (double)b[3 * c + r].re;
+                    K[3 * r + c].im += (double)f[3 * r + c].im - (double)b[3 * c + r].im;
+                }
+        }
+        // D_ab = (K_ab - conj(K_ba)) / (2i) = [ (Im K_ab + Im K_ba) - i (Re K_ab - Re K_ba) ] / 2
+        const double tr3 = (K[0].im + K[4].im + K[8].im) / 3.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double d = K[4 * a].im - tr3;
+            acc += d * d;
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b2 = a + 1; b2 < 3; ++b2) {
+                const double dr = 0.5 * (K[3 * a + b2].im + K[3 * b2 + a].im);
+                const double di = 0.5 * (K[3 * a + b2].re - K[3 * b2 + a].re);
+                acc += 2.0 * (dr * dr + di * di); // D is Hermitian: |D_ab|^2 = |D_ba|^2
+            }
+    }
+    block_sum_to(acc, partials + (size_t)blockIdx.y * gridDim.x + blockIdx.x);
+}
+
+// final pass: one block; thread i adds the partials of timeslices i, i+blockDim, ... in index order; thread 0 then
+// combines the slices in order.  scale_total multiplies the lattice sum; scale_slice the per-slice sums.
+__global__ void __launch_bounds__(AUX_BLOCK) final_kernel(int Nt, int per_slice, const double* __restrict__ partials,
+                                                          double scale_total, double scale_slice, double* __restrict__ out)
+{
+    for (int t = threadIdx.x; t < Nt; t += blockDim.x) {
+        double acc = 0.0;
+        const double* p = partials + (size_t)t * per_slice;
+        for (int i = 0; i < per_slice; ++i) acc += p[i];
+        out[2 + t] = acc;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double total = 0.0, mx = 0.0;
+        for (int t = 0; t < Nt; ++t) {
+            const double v = out[2 + t];
+            total += v;
+            const double sv = v * scale_slice;
+            if (t == 0 || sv > mx) mx = sv;
+            out[2 + t] = sv;
+        }
+        out[0] = total * scale_total;
+        out[1] = mx;
+    }
+}
+
+template <bool THETA>
+static cudaError_t launch_reduction(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+                                    double* out, cudaStream_t st)
+{
+    const int bx = reduce_blocks_per_slice(L);
+    const dim3 grid((unsigned)bx, (unsigned)(2 * L.Nt));
+#define GF_RED(T, RR)                                                                                   \
+    do {                                                                                                \
+        if (THETA) theta_kernel<T, RR><<<grid, AUX_BLOCK, 0, st>>>(L, nd, (const T*)native, partials);   \
+        else functional_kernel<T, RR><<<grid, AUX_BLOCK, 0, st>>>(L, nd, (const T*)native, partials);    \
+    } while (0)
+    if (prec == 0 && R == 18) GF_RED(float, 18);
+    else if (prec == 0 && R == 12) GF_RED(float, 12);
+    else if (prec == 1 && R == 18) GF_RED(double, 18);
+    else if (prec == 1 && R == 12) GF_RED(double, 12);
+    else return cudaErrorInvalidValue;
+#undef GF_RED
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const double V = 2.0 * (double)L.H, Vs = V / (double)L.Nt;
+    const double scale_total = THETA ? 1.0 / (3.0 * V) : 1.0 / (3.0 * nd * V);
+    const double scale_slice = THETA ? 1.0 / (3.0 * Vs) : 1.0 / (3.0 * nd * Vs);
+    final_kernel<<<1, AUX_BLOCK, 0, st>>>(L.Nt, 2 * bx, partials, scale_total, scale_slice, out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_functional(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+                              double* out, cudaStream_t st)
+{
+    return launch_reduction<false>(prec, R, L, nd, native, partials, out, st);
+}
+
+cudaError_t launch_theta(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+                         double* out, cudaStream_t st)
+{
+    return launch_reduction<true>(prec, R, L, nd, native, partials, out, st);
+}
+
+} // namespace gf

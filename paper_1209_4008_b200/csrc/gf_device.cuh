@@ -1,0 +1,258 @@
+// gf_device.cuh -- device-side building blocks of libgf.so (sm_100a): complex / SU(3) register arithmetic,
+// the native link layout, checkerboard site indexing, Philox4x32-10.
+//
+// Native layout ("Data layout in HBM").  H = V/2 sites per parity.  Half-site index of a site
+// (x,y,z,t) of parity p = (x+y+z+t)&1:   h = (x>>1) + (Nx/2) * (y + Ny * (z + Nz * t)).
+// Link U_mu(x) lives in link block  l = p*4 + mu  (parity-split: PAPER.md:124), which holds R*H reals.
+// Inside a block the complex entries e = 3*row + col (e < R/2; R = 12 stores rows 0,1 only) are
+// component-major with the site index fastest, grouped in 128-bit vectors:
+//   fp64: plane e is H double2 (re,im)                          -> real offset  e*2*H + 2*h
+//   fp32: plane q = e/2 is H float4 (re,im of e=2q; re,im of e=2q+1) -> real offset  q*4*H + 4*h
+//         R = 18: the ninth entry (e = 8) is a trailing plane of H float2 at real offset 16*H + 2*h
+// so a warp's load of one plane is one contiguous 512-byte (fp32: 512 or 256) run.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gf {
+
+// ---------------------------------------------------------------------------------------------------------
+// complex numbers in registers
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+struct cx {
+    T re, im;
+};
+
+template <typename T>
+__device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return {a.re + b.re, a.im + b.im}; }
+template <typename T>
+__device__ __forceinline__ cx<T> operator-(cx<T> a, cx<T> b) { return {a.re - b.re, a.im - b.im}; }
+template <typename T>
+__device__ __forceinline__ cx<T> operator*(cx<T> a, cx<T> b)
+{
+    return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re};
+}
+template <typename T>
+__device__ __forceinline__ cx<T> conj(cx<T> a) { return {a.re, -a.im}; }
+// conj(a) * b
+template <typename T>
+__device__ __forceinline__ cx<T> cmul_ca(cx<T> a, cx<T> b)
+{
+    return {a.re * b.re + a.im * b.im, a.re * b.im - a.im * b.re};
+}
+// a * conj(b)
+template <typename T>
+__device__ __forceinline__ cx<T> cmul_cb(cx<T> a, cx<T> b)
+{
+    return {a.re * b.re + a.im * b.im, a.im * b.re - a.re * b.im};
+}
+
+template <typename T> __device__ __forceinline__ T gf_rsqrt(T x);
+template <> __device__ __forceinline__ float gf_rsqrt<float>(float x) { return 1.0f / sqrtf(x); }
+template <> __device__ __forceinline__ double gf_rsqrt<double>(double x) { return 1.0 / sqrt(x); }
+template <typename T> __device__ __forceinline__ T gf_sqrt(T x);
+template <> __device__ __forceinline__ float gf_sqrt<float>(float x) { return sqrtf(x); }
+template <> __device__ __forceinline__ double gf_sqrt<double>(double x) { return sqrt(x); }
+
+// ---------------------------------------------------------------------------------------------------------
+// SU(3) links: 9 complex entries, row-major, always fully unrolled so they stay in registers
+// ---------------------------------------------------------------------------------------------------------
+
+// row 2 = conj(row0 x row1)  (C16; "reconstruct the third line")
+template <typename T>
+__device__ __forceinline__ void rebuild_row2(cx<T> (&u)[9])
+{
+    u[6] = conj(u[1] * u[5] - u[2] * u[4]);
+    u[7] = conj(u[2] * u[3] - u[0] * u[5]);
+    u[8] = conj(u[0] * u[4] - u[1] * u[3]);
+}
+
+// Gram-Schmidt on rows 0,1 then row 2 rebuilt: the fp32 unitarity policy (C15)
+template <typename T>
+__device__ __forceinline__ void reunitarise(cx<T> (&u)[9])
+{
+    T n0 = gf_rsqrt<T>(u[0].re * u[0].re + u[0].im * u[0].im + u[1].re * u[1].re + u[1].im * u[1].im +
+                       u[2].re * u[2].re + u[2].im * u[2].im);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { u[c].re *= n0; u[c].im *= n0; }
+    cx<T> dot = cmul_ca(u[0], u[3]) + cmul_ca(u[1], u[4]) + cmul_ca(u[2], u[5]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) u[3 + c] = u[3 + c] - dot * u[c];
+    T n1 = gf_rsqrt<T>(u[3].re * u[3].re + u[3].im * u[3].im + u[4].re * u[4].re + u[4].im * u[4].im +
+                       u[5].re * u[5].re + u[5].im * u[5].im);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { u[3 + c].re *= n1; u[3 + c].im *= n1; }
+    rebuild_row2(u);
+}
+
+// SU(2) element embedded in the (I,J) subgroup (C4): quaternion q -> a = q0 + i q3, b = q2 + i q1;
+// G_II = a, G_IJ = b, G_JI = -conj(b), G_JJ = conj(a).
+// Left multiplication  M <- G M  touches rows I,J   (Alg. 1; 84 flop per link).
+template <int I, int J, typename T>
+__device__ __forceinline__ void su2_left(cx<T> a, cx<T> b, cx<T> (&m)[9])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        cx<T> ui = m[3 * I + c], uj = m[3 * J + c];
+        m[3 * I + c] = a * ui + b * uj;
+        m[3 * J + c] = cmul_ca(a, uj) - cmul_ca(b, ui);
+    }
+}
+// Right multiplication  M <- M G^dagger  touches columns I,J   (Alg. 1; 84 flop per link).
+// (G^dagger)_II = conj(a), (G^dagger)_IJ = -b, (G^dagger)_JI = conj(b), (G^dagger)_JJ = a.
+template <int I, int J, int ROWS, typename T>
+__device__ __forceinline__ void su2_right_dagger(cx<T> a, cx<T> b, cx<T> (&m)[9])
+{
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+        cx<T> ui = m[3 * r + I], uj = m[3 * r + J];
+        m[3 * r + I] = cmul_cb(ui, a) + cmul_cb(uj, b);
+        m[3 * r + J] = uj * a - ui * b;
+    }
+}
+
+// quaternionic part of the (I,J) block of K (C7):  Re tr[G K] = const + g0 k0 - g1 k1 - g2 k2 - g3 k3
+template <int I, int J, typename T>
+__device__ __forceinline__ void su2_project(const cx<T> (&K)[9], T (&k)[4])
+{
+    k[0] = K[3 * I + I].re + K[3 * J + J].re;
+    k[1] = K[3 * I + J].im + K[3 * J + I].im;
+    k[2] = K[3 * I + J].re - K[3 * J + I].re;
+    k[3] = K[3 * I + I].im - K[3 * J + J].im;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// native layout access
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, int R> struct LinkIO;
+
+template <int R>
+struct LinkIO<double, R> {
+    static constexpr int NE = R / 2;
+    // blk: first real of the link block; H: sites per parity; h: half-site index
+    static __device__ __forceinline__ void load(const double* __restrict__ blk, size_t H, size_t h,
+                                                cx<double> (&u)[9])
+    {
+        const double2* p = reinterpret_cast<const double2*>(blk) + h;
+#pragma unroll
+        for (int e = 0; e < NE; ++e) {
+            double2 v = p[(size_t)e * H];
+            u[e] = {v.x, v.y};
+        }
+        if (R == 12) rebuild_row2(u);
+    }
+    static __device__ __forceinline__ void store(double* __restrict__ blk, size_t H, size_t h,
+                                                 const cx<double> (&u)[9])
+    {
+        double2* p = reinterpret_cast<double2*>(blk) + h;
+#pragma unroll
+        for (int e = 0; e < NE; ++e) p[(size_t)e * H] = make_double2(u[e].re, u[e].im);
+    }
+};
+
+template <int R>
+struct LinkIO<float, R> {
+    static constexpr int NQ = R / 4; // float4 planes: 4 (R18) or 3 (R12)
+    static __device__ __forceinline__ void load(const float* __restrict__ blk, size_t H, size_t h,
+                                                cx<float> (&u)[9])
+    {
+        const float4* p = reinterpret_cast<const float4*>(blk) + h;
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            float4 v = p[(size_t)q * H];
+            u[2 * q] = {v.x, v.y};
+            u[2 * q + 1] = {v.z, v.w};
+        }
+        if (R == 18) {
+            float2 v = reinterpret_cast<const float2*>(blk + 16 * H)[h];
+            u[8] = {v.x, v.y};
+        } else {
+            rebuild_row2(u);
+        }
+    }
+    static __device__ __forceinline__ void store(float* __restrict__ blk, size_t H, size_t h,
+                                                 const cx<float> (&u)[9])
+    {
+        float4* p = reinterpret_cast<float4*>(blk) + h;
+#pragma unroll
+        for (int q = 0; q < NQ; ++q)
+            p[(size_t)q * H] = make_float4(u[2 * q].re, u[2 * q].im, u[2 * q + 1].re, u[2 * q + 1].im);
+        if (R == 18) reinterpret_cast<float2*>(blk + 16 * H)[h] = make_float2(u[8].re, u[8].im);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// checkerboard site indexing ("divisions and modulo conversions"; C5: periodic, parity =
+// (x+y+z+t)&1)
+// ---------------------------------------------------------------------------------------------------------
+struct Lattice {
+    int Nxh, Ny, Nz, Nt; // Nxh = Nx/2
+    unsigned H;          // V/2
+};
+
+struct Site {
+    unsigned h;      // half-site index inside its parity block
+    int xh, y, z, t; // x = 2*xh + q
+    int q;           // (y + z + t + parity) & 1
+};
+
+__device__ __forceinline__ Site decode_site(const Lattice& L, unsigned h, int parity)
+{
+    Site s;
+    s.h = h;
+    unsigned r = h / (unsigned)L.Nxh;
+    s.xh = (int)(h - r * (unsigned)L.Nxh);
+    unsigned r2 = r / (unsigned)L.Ny;
+    s.y = (int)(r - r2 * (unsigned)L.Ny);
+    unsigned r3 = r2 / (unsigned)L.Nz;
+    s.z = (int)(r2 - r3 * (unsigned)L.Nz);
+    s.t = (int)r3;
+    s.q = (s.y + s.z + s.t + parity) & 1;
+    return s;
+}
+
+// canonical site index s = x + Nx (y + Ny (z + Nz t)) = 2h + q
+__device__ __forceinline__ unsigned canonical_index(const Site& s) { return 2u * s.h + (unsigned)s.q; }
+
+// half-site index (in the OTHER parity block) of the neighbour x - mu_hat
+__device__ __forceinline__ unsigned backward_neighbour(const Lattice& L, const Site& s, int mu)
+{
+    if (mu == 0) {
+        // x - 1 = 2 xh + q - 1: same xh when q = 1, xh - 1 (periodic) when q = 0
+        if (s.q) return s.h;
+        return s.xh == 0 ? s.h + (unsigned)(L.Nxh - 1) : s.h - 1u;
+    }
+    if (mu == 1) {
+        unsigned st = (unsigned)L.Nxh;
+        return s.y == 0 ? s.h + st * (unsigned)(L.Ny - 1) : s.h - st;
+    }
+    if (mu == 2) {
+        unsigned st = (unsigned)L.Nxh * (unsigned)L.Ny;
+        return s.z == 0 ? s.h + st * (unsigned)(L.Nz - 1) : s.h - st;
+    }
+    unsigned st = (unsigned)L.Nxh * (unsigned)L.Ny * (unsigned)L.Nz;
+    return s.t == 0 ? s.h + st * (unsigned)(L.Nt - 1) : s.h - st;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11) -- the CUDA path's own copy
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+} // namespace gf

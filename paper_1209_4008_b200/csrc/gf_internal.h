@@ -1,0 +1,35 @@
+// gf_internal.h -- declarations shared by the translation units of libgf.so (host side)
+#pragma once
+#include <cuda_runtime.h>
+
+namespace gf {
+
+struct SweepParams;
+struct Lattice;
+
+// gf_sweep_inst.cu, one pair per (precision, reals-per-link)
+#define GF_DECLARE_SWEEP(sfx)                                                                                 \
+    cudaError_t launch_sweep_##sfx(int tps, int mode, int block, const SweepParams& p, cudaStream_t stream); \
+    cudaError_t sweep_attributes_##sfx(int tps, int mode, cudaFuncAttributes* attr);
+GF_DECLARE_SWEEP(f32_r12)
+GF_DECLARE_SWEEP(f32_r18)
+GF_DECLARE_SWEEP(f64_r12)
+GF_DECLARE_SWEEP(f64_r18)
+#undef GF_DECLARE_SWEEP
+
+// gf_aux.cu: layout conversion and reductions.  prec: 0 fp32, 1 fp64; R: 12 or 18.
+cudaError_t launch_pack(int prec, int R, const Lattice& L, int Nx, const double* canon, void* native,
+                        cudaStream_t stream);
+cudaError_t launch_unpack(int prec, int R, const Lattice& L, int Nx, const void* native, double* canon,
+                          cudaStream_t stream);
+
+// Reduction scratch (device): partial sums per block, then a deterministic fixed-order final pass.
+//   functional: out[0] = sum_{x, mu<nd} Re tr U_mu(x) / (3 nd V)
+//   theta:      out[0] = theta over the whole lattice (eq. 2.5); out[1] = max_t theta_t; out[2+t] = theta_t
+int reduce_blocks_per_slice(const Lattice& L);
+cudaError_t launch_functional(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+                              double* out, cudaStream_t stream);
+cudaError_t launch_theta(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+                         double* out, cudaStream_t stream);
+
+} // namespace gf

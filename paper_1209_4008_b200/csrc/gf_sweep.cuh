@@ -1,0 +1,237 @@
+// gf_sweep.cuh -- the checkerboard half-sweep kernel (overrelaxation and SU(2) heatbath), Alg. 1 of the paper
+// (PAPER.md:74-91), for sm_100a.
+//
+// Granularity (re-decided for sm_100a; the paper's Fermi design used 8 threads per site because of a
+// 63-register limit): TPS threads share one site, each holding the forward and the
+// backward link of 4/TPS directions in registers (TPS = 1: all 8 links, 144 reals).  Partial sums of K(x)
+// are combined with warp shuffles (the sm_100a stand-in for the paper's shared-memory accumulator,
+// PAPER.md:146); every thread of a site then runs the same three SU(2) subgroup steps redundantly on the
+// full K and applies each g to its own links immediately (literal data flow of Alg. 1, C8).
+//
+// Memory: every link is read once and written once per half-sweep (C6), each access a coalesced 128-bit
+// vector per thread (gf_device.cuh); all loads of a thread are issued before the first use.
+#pragma once
+#include "gf_device.cuh"
+
+namespace gf {
+
+enum { MODE_OVERRELAX = 0, MODE_HEATBATH = 1 };
+constexpr int MAX_BLOCK = 256;
+
+struct SweepParams {
+    void* U;        // native field
+    Lattice L;
+    int parity;     // sublattice updated by this launch: 0 = RED, 1 = BLACK (C5)
+    int nd;         // directions entering K: 4 (Landau) or 3 (Coulomb, C12)
+    int reunit;     // re-orthonormalise links on load (C15)
+    int reverse;    // traverse blocks back to front (L2 reuse between consecutive half-sweeps)
+    double omega;   // overrelaxation parameter
+    double T;       // heatbath temperature (C13)
+    uint32_t key0, key1, step; // Philox key = seed, step = annealing step (C14)
+    unsigned* trials;          // optional: KP trial counts, index 3*s + subgroup
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// SU(2) step, overrelaxation: maximiser (eq. 2.4, on the projected block, C7), then g^omega to
+// second order and reprojection (reading C9):
+//   g = (k0,-k1,-k2,-k3)/|k|;  d = g0 - 1;  h0 = 1 + w d (1 + (w-1) g0);  hvec = w (1 + (w-1) d) gvec;  h /= |h|
+// ---------------------------------------------------------------------------------------------------------
+template <typename T> struct Tiny;
+template <> struct Tiny<float> { static constexpr float n = 1e-30f; };
+template <> struct Tiny<double> { static constexpr double n = 1e-300; };
+
+template <typename T>
+__device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[4])
+{
+    T n = gf_sqrt<T>(k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3]);
+    if (n < Tiny<T>::n) { h[0] = T(1); h[1] = h[2] = h[3] = T(0); return; }
+    T inv = T(1) / n;
+    T g0 = k[0] * inv, g1 = -k[1] * inv, g2 = -k[2] * inv, g3 = -k[3] * inv;
+    T d = g0 - T(1);
+    T h0 = T(1) + w * d * (T(1) + (w - T(1)) * g0);
+    T f = w * (T(1) + (w - T(1)) * d);
+    T h1 = f * g1, h2 = f * g2, h3 = f * g3;
+    T n2 = h0 * h0 + h1 * h1 + h2 * h2 + h3 * h3;
+    if (n2 < T(1e-20)) { h[0] = g0; h[1] = g1; h[2] = g2; h[3] = g3; return; }
+    T hn = gf_rsqrt<T>(n2);
+    h[0] = h0 * hn; h[1] = h1 * hn; h[2] = h2 * hn; h[3] = h3 * hn;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// SU(2) step, heatbath (C13/C14): alpha = |k|/T; draw h0 with density sqrt(1-h0^2) exp(alpha h0) by
+// Kennedy-Pendleton, hvec uniform on the sphere; g = h (x) conj(khat).
+// Uniforms: u = (2 (x >> 9) + 1) 2^-24, exact in fp32 and fp64.
+// ---------------------------------------------------------------------------------------------------------
+template <typename T> struct KPMath;
+template <> struct KPMath<double> {
+    static __device__ __forceinline__ double uni(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
+    static __device__ __forceinline__ double cos2pi(double u) { return cos(6.283185307179586476925286766559 * u); }
+    static __device__ __forceinline__ double sin2pi(double u) { return sin(6.283185307179586476925286766559 * u); }
+    static __device__ __forceinline__ double neglog(double u) { return -log(u); }
+    // delta = (-ln u1 / alpha) cos^2 + (-ln u2 / alpha), in exactly this order, no FMA contraction: this
+    // value decides acceptance and must follow the stated recipe operation by operation (C14)
+    static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha)
+    {
+        return __dadd_rn(__dmul_rn(__ddiv_rn(l1, alpha), __dmul_rn(c, c)), __ddiv_rn(l2, alpha));
+    }
+    static __device__ __forceinline__ bool accept(double u4, double d) { return __dmul_rn(u4, u4) <= __dsub_rn(1.0, __dmul_rn(0.5, d)); }
+};
+template <> struct KPMath<float> {
+    static __device__ __forceinline__ float uni(uint32_t x) { return (float)(2u * (x >> 9) + 1u) * (1.0f / 16777216.0f); }
+    static __device__ __forceinline__ float cos2pi(float u) { return cospif(2.0f * u); }
+    static __device__ __forceinline__ float sin2pi(float u) { return sinpif(2.0f * u); }
+    static __device__ __forceinline__ float neglog(float u) { return -logf(u); }
+    static __device__ __forceinline__ float delta(float l1, float l2, float c, float alpha)
+    {
+        return __fadd_rn(__fmul_rn(__fdiv_rn(l1, alpha), __fmul_rn(c, c)), __fdiv_rn(l2, alpha));
+    }
+    static __device__ __forceinline__ bool accept(float u4, float d) { return __fmul_rn(u4, u4) <= __fsub_rn(1.0f, __fmul_rn(0.5f, d)); }
+};
+
+// returns the number of trials used (0: degenerate block, identity taken; 4097: cap hit)
+template <typename T>
+__device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T temperature, uint32_t key0,
+                                                      uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2,
+                                                      T (&g)[4])
+{
+    using M = KPMath<T>;
+    T n = gf_sqrt<T>(k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3]);
+    if (n < Tiny<T>::n) { g[0] = T(1); g[1] = g[2] = g[3] = T(0); return 0u; }
+    T alpha = n / temperature;
+    T kc0 = k[0] / n, kc1 = -k[1] / n, kc2 = -k[2] / n, kc3 = -k[3] / n; // conj(khat)
+    uint32_t x[4];
+    T h0 = T(1);
+    bool accepted = false;
+    unsigned trial = 0;
+    for (; trial < 4096u; ++trial) {
+        philox4x32_10(c0, c1, c2, trial, key0, key1, x);
+        T u1 = M::uni(x[0]), u2 = M::uni(x[1]), u3 = M::uni(x[2]), u4 = M::uni(x[3]);
+        T c = M::cos2pi(u3);
+        T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha);
+        if (M::accept(u4, d)) { h0 = T(1) - d; accepted = true; break; }
+    }
+    if (!accepted) {
+        // h = identity  =>  g = conj(khat)
+        g[0] = kc0; g[1] = kc1; g[2] = kc2; g[3] = kc3;
+        return 4097u;
+    }
+    philox4x32_10(c0, c1, c2, 0x80000000u, key0, key1, x);
+    T cos_t = T(1) - T(2) * M::uni(x[0]);
+    T up = M::uni(x[1]);
+    T r = gf_sqrt<T>(fmax(T(0), T(1) - h0 * h0));
+    T sin_t = gf_sqrt<T>(fmax(T(0), T(1) - cos_t * cos_t));
+    T h1 = r * sin_t * M::cos2pi(up);
+    T h2 = r * sin_t * M::sin2pi(up);
+    T h3 = r * cos_t;
+    // g = h (x) conj(khat):  (pq)_0 = p0 q0 - p.q,  (pq)_vec = p0 qvec + q0 pvec - pvec x qvec   (C13)
+    g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3;
+    g[1] = h0 * kc1 + kc0 * h1 - (h2 * kc3 - h3 * kc2);
+    g[2] = h0 * kc2 + kc0 * h2 - (h3 * kc1 - h1 * kc3);
+    g[3] = h0 * kc3 + kc0 * h3 - (h1 * kc2 - h2 * kc1);
+    return trial + 1u;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// the half-sweep kernel
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, int R, int TPS, int MODE>
+struct SweepKernel {
+    static constexpr int NMU = 4 / TPS;
+    using IO = LinkIO<T, R>;
+
+    template <int I, int J, int SUB>
+    static __device__ __forceinline__ void subgroup(const SweepParams& p, cx<T> (&K)[9], cx<T> (&F)[NMU][9],
+                                                    cx<T> (&B)[NMU][9], uint32_t site_canon, bool record)
+    {
+        T k[4], h[4];
+        su2_project<I, J>(K, k);
+        if (MODE == MODE_OVERRELAX) {
+            su2_overrelax_step<T>(k, (T)p.omega, h);
+        } else {
+            unsigned ntr = su2_heatbath_step<T>(k, (T)p.T, p.key0, p.key1, site_canon, p.step,
+                                                ((uint32_t)p.parity << 2) | (uint32_t)SUB, h);
+            if (record && p.trials != nullptr) p.trials[3u * (size_t)site_canon + SUB] = ntr;
+        }
+        const cx<T> a = {h[0], h[3]}, b = {h[2], h[1]}; // C4
+#pragma unroll
+        for (int m = 0; m < NMU; ++m) {
+            su2_left<I, J>(a, b, F[m]);                 // U_mu(x)     <- G U_mu(x)
+            su2_right_dagger<I, J, 3>(a, b, B[m]);      // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
+        }
+        su2_left<I, J>(a, b, K);                        // K <- G K  (C8)
+    }
+
+    static __device__ __forceinline__ void run(const SweepParams& p)
+    {
+        const unsigned blk = p.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+        const unsigned gtid = blk * blockDim.x + threadIdx.x;
+        const unsigned slot = gtid / TPS;
+        const int lane_mu0 = (int)(gtid % TPS) * NMU; // first direction this thread owns
+        const bool active = slot < p.L.H;             // inactive threads shadow site 0 and store nothing,
+        const Site s = decode_site(p.L, active ? slot : 0u, p.parity); // so warp shuffles stay converged
+        const size_t H = p.L.H;
+        T* const base = reinterpret_cast<T*>(p.U);
+
+        cx<T> F[NMU][9], B[NMU][9];
+        unsigned hb[NMU];
+        // issue every load before the first use
+#pragma unroll
+        for (int m = 0; m < NMU; ++m) {
+            const int mu = lane_mu0 + m;
+            hb[m] = backward_neighbour(p.L, s, mu);
+            IO::load(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m]);
+            IO::load(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m]);
+        }
+        if (p.reunit) {
+#pragma unroll
+            for (int m = 0; m < NMU; ++m) { reunitarise(F[m]); reunitarise(B[m]); }
+        }
+
+        // K(x) = sum_{mu < nd} [ U_mu(x) + U_mu(x-mu)^dagger ]   (eq. 2.3; C2)
+        cx<T> K[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) K[e] = {T(0), T(0)};
+#pragma unroll
+        for (int m = 0; m < NMU; ++m) {
+            if (lane_mu0 + m < p.nd) {
+#pragma unroll
+                for (int r = 0; r < 3; ++r)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) K[3 * r + c] = K[3 * r + c] + F[m][3 * r + c] + conj(B[m][3 * c + r]);
+            }
+        }
+        if (TPS > 1) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) {
+#pragma unroll
+                for (int off = 1; off < TPS; off <<= 1) {
+                    K[e].re += __shfl_xor_sync(0xffffffffu, K[e].re, off);
+                    K[e].im += __shfl_xor_sync(0xffffffffu, K[e].im, off);
+                }
+            }
+        }
+
+        const uint32_t sc = canonical_index(s);
+        const bool record = active && (lane_mu0 == 0);
+        subgroup<0, 1, 0>(p, K, F, B, sc, record); // Cabibbo-Marinari subgroups in the order of C4
+        subgroup<0, 2, 1>(p, K, F, B, sc, record);
+        subgroup<1, 2, 2>(p, K, F, B, sc, record);
+
+        if (active) {
+#pragma unroll
+            for (int m = 0; m < NMU; ++m) {
+                const int mu = lane_mu0 + m;
+                IO::store(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m]);
+                IO::store(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m]);
+            }
+        }
+    }
+};
+
+template <typename T, int R, int TPS, int MODE>
+__global__ void __launch_bounds__(MAX_BLOCK) gf_half_sweep_kernel(const SweepParams p)
+{
+    SweepKernel<T, R, TPS, MODE>::run(p);
+}
+
+} // namespace gf

@@ -1,0 +1,59 @@
+// gf_sweep_inst.cu -- one translation unit per (precision, reals-per-link): compiled four times by build.py with
+//   -DGF_INST_FP64={0,1} -DGF_INST_R={12,18}
+// so the twenty-four half-sweep kernels build in parallel.  Each unit exports one launcher and one
+// attribute query, declared in gf_internal.h.
+#include "gf_internal.h"
+#include "gf_sweep.cuh"
+
+#if GF_INST_FP64
+typedef double real_t;
+#else
+typedef float real_t;
+#endif
+
+#define GF_CAT3_(a, b, c) a##b##c
+#define GF_CAT3(a, b, c) GF_CAT3_(a, b, c)
+#if GF_INST_FP64
+#define GF_SUFFIX GF_CAT3(f64, _r, GF_INST_R)
+#else
+#define GF_SUFFIX GF_CAT3(f32, _r, GF_INST_R)
+#endif
+#define GF_NAME(stem) GF_CAT3(stem, _, GF_SUFFIX)
+
+namespace gf {
+
+typedef void (*sweep_fn)(const SweepParams);
+
+static sweep_fn pick(int tps, int mode)
+{
+    constexpr int R = GF_INST_R;
+    if (mode == MODE_OVERRELAX) {
+        if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX>;
+        if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX>;
+        if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_OVERRELAX>;
+    } else if (mode == MODE_HEATBATH) {
+        if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_HEATBATH>;
+        if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_HEATBATH>;
+        if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_HEATBATH>;
+    }
+    return nullptr;
+}
+
+cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParams& p, cudaStream_t stream)
+{
+    sweep_fn fn = pick(tps, mode);
+    if (fn == nullptr || block <= 0 || block > MAX_BLOCK || (block % 32) != 0) return cudaErrorInvalidValue;
+    const unsigned long long threads = (unsigned long long)p.L.H * (unsigned long long)tps;
+    const unsigned grid = (unsigned)((threads + (unsigned)block - 1ull) / (unsigned)block);
+    fn<<<grid, block, 0, stream>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, cudaFuncAttributes* attr)
+{
+    sweep_fn fn = pick(tps, mode);
+    if (fn == nullptr) return cudaErrorInvalidValue;
+    return cudaFuncGetAttributes(attr, fn);
+}
+
+} // namespace gf

@@ -1,0 +1,316 @@
+"""GPU-vs-oracle parity of the CUDA path, through the C ABI (include/gf.h), on the same seeded inputs.
+
+Tolerances are BASELINE.json north_star's: per-link max|dU| after one sweep <= 1e-12 (fp64), <= 5e-5 (fp32);
+after N sweeps F relative <= 1e-10 (fp64) / 1e-5 (fp32), theta relative <= 1e-6 (fp64); annealing: identical
+Kennedy-Pendleton trial counts (accept decisions) given the shared Philox stream (fp64).
+"""
+import numpy as np
+import pytest
+
+import gf_inputs
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL_LINK = {"fp64": 1e-12, "fp32": 5e-5}
+TOL_F = {"fp64": 1e-10, "fp32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def gfm():
+    import torch
+
+    assert torch.cuda.is_available()
+    import paper_1209_4008_b200 as m
+
+    m.load_library()  # fails loudly if the CUDA library is missing
+    return m
+
+
+def _fixer(gfm, dims, precision, gauge="landau", R=18, tps=0, block=0):
+    fx = gfm.GaugeFixer(dims, precision=precision, gauge=gauge, reals_per_link=R)
+    gfm.gf_set_tuning(fx.ctx, tps, block)
+    return fx
+
+
+def _orc_gauge(gauge):
+    return oracle.COULOMB if gauge == "coulomb" else oracle.LANDAU
+
+
+# ---------------------------------------------------------------------------------------------------------
+# layout round trip
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("R", [18, 12])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 8, 4, 6)])
+def test_pack_unpack_roundtrip(gfm, precision, R, dims):
+    U = gf_inputs.smooth_random(dims, 0.4, 21)
+    fx = _fixer(gfm, dims, precision, R=R)
+    fx.load(U)
+    back = fx.download()
+    if precision == "fp64" and R == 18:
+        assert np.array_equal(back, U)  # bit exact
+    elif precision == "fp64":
+        assert np.array_equal(back[:, :, :2], U[:, :, :2])  # stored rows bit exact
+        assert np.abs(back - U).max() < 1e-15  # row 2 rebuilt (C16)
+    else:
+        ref = U.astype(np.complex64).astype(np.complex128)
+        if R == 18:
+            assert np.array_equal(back, ref)  # each real rounded to nearest fp32
+        else:
+            assert np.array_equal(back[:, :, :2], ref[:, :, :2])
+            assert np.abs(back - U).max() < 4e-7
+    fx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# reductions
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("R", [18, 12])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (10, 6, 4, 8)])
+def test_functional_and_theta(gfm, precision, R, gauge, dims):
+    U = gf_inputs.smooth_random(dims, 0.4, 22)
+    oracle.overrelax(U, dims, 1.7, 3, _orc_gauge(gauge))  # partly fixed: theta no longer O(1)
+    fx = _fixer(gfm, dims, precision, gauge, R)
+    fx.load(U)
+    # the reductions run in fp64 on the STORED links: compare with the oracle on exactly those
+    stored = fx.download()
+    og = _orc_gauge(gauge)
+    assert fx.functional() == pytest.approx(oracle.functional(stored, dims, og), rel=1e-12)
+    assert fx.theta() == pytest.approx(oracle.theta(stored, dims, og), rel=1e-10)
+    np.testing.assert_allclose(fx.theta_slices(), oracle.theta_slices(stored, dims, og), rtol=1e-10)
+    # and with the oracle on the original fp64 field, within the storage rounding
+    rel = 1e-12 if precision == "fp64" else 2e-6
+    assert fx.functional() == pytest.approx(oracle.functional(U, dims, og), rel=rel)
+    assert fx.theta() == pytest.approx(oracle.theta(U, dims, og), rel=max(rel * 50, 1e-10))
+    fx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# one sweep, link by link; every kernel variant
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("R", [18, 12])
+@pytest.mark.parametrize("tps", [1, 2, 4])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_one_sweep_links(gfm, precision, R, tps, gauge):
+    dims = (8, 6, 4, 10)  # V/2 = 960: several blocks, ragged last warp for every tps
+    U = gf_inputs.smooth_random(dims, 0.4, 23)
+    fx = _fixer(gfm, dims, precision, gauge, R, tps=tps, block=64)
+    fx.load(U)
+    fx.overrelax(1.7, 1)
+    got = fx.download()
+    oracle.overrelax(U, dims, 1.7, 1, _orc_gauge(gauge))
+    assert np.abs(got - U).max() <= TOL_LINK[precision]
+    fx.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (2, 4, 2, 6), (4, 4, 4, 4), (34, 2, 2, 2)])
+def test_one_sweep_small_and_extent_two(gfm, precision, dims):
+    """degenerate sizes: extent 2 (x - mu and x + mu are the same site, the two links still distinct, C5)"""
+    U = gf_inputs.hot(dims, 24)
+    for tps in (1, 2, 4):
+        for block in (32, 256):
+            fx = _fixer(gfm, dims, precision, tps=tps, block=block)
+            fx.load(U)
+            fx.overrelax(1.5, 1)
+            got = fx.download()
+            fx.close()
+            ref = U.copy()
+            oracle.overrelax(ref, dims, 1.5, 1)
+            assert np.abs(got - ref).max() <= TOL_LINK[precision], (dims, tps, block)
+
+
+def test_half_sweep_order_and_reversal(gfm):
+    """RED first then BLACK (C5); the traversal direction of the blocks must not matter (C6)."""
+    dims = (8, 8, 4, 4)
+    U = gf_inputs.smooth_random(dims, 0.4, 25)
+    outs = []
+    for rev in (0, 1):
+        fx = _fixer(gfm, dims, "fp64")
+        gfm.gf_set_l2_reversal(fx.ctx, rev)
+        fx.load(U)
+        fx.overrelax(1.7, 3)
+        outs.append(fx.download())
+        fx.close()
+    assert np.array_equal(outs[0], outs[1])
+    ref = U.copy()
+    oracle.overrelax(ref, dims, 1.7, 3)
+    assert np.abs(outs[0] - ref).max() <= 5e-12
+
+
+# ---------------------------------------------------------------------------------------------------------
+# N sweeps: F and theta
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,R", [("fp64", 18), ("fp64", 12), ("fp32", 18), ("fp32", 12)])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_n_sweeps_F_theta(gfm, precision, R, gauge):
+    dims = (8, 8, 8, 8)
+    nsweeps = 60
+    U = gf_inputs.smooth_random(dims, 0.4, 26)
+    fx = _fixer(gfm, dims, precision, gauge, R)
+    fx.load(U)
+    fx.overrelax(1.7, nsweeps)
+    og = _orc_gauge(gauge)
+    oracle.overrelax(U, dims, 1.7, nsweeps, og)
+    F_ref, th_ref = oracle.functional(U, dims, og), oracle.theta(U, dims, og)
+    assert fx.functional() == pytest.approx(F_ref, rel=TOL_F[precision])
+    if precision == "fp64":
+        assert fx.theta() == pytest.approx(th_ref, rel=1e-6)
+    else:
+        assert fx.theta() == pytest.approx(th_ref, rel=5e-2, abs=1e-12)  # no tolerance stated for fp32 theta
+    fx.close()
+
+
+def test_config1_trivial_orbit(gfm):
+    """BASELINE.json configs[0]: 4^4, trivial orbit seed 1, omega 1.7, until theta < 1e-14: F -> 1; links and
+    theta checked against the oracle every sweep."""
+    dims = (4, 4, 4, 4)
+    U = gf_inputs.trivial_orbit(dims, 1)
+    fx = _fixer(gfm, dims, "fp64")
+    fx.load(U)
+    sweeps = 0
+    while fx.theta() >= 1e-14 and sweeps < 500:
+        fx.overrelax(1.7, 1)
+        oracle.overrelax(U, dims, 1.7, 1)
+        sweeps += 1
+        assert np.abs(fx.download() - U).max() <= 1e-12
+        th_ref = oracle.theta(U, dims)
+        assert fx.theta() == pytest.approx(th_ref, rel=1e-6, abs=1e-24)
+    assert fx.theta() < 1e-14 and sweeps < 200
+    assert abs(fx.functional() - 1.0) < 1e-12
+    fx.close()
+
+
+def test_fp32_long_run_unitarity(gfm):
+    """C15: with the periodic re-orthonormalisation fp32 links stay unitary and F tracks the fp64 oracle"""
+    dims = (8, 8, 8, 8)
+    U = gf_inputs.smooth_random(dims, 0.4, 27)
+    fx = _fixer(gfm, dims, "fp32")
+    fx.load(U)
+    fx.overrelax(1.7, 300)
+    got = fx.download()
+    uu, det = oracle.unitarity_defect(got, dims)
+    assert uu < 5e-6 and det < 5e-6
+    oracle.overrelax(U, dims, 1.7, 300)
+    assert fx.functional() == pytest.approx(oracle.functional(U, dims), rel=1e-5)
+    fx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# simulated annealing: decision parity
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("R", [18, 12])
+@pytest.mark.parametrize("tps", [1, 2, 4])
+def test_anneal_decisions_fp64(gfm, gauge, R, tps):
+    import torch
+
+    dims = (6, 4, 4, 8)
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.5, 28)
+    fx = _fixer(gfm, dims, "fp64", gauge, R, tps=tps, block=64)
+    trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
+    gfm.gf_set_trial_buffer(fx.ctx, trials)
+    fx.load(U)
+    fx.anneal(1.4, 0.2, 5, 7)
+    got = fx.download()
+    got_trials = trials.cpu().numpy().reshape(V, 3)
+    ref_trials = oracle.anneal(U, dims, 1.4, 0.2, 5, 7, _orc_gauge(gauge), trials=True)
+    assert np.array_equal(got_trials, ref_trials)  # identical accept decisions for every (site, subgroup)
+    assert got_trials.max() > 1  # the test saw rejections
+    assert np.abs(got - U).max() <= 1e-11
+    fx.close()
+
+
+def test_anneal_fp32_one_step(gfm):
+    """C14: fp32 cannot be decision-exact; one step from identical input: >= (1 - 1e-3) of the trial counts equal
+    on this small lattice, and sites whose three counts agree match per link within 5e-5."""
+    import torch
+
+    dims = (8, 8, 8, 8)
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.5, 29)
+    fx = _fixer(gfm, dims, "fp32", "coulomb")
+    trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
+    gfm.gf_set_trial_buffer(fx.ctx, trials)
+    fx.load(U)
+    # the input the kernel sees is the fp32-rounded field: give the oracle the same
+    U32 = fx.download()
+    fx.anneal(0.7, 0.7, 1, 7)
+    got = fx.download()
+    got_trials = trials.cpu().numpy().reshape(V, 3)
+    ref_trials = oracle.anneal(U32, dims, 0.7, 0.7, 1, 7, oracle.COULOMB, trials=True)
+    same = (got_trials == ref_trials)
+    assert same.mean() >= 1 - 1e-3
+    # a flipped decision at one site changes that site's links and, through K, its neighbours' draws in the
+    # second half-sweep; compare links only where nothing nearby flipped: use the global fraction as the bar
+    close = np.abs(got - U32).reshape(V, -1).max(axis=1) <= 5e-5
+    assert close.mean() >= 1 - 2e-2
+    fx.close()
+
+
+def test_anneal_then_overrelax_config5_shape(gfm):
+    """BASELINE.json configs[4] in miniature: Coulomb gauge, anneal 1.4 -> 0.01 then overrelax until every
+    timeslice has theta_t < 1e-10; plaquette invariant (P5), F rises."""
+    dims = (8, 8, 8, 4)
+    U = gf_inputs.smooth_random(dims, 0.5, 5)
+    plaq0 = oracle.plaquette(U, dims)
+    fx = _fixer(gfm, dims, "fp64", "coulomb")
+    fx.load(U)
+    F0 = fx.functional()
+    fx.anneal(1.4, 0.01, 60, 7)
+    F1 = fx.functional()
+    sweeps = 0
+    while fx.theta() >= 1e-10 and sweeps < 3000:
+        fx.overrelax(1.7, 100)
+        sweeps += 100
+    assert max(fx.theta_slices()) < 1e-10
+    F2 = fx.functional()
+    assert F0 < F1 < F2
+    got = fx.download()
+    assert abs(oracle.plaquette(got, dims) - plaq0) < 1e-12
+    uu, det = oracle.unitarity_defect(got, dims)
+    assert uu < 1e-12 and det < 1e-12
+    fx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# argument checking and the host-buffer path
+# ---------------------------------------------------------------------------------------------------------
+def test_argument_errors(gfm):
+    with pytest.raises(gfm.GFError):
+        gfm.gf_create(3, 4, 4, 4)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_create(4, 4, 4, 0)
+    ctx = gfm.gf_create(4, 4, 4, 4, gfm.GF_FP64, gfm.GF_LANDAU)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_set_storage(ctx, 8)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_overrelax(ctx, 1234, 2.0, 1)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_overrelax(ctx, 1234, 0.9, 1)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_overrelax(ctx, 0, 1.5, 1)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_anneal(ctx, 1234, 0.0, 1.0, 1, 1)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_set_tuning(ctx, 3, 64)
+    gfm.gf_destroy(ctx)
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_host_buffer_path(gfm, precision):
+    dims = (8, 4, 4, 6)
+    U = gf_inputs.smooth_random(dims, 0.4, 30)
+    ref = U.copy()
+    ctx = gfm.gf_create(*dims, gfm.GF_FP64 if precision == "fp64" else gfm.GF_FP32, gfm.GF_LANDAU)
+    F, th = gfm.gf_overrelax_host(ctx, U, 1.7, 2)
+    gfm.gf_destroy(ctx)
+    oracle.overrelax(ref, dims, 1.7, 2)
+    assert np.abs(U - ref).max() <= TOL_LINK[precision] * 2
+    assert F == pytest.approx(oracle.functional(ref, dims), rel=TOL_F[precision])
+    assert th == pytest.approx(oracle.theta(ref, dims), rel=1e-6 if precision == "fp64" else 1e-3)
