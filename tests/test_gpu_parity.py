@@ -52,7 +52,7 @@ def test_pack_unpack_roundtrip(gfm, precision, R, dims):
         assert np.array_equal(back, U)  # bit exact
     elif precision == "fp64":
         assert np.array_equal(back[:, :, :2], U[:, :, :2])  # stored rows bit exact
-        assert np.abs(back - U).max() < 1e-15  # row 2 rebuilt (C16)
+        assert np.abs(back - U).max() < 4e-15  # row 2 rebuilt (C16)
     else:
         ref = U.astype(np.complex64).astype(np.complex128)
         if R == 18:
