@@ -1,0 +1,438 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the gauge-fixing hot path on B200, one JSON line on stdout (rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A STEP is one pass of the whole path at the paper's cadence (F and theta are evaluated after every
+100th iteration): `--sweeps-per-step` (default 100) checkerboard overrelaxation sweeps (RED + BLACK half-sweeps,
+Alg. 1) at omega, then gf_functional and gf_theta with their scalar read-back.
+Metric: site-updates/s (one site-update = the full SU(3) update of one site: 3 SU(2) subgroups, 8 links);
+GFlop/s = site-updates/s x 2253 (paper flop model).
+
+Workloads (BASELINE.json configs; seeded synthetic fields, recipe in DESIGN.md "Inputs"):
+    32^4-f32-r18 (default, the headline config), 32^4-f32-r12, 32^4-f64-r18, 64^4-f64-r18, 64^4-f32-r18,
+    16^3x32-f32-r18, 16^3x32-f64-r18, 48^3x64-f32-r18-coulomb-anneal
+N > 1 (torchrun): the path does not shard on one GPU's problem ("replicas only"): every rank runs an
+independent replica of the workload on its own GPU, no data-path collective; value = all ranks' site-updates /
+max-over-ranks time.
+
+--impl reference times the fp64 CPU oracle (oracle/, as it stands) on the host cores on the same config.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 2253
+L2_BYTES = 126 * 2**20
+
+# name -> dims, precision, R, gauge, omega, generator (eps, seed), mode
+WORKLOADS = {
+    "32^4-f32-r18": dict(dims=(32, 32, 32, 32), precision="fp32", R=18, gauge="landau", omega=1.7, eps=0.4, seed=3),
+    "32^4-f32-r12": dict(dims=(32, 32, 32, 32), precision="fp32", R=12, gauge="landau", omega=1.7, eps=0.4, seed=3),
+    "32^4-f64-r18": dict(dims=(32, 32, 32, 32), precision="fp64", R=18, gauge="landau", omega=1.7, eps=0.4, seed=3),
+    "32^4-f64-r12": dict(dims=(32, 32, 32, 32), precision="fp64", R=12, gauge="landau", omega=1.7, eps=0.4, seed=3),
+    "64^4-f64-r18": dict(dims=(64, 64, 64, 64), precision="fp64", R=18, gauge="landau", omega=1.8, eps=0.4, seed=4),
+    "64^4-f32-r18": dict(dims=(64, 64, 64, 64), precision="fp32", R=18, gauge="landau", omega=1.8, eps=0.4, seed=4),
+    "16^3x32-f32-r18": dict(dims=(16, 16, 16, 32), precision="fp32", R=18, gauge="landau", omega=1.7, eps=0.3, seed=2),
+    "16^3x32-f64-r18": dict(dims=(16, 16, 16, 32), precision="fp64", R=18, gauge="landau", omega=1.7, eps=0.3, seed=2),
+    "48^3x64-f32-r18-coulomb": dict(dims=(48, 48, 48, 64), precision="fp32", R=18, gauge="coulomb", omega=1.7,
+                                    eps=0.5, seed=5),
+    "48^3x64-f32-r18-coulomb-anneal": dict(dims=(48, 48, 48, 64), precision="fp32", R=18, gauge="coulomb",
+                                           omega=1.7, eps=0.5, seed=5, anneal=True),
+}
+ALSO_DEFAULT = ["32^4-f32-r12", "32^4-f64-r18"]
+
+
+def volume(dims):
+    return dims[0] * dims[1] * dims[2] * dims[3]
+
+
+def model_bytes_per_site_update(R: int, precision: str) -> int:
+    """every half-sweep reads and writes every link once (C6): 16 R s bytes per site-update"""
+    return 16 * R * (8 if precision == "fp64" else 4)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------------------------
+# inputs: seeded synthetic fields from gf_inputs (host, canonical fp64).  Lattices above 32^4 sites are built
+# by generating the field of half the extents and repeating it twice per direction (still a periodic gauge
+# field of the same smoothness; keeps the default run's host time and memory bounded) -- named in `config`.
+# ---------------------------------------------------------------------------------------------------------
+def base_field(w):
+    import gf_inputs
+
+    dims = w["dims"]
+    tiled = volume(dims) > 32**4
+    gdims = tuple(d // 2 for d in dims) if tiled else dims
+    U = gf_inputs.smooth_random(gdims, w["eps"], w["seed"])
+    return U, gdims, tiled
+
+
+def device_canonical(U, gdims, dims, tiled):
+    """host canonical (numpy complex128 (V,4,3,3)) -> device float64 tensor of V*72 reals (tiled if asked)"""
+    import torch
+
+    t = torch.from_numpy(U.view("float64").reshape(-1)).to("cuda")
+    if tiled:
+        Nx, Ny, Nz, Nt = gdims
+        t = t.view(Nt, Nz, Ny, Nx, 72).repeat(2, 2, 2, 2, 1).contiguous().view(-1)
+    assert t.numel() == volume(dims) * 72
+    return t
+
+
+class ClockSampler:
+    """samples nvidia-smi clocks and throttle reasons while the timed region runs (B200_PROFILING.md)"""
+
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------------------
+def make_fixer(gfm, w, canon_dev):
+    fx = gfm.GaugeFixer(w["dims"], precision=w["precision"], gauge=w["gauge"], reals_per_link=w["R"])
+    gfm.gf_pack(fx.ctx, canon_dev, fx.U)
+    return fx
+
+
+def run_step(gfm, fx, w, sweeps, stream, ev=None):
+    """one step: `sweeps` sweeps, then F and theta with their read-back.  ev = (start, stop) CUDA events recorded
+    on `stream` around the sweep launches alone (roofline of the half-sweep kernel)."""
+    if ev is not None:
+        ev[0].record(stream)
+    if w.get("anneal"):
+        gfm.gf_anneal(fx.ctx, fx.U, 1.4, 0.01, sweeps, 7, stream)
+    else:
+        gfm.gf_overrelax(fx.ctx, fx.U, w["omega"], sweeps, stream)
+    if ev is not None:
+        ev[1].record(stream)
+    return gfm.gf_functional(fx.ctx, fx.U), gfm.gf_theta(fx.ctx, fx.U)
+
+
+def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler=None):
+    """W untimed steps, then K steps timed with CUDA events on the launching stream.
+    Returns (seconds for K steps, seconds inside the sweep launches, launches, last F, last theta, clocks)."""
+    import torch
+
+    for _ in range(warmup):
+        run_step(gfm, fx, w, sweeps, stream)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    if barrier is not None:
+        barrier()
+    if sampler is not None:
+        sampler.start()
+    launches0 = gfm.gf_launch_count(fx.ctx)
+    t0.record(stream)
+    for k in range(steps):
+        F, th = run_step(gfm, fx, w, sweeps, stream, evs[k])
+    t1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler is not None else None
+    if barrier is not None:
+        barrier()
+    total = t0.elapsed_time(t1) * 1e-3
+    in_sweeps = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    return total, in_sweeps, gfm.gf_launch_count(fx.ctx) - launches0, F, th, clocks
+
+
+def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None):
+    """dominant kernel = the half-sweep kernel: algorithmic bytes per launch = (V/2) * 16 R s"""
+    peak, which = measured_peaks()
+    per_launch_bytes = (volume(w["dims"]) // 2) * model_bytes_per_site_update(w["R"], w["precision"])
+    nlaunch = 2 * sweeps * steps
+    avg_s = in_sweeps_s / nlaunch
+    achieved = per_launch_bytes / avg_s / 1e9
+    return {"bound": "hbm", "kernel": "gf_half_sweep_kernel", "achieved": round(achieved, 1), "peak": peak,
+            "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": traffic,
+            "bytes_per_launch": per_launch_bytes, "avg_launch_us": round(avg_s * 1e6, 3), "peak_source": which,
+            "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
+
+
+def time_e2e(gfm, w, U_host_pinned, sweeps, steps, warmup):
+    """the host-buffer C-ABI call: H2D of the canonical field, pack, sweeps, F, theta, unpack, D2H -- all inside"""
+    import torch
+
+    prec = gfm.GF_FP64 if w["precision"] == "fp64" else gfm.GF_FP32
+    ctx = gfm.gf_create(*w["dims"], prec, gfm.GF_COULOMB if w["gauge"] == "coulomb" else gfm.GF_LANDAU)
+    gfm.gf_set_storage(ctx, w["R"])
+    for _ in range(warmup):
+        gfm.gf_overrelax_host(ctx, U_host_pinned, w["omega"], sweeps)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        gfm.gf_overrelax_host(ctx, U_host_pinned, w["omega"], sweeps)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    gfm.gf_destroy(ctx)
+    nbytes = volume(w["dims"]) * 72 * 8
+    return dt, nbytes, nbytes + 16
+
+
+def time_oracle(w, U, sweeps, reps):
+    """the oracle as it stands (gcc -O2 -fopenmp), fp64, on the host cores; returns seconds per repetition"""
+    import oracle
+
+    gauge = oracle.COULOMB if w["gauge"] == "coulomb" else oracle.LANDAU
+    dims = w["dims"]
+    oracle.overrelax(U, dims, w["omega"], 1, gauge)  # warm-up (page in, thread pool)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        oracle.overrelax(U, dims, w["omega"], sweeps, gauge)
+        oracle.functional(U, dims, gauge)
+        oracle.theta(U, dims, gauge)
+    return (time.perf_counter() - t0) / reps
+
+
+def oracle_sample_dims(w):
+    """bounded sample of the workload for the CPU legs: the same generator on a lattice of at most 16^3x32 sites"""
+    dims = w["dims"]
+    if volume(dims) <= 16 * 16 * 16 * 32:
+        return dims
+    return (16, 16, 16, 32)
+
+
+def main_reference(args, w, rank):
+    """--impl reference: the oracle timed on the host cores, same config / metric / unit (rank 0 only)"""
+    if rank != 0:
+        return
+    import gf_inputs
+    import oracle
+
+    sdims = oracle_sample_dims(w)
+    ws = dict(w, dims=sdims)
+    U = gf_inputs.smooth_random(sdims, w["eps"], w["seed"])
+    sweeps = args.ref_sweeps
+    for _ in range(args.warmup):
+        time_oracle(ws, U, sweeps, 1)
+    sec = time_oracle(ws, U, sweeps, args.steps)
+    cores = oracle.max_threads()
+    value = volume(sdims) * sweeps / sec
+    sample = (f"{sweeps} sweeps + F + theta per step on a {'x'.join(map(str, sdims))} lattice from the same "
+              f"generator (eps={w['eps']}, seed={w['seed']}), fp64")
+    line = {
+        "impl": "reference", "metric": "site-updates/s", "value": value, "unit": "site-updates/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "gflops_paper_model": value * FLOP_PER_SITE / 1e9,
+        "cpu_baseline": {"value": value, "unit": "site-updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="32^4-f32-r18", choices=sorted(WORKLOADS))
+    ap.add_argument("--sweeps-per-step", type=int, default=100)
+    ap.add_argument("--ref-sweeps", type=int, default=5, help="sweeps per step of the --impl reference arm")
+    ap.add_argument("--also", default=",".join(ALSO_DEFAULT), help="comma list of further workloads timed after "
+                    "the main one and reported under 'also' ('' = none)")
+    ap.add_argument("--tps", type=int, default=0, help="threads per site override (0 = library default)")
+    ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"),
+                    help="ncu dram bytes per launch per workload, written from profiles/ (optional)")
+    args = ap.parse_args()
+    w = WORKLOADS[args.workload]
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        main_reference(args, w, rank)
+        return
+
+    import torch
+    import paper_1209_4008_b200 as gfm
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path (use --impl reference for the oracle)")
+    gfm.load_library()
+    torch.cuda.set_device(local_rank)
+    barrier = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        barrier = dist.barrier
+    stream = torch.cuda.Stream()
+    sweeps, steps, warmup = args.sweeps_per_step, args.steps, max(args.warmup, 3)
+
+    traffic = {}
+    if os.path.exists(args.traffic_json):
+        with open(args.traffic_json) as fh:
+            traffic = json.load(fh)
+
+    def measure(name, wl, sampler=None, bar=None):
+        U, gdims, tiled = base_field(wl)
+        canon = device_canonical(U, gdims, wl["dims"], tiled)
+        fx = make_fixer(gfm, wl, canon)
+        gfm.gf_set_tuning(fx.ctx, args.tps, args.block)
+        del canon
+        torch.cuda.synchronize()
+        total, in_sw, launches, F, th, clocks = time_device(gfm, fx, wl, sweeps, steps, warmup, stream, bar, sampler)
+        regs, spill = gfm.gf_kernel_info(fx.ctx, 1 if wl.get("anneal") else 0)
+        fx.close()
+        return dict(U=U if not tiled else None, total=total, in_sweeps=in_sw, launches=launches, F=F, theta=th,
+                    clocks=clocks, regs=regs, spill=spill, tiled=tiled, gdims=gdims,
+                    roofline=roofline_entry(wl, sweeps, steps, in_sw, traffic.get(name)))
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    m = measure(args.workload, w, sampler, barrier)
+    total = m["total"]
+    if world > 1:
+        tt = torch.tensor([total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total = float(tt.item())
+    V = volume(w["dims"])
+    value = world * V * sweeps * steps / total
+
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+
+    # ---- rank 0, N = 1 extras: end-to-end through the host-buffer call, further workloads, the CPU baseline ----
+    e2e = None
+    if not args.no_e2e and not w.get("anneal"):
+        U = m["U"] if m["U"] is not None else base_field(dict(w, dims=m["gdims"]))[0]
+        if m["tiled"]:
+            import numpy as np
+
+            Nx, Ny, Nz, Nt = m["gdims"]
+            U = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(-1, 4, 3, 3)
+        host = torch.from_numpy(U.view("float64").reshape(-1)).pin_memory()
+        e_steps = max(1, min(steps, 5))
+        dt, h2d, d2h = time_e2e(gfm, w, host, sweeps, e_steps, 1)
+        e2e = {"value": world * V * sweeps * e_steps / dt, "unit": "site-updates/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": e_steps, "ms_per_step": dt / e_steps * 1e3,
+               "call": "gf_overrelax_host (canonical fp64 field in pinned host memory in, fixed field + F + theta out)"}
+        del host
+
+    also = []
+    for name in [n for n in args.also.split(",") if n and n != args.workload]:
+        wl = WORKLOADS[name]
+        a = measure(name, wl)
+        Va = volume(wl["dims"])
+        va = Va * sweeps * steps / a["total"]
+        also.append({"workload": name, "value": va, "unit": "site-updates/s", "gflops_paper_model": va * FLOP_PER_SITE / 1e9,
+                     "ms_per_step": a["total"] / steps * 1e3, "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
+                     "regs_per_thread": a["regs"], "spill_bytes": a["spill"]})
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        import gf_inputs
+        import oracle
+
+        sdims = oracle_sample_dims(w)
+        ws = dict(w, dims=sdims)
+        Us = gf_inputs.smooth_random(sdims, w["eps"], w["seed"])
+        probe = time_oracle(ws, Us, 1, 1)
+        n = max(1, min(200, int(15.0 / max(probe, 1e-3))))  # about 15 s of CPU work
+        sec = time_oracle(ws, Us, n, 1)
+        cpu = {"value": volume(sdims) * n / sec, "unit": "site-updates/s", "cores": oracle.max_threads(), "kind": "oracle",
+               "sample": f"{n} sweeps + F + theta on a {'x'.join(map(str, sdims))} lattice from the same generator "
+                         f"(eps={w['eps']}, seed={w['seed']}), fp64, gcc -O2 -fopenmp"}
+
+    field_bytes = 4 * V * w["R"] * (8 if w["precision"] == "fp64" else 4)
+    line = {
+        "metric": "site-updates/s", "value": value, "unit": "site-updates/s", "n_gpus": world, "steps": steps,
+        "warmup": warmup, "ms_per_step": total / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64" if w["precision"] == "fp64" else "f32", "data": "synthetic",
+        "config": {
+            "workload": args.workload, "dims": list(w["dims"]), "gauge": w["gauge"], "reals_per_link": w["R"],
+            "omega": w["omega"], "step": f"{sweeps} {'annealing' if w.get('anneal') else 'overrelaxation'} sweeps + "
+                                         "gf_functional + gf_theta",
+            "input": f"smooth-random eps={w['eps']} seed={w['seed']}" + (" on half extents, repeated 2x per direction"
+                                                                          if m["tiled"] else ""),
+            "l2": f"inputs larger than L2: field {field_bytes / 2**20:.0f} MiB vs 126 MiB L2, no flush"
+                  if field_bytes > L2_BYTES else f"field {field_bytes / 2**20:.0f} MiB fits L2 (126 MiB): not a bandwidth figure",
+            "parallelism": "replicas only" if world > 1 else "single GPU",
+        },
+        "gflops_paper_model": value * FLOP_PER_SITE / 1e9,
+        "paper_context": "300 GFlops on GTX 580 (PAPER.md:13), another machine: context, not the target",
+        "F": m["F"], "theta": m["theta"],
+        "regs_per_thread": m["regs"], "spill_bytes": m["spill"],
+        "roofline": m["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
+        "clocks": m["clocks"], "also": also,
+    }
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()
