@@ -112,8 +112,8 @@ int gf_overrelax_host(gf_ctx* ctx, double* U_canon_host, double omega, int nswee
 
 /* Launch shape of the sweep kernels: threads_per_site in {1,2,4} (1: one thread holds all 8 links of a site;
  * 2: two threads hold the links of 2 directions each; 4: one direction each; partial K summed by warp
- * shuffles), block = threads per block (multiple of 32, <= 256).  0 keeps the current value.  Defaults are
- * chosen per precision from the ncu measurements in profiles/. */
+ * shuffles), block = threads per block (multiple of 32, <= 256).  0 = automatic (the default): chosen per
+ * (precision, storage) from the measurements in profiles/. */
 int gf_set_tuning(gf_ctx* ctx, int threads_per_site, int block);
 /* fp32 unitarity policy (C15): every `every`-th sweep the RED half-sweep re-orthonormalises rows 0,1 of each
  * link on load (and rebuilds row 2).  0 = never.  Default: 16 for fp32, 0 for fp64. */
@@ -121,6 +121,13 @@ int gf_set_reunit(gf_ctx* ctx, int every);
 /* Alternate the block traversal direction between consecutive half-sweeps so that the tail of one
  * half-sweep, still in L2, is what the next one reads first (1 = on, default; 0 = off). */
 int gf_set_l2_reversal(gf_ctx* ctx, int on);
+/* L2 eviction policy of the link accesses of the sweep kernels: 0 = normal, 1 = evict first, 2 = evict last.
+ * Default (0, 2): loads keep the normal policy, stores ask L2 to keep
+ * the freshly written lines, which the next half-sweep (traversing in the opposite direction) reads first. */
+int gf_set_l2_policy(gf_ctx* ctx, int load_policy, int store_policy);
+/* Programmatic dependent launch of consecutive half-sweeps (1 = on, default): the next half-sweep's grid becomes
+ * resident while the current one drains and waits on the device before it touches the field. */
+int gf_set_pdl(gf_ctx* ctx, int on);
 /* Optional debug output of gf_anneal: d_trials (device, V*3 unsigned, index 3*s + subgroup) receives the
  * number of Kennedy-Pendleton trials of every (site, subgroup) of the LAST step; NULL switches it off. */
 int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);

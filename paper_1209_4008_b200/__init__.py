@@ -45,6 +45,8 @@ SIGNATURES = {
     "gf_set_tuning": (_i, [_vp, _i, _i]),
     "gf_set_reunit": (_i, [_vp, _i]),
     "gf_set_l2_reversal": (_i, [_vp, _i]),
+    "gf_set_l2_policy": (_i, [_vp, _i, _i]),
+    "gf_set_pdl": (_i, [_vp, _i]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
     "gf_launch_count": (_ull, [_vp]),
     "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
@@ -179,6 +181,14 @@ def gf_set_reunit(ctx, every: int) -> None:
 
 def gf_set_l2_reversal(ctx, on: bool) -> None:
     _check(ctx, load_library().gf_set_l2_reversal(ctx, int(bool(on))))
+
+
+def gf_set_l2_policy(ctx, load_policy: int, store_policy: int) -> None:
+    _check(ctx, load_library().gf_set_l2_policy(ctx, int(load_policy), int(store_policy)))
+
+
+def gf_set_pdl(ctx, on: bool) -> None:
+    _check(ctx, load_library().gf_set_pdl(ctx, int(bool(on))))
 
 
 def gf_set_trial_buffer(ctx, d_trials) -> None:

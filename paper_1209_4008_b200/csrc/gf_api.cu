@@ -18,6 +18,8 @@ struct gf_ctx {
     int tps, block;
     int reunit_every;
     int l2_reversal;
+    int ld_policy, st_policy;         // L2 eviction policy of the sweep's link loads / stores
+    int pdl;                          // programmatic dependent launch of consecutive half-sweeps
     unsigned long long sweeps_done;   // overrelaxation sweeps since creation (cadence of the fp32 reunitarisation)
     unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
     unsigned long long launches;
@@ -78,11 +80,12 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->Nx = Nx; c->Ny = Ny; c->Nz = Nz; c->Nt = Nt;
     c->precision = precision; c->gauge = gauge; c->R = 18;
     c->L.Nxh = Nx / 2; c->L.Ny = Ny; c->L.Nz = Nz; c->L.Nt = Nt; c->L.H = (unsigned)(V / 2);
-    // launch shape chosen from the measurements in profiles/ 
-    c->tps = precision == GF_FP64 ? 4 : 1;
-    c->block = 64;
+    c->tps = 0;   // 0 = automatic: resolved per (precision, storage, mode) by auto_tps()
+    c->block = 0; // 0 = automatic
     c->reunit_every = precision == GF_FP32 ? 16 : 0;
     c->l2_reversal = 1;
+    c->ld_policy = POLICY_NORMAL; c->st_policy = POLICY_EVICT_LAST; // measured best: profiles/r1_variants.md
+    c->pdl = 1;
     c->sweeps_done = 0; c->half_sweeps = 0; c->launches = 0;
     c->d_trials = nullptr; c->last_stream = nullptr;
     c->d_canon = nullptr; c->d_native = nullptr;
@@ -132,8 +135,8 @@ extern "C" int gf_set_tuning(gf_ctx* c, int tps, int block)
     if (c == nullptr) return GF_EINVAL;
     if (tps != 0 && tps != 1 && tps != 2 && tps != 4) return fail(c, GF_EINVAL, "gf_set_tuning: threads_per_site must be 1, 2 or 4");
     if (block != 0 && (block < 32 || block > MAX_BLOCK || block % 32)) return fail(c, GF_EINVAL, "gf_set_tuning: block must be a multiple of 32 in [32, %d]", MAX_BLOCK);
-    if (tps) c->tps = tps;
-    if (block) c->block = block;
+    c->tps = tps;     // 0 returns to the automatic choice
+    c->block = block;
     return GF_OK;
 }
 
@@ -152,6 +155,23 @@ extern "C" int gf_set_l2_reversal(gf_ctx* c, int on)
     return GF_OK;
 }
 
+extern "C" int gf_set_l2_policy(gf_ctx* c, int load_policy, int store_policy)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (load_policy < 0 || load_policy > 2 || store_policy < 0 || store_policy > 2)
+        return fail(c, GF_EINVAL, "gf_set_l2_policy: policies must be 0 (normal), 1 (evict first) or 2 (evict last)");
+    c->ld_policy = load_policy;
+    c->st_policy = store_policy;
+    return GF_OK;
+}
+
+extern "C" int gf_set_pdl(gf_ctx* c, int on)
+{
+    if (c == nullptr) return GF_EINVAL;
+    c->pdl = on ? 1 : 0;
+    return GF_OK;
+}
+
 extern "C" int gf_set_trial_buffer(gf_ctx* c, unsigned* d_trials)
 {
     if (c == nullptr) return GF_EINVAL;
@@ -161,10 +181,24 @@ extern "C" int gf_set_trial_buffer(gf_ctx* c, unsigned* d_trials)
 
 extern "C" unsigned long long gf_launch_count(const gf_ctx* c) { return c ? c->launches : 0ull; }
 
+// Launch shape chosen from the measurements in profiles/ (DESIGN.md "Kernels"): the kernel is latency/bandwidth
+// bound and wants as many bytes in flight per SM as the register file allows -- few, fat threads in one-warp
+// blocks.  fp32 R18: one thread per site (8 links = 144 reals in registers); fp32 R12 and fp64: two threads per
+// site (forward+backward links of two directions each), K combined with one warp shuffle.
+static int auto_tps(const gf_ctx* c, int mode)
+{
+    if (c->tps) return c->tps;
+    (void)mode;
+    if (c->precision == GF_FP64) return 2;
+    return c->R == 18 ? 1 : 2;
+}
+static int auto_block(const gf_ctx* c) { return c->block ? c->block : 32; }
+
 static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p, cudaStream_t st)
 {
-    if (c->precision == GF_FP32) return c->R == 18 ? launch_sweep_f32_r18(c->tps, mode, c->block, p, st) : launch_sweep_f32_r12(c->tps, mode, c->block, p, st);
-    return c->R == 18 ? launch_sweep_f64_r18(c->tps, mode, c->block, p, st) : launch_sweep_f64_r12(c->tps, mode, c->block, p, st);
+    const int tps = auto_tps(c, mode), block = auto_block(c);
+    if (c->precision == GF_FP32) return c->R == 18 ? launch_sweep_f32_r18(tps, mode, block, p, st) : launch_sweep_f32_r12(tps, mode, block, p, st);
+    return c->R == 18 ? launch_sweep_f64_r18(tps, mode, block, p, st) : launch_sweep_f64_r12(tps, mode, block, p, st);
 }
 
 extern "C" int gf_kernel_info(gf_ctx* c, int mode, int* regs, int* local_bytes)
@@ -173,8 +207,9 @@ extern "C" int gf_kernel_info(gf_ctx* c, int mode, int* regs, int* local_bytes)
     if (mode != 0 && mode != 1) return fail(c, GF_EINVAL, "gf_kernel_info: mode must be 0 or 1");
     cudaFuncAttributes a;
     cudaError_t e;
-    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(c->tps, mode, &a) : sweep_attributes_f32_r12(c->tps, mode, &a);
-    else e = c->R == 18 ? sweep_attributes_f64_r18(c->tps, mode, &a) : sweep_attributes_f64_r12(c->tps, mode, &a);
+    const int tps = auto_tps(c, mode);
+    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(tps, mode, &a) : sweep_attributes_f32_r12(tps, mode, &a);
+    else e = c->R == 18 ? sweep_attributes_f64_r18(tps, mode, &a) : sweep_attributes_f64_r12(tps, mode, &a);
     if (e != cudaSuccess) return cuda_fail(c, e, "gf_kernel_info");
     if (regs) *regs = a.numRegs;
     if (local_bytes) *local_bytes = (int)a.localSizeBytes;
@@ -190,6 +225,9 @@ static SweepParams base_params(gf_ctx* c, void* U)
     p.nd = c->gauge == GF_COULOMB ? 3 : 4;
     p.omega = 1.0;
     p.T = 1.0;
+    p.ld_policy = c->ld_policy;
+    p.st_policy = c->st_policy;
+    p.pdl = c->pdl;
     return p;
 }
 

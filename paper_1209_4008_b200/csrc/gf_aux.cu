@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, const double
     cx<T> u[9];
 #pragma unroll
     for (int e = 0; e < 9; ++e) u[e] = {(T)src[2 * e], (T)src[2 * e + 1]};
-    LinkIO<T, R>::store(native + (size_t)l * R * L.H, L.H, h, u);
+    LinkIO<T, R>::store(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
 }
 
 template <typename T, int R>
@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* _
     const int l = (int)(gid / L.H), parity = l >> 2, mu = l & 3;
     const Site s = decode_site(L, h, parity);
     cx<T> u[9];
-    LinkIO<T, R>::load(native + (size_t)l * R * L.H, L.H, h, u);
+    LinkIO<T, R>::load(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
     double* dst = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
 #pragma unroll
     for (int e = 0; e < 9; ++e) { dst[2 * e] = (double)u[e].re; dst[2 * e + 1] = (double)u[e].im; }
@@ -100,11 +100,12 @@ __global__ void __launch_bounds__(AUX_BLOCK) functional_kernel(Lattice L, int nd
     const unsigned local = blockIdx.x * blockDim.x + threadIdx.x;
     const int t = blockIdx.y >> 1, parity = blockIdx.y & 1;
     double acc = 0.0;
+    const uint64_t pol = make_l2_policy(POLICY_NORMAL);
     if (local < Hs) {
         const unsigned h = (unsigned)t * Hs + local;
         for (int mu = 0; mu < nd; ++mu) {
             cx<T> u[9];
-            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, h, u);
+            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, h, u, pol);
             acc += (double)u[0].re + (double)u[4].re + (double)u[8].re;
         }
     }
@@ -121,6 +122,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) theta_kernel(Lattice L, int nd, con
     const unsigned local = blockIdx.x * blockDim.x + threadIdx.x;
     const int t = blockIdx.y >> 1, parity = blockIdx.y & 1;
     double acc = 0.0;
+    const uint64_t pol = make_l2_policy(POLICY_NORMAL);
     if (local < Hs) {
         const Site s = decode_site(L, (unsigned)t * Hs + local, parity);
         cx<double> K[9];
@@ -128,8 +130,8 @@ __global__ void __launch_bounds__(AUX_BLOCK) theta_kernel(Lattice L, int nd, con
         for (int e = 0; e < 9; ++e) K[e] = {0.0, 0.0};
         for (int mu = 0; mu < nd; ++mu) {
             cx<T> f[9], b[9];
-            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, s.h, f);
-            LinkIO<T, R>::load(native + (size_t)((1 - parity) * 4 + mu) * R * L.H, L.H, backward_neighbour(L, s, mu), b);
+            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, s.h, f, pol);
+            LinkIO<T, R>::load(native + (size_t)((1 - parity) * 4 + mu) * R * L.H, L.H, backward_neighbour(L, s, mu), b, pol);
 #pragma unroll
             for (int r = 0; r < 3; ++r)
 #pragma unroll

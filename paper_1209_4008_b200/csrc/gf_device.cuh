@@ -123,62 +123,110 @@ __device__ __forceinline__ void su2_project(const cx<T> (&K)[9], T (&k)[4])
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// native layout access
+// native layout access.  Every access is one 128-bit (fp32 R18 tail plane: 64-bit) vector per thread with an
+// explicit L2 cache policy (createpolicy + .L2::cache_hint): within a half-sweep every link is read exactly
+// once and written exactly once (C6), so loads are streaming (L1 no-allocate, L2 evict-first by default) while
+// stores may ask L2 to keep the line (evict-last) for the next half-sweep, which starts where this one ended
+// (gf_set_l2_reversal).  DESIGN.md "Kernels / L2 policy".
 // ---------------------------------------------------------------------------------------------------------
+enum { POLICY_NORMAL = 0, POLICY_EVICT_FIRST = 1, POLICY_EVICT_LAST = 2 };
+
+__device__ __forceinline__ uint64_t make_l2_policy(int kind)
+{
+    uint64_t p;
+    if (kind == POLICY_EVICT_FIRST) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else if (kind == POLICY_EVICT_LAST) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+struct MemPolicy {
+    uint64_t ld, st;
+};
+
+__device__ __forceinline__ float4 ldg(const float4* p, uint64_t pol)
+{
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float2 ldg(const float2* p, uint64_t pol)
+{
+    float2 v;
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 ldg(const double2* p, uint64_t pol)
+{
+    double2 v;
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void stg(float4* p, float4 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;"
+                 :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void stg(float2* p, float2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1,%2}, %3;" :: "l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void stg(double2* p, double2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
 template <typename T, int R> struct LinkIO;
 
 template <int R>
 struct LinkIO<double, R> {
     static constexpr int NE = R / 2;
     // blk: first real of the link block; H: sites per parity; h: half-site index
-    static __device__ __forceinline__ void load(const double* __restrict__ blk, size_t H, size_t h,
-                                                cx<double> (&u)[9])
+    static __device__ __forceinline__ void load(const double* blk, size_t H, size_t h, cx<double> (&u)[9], uint64_t pol)
     {
         const double2* p = reinterpret_cast<const double2*>(blk) + h;
 #pragma unroll
         for (int e = 0; e < NE; ++e) {
-            double2 v = p[(size_t)e * H];
+            double2 v = ldg(p + (size_t)e * H, pol);
             u[e] = {v.x, v.y};
         }
         if (R == 12) rebuild_row2(u);
     }
-    static __device__ __forceinline__ void store(double* __restrict__ blk, size_t H, size_t h,
-                                                 const cx<double> (&u)[9])
+    static __device__ __forceinline__ void store(double* blk, size_t H, size_t h, const cx<double> (&u)[9], uint64_t pol)
     {
         double2* p = reinterpret_cast<double2*>(blk) + h;
 #pragma unroll
-        for (int e = 0; e < NE; ++e) p[(size_t)e * H] = make_double2(u[e].re, u[e].im);
+        for (int e = 0; e < NE; ++e) stg(p + (size_t)e * H, make_double2(u[e].re, u[e].im), pol);
     }
 };
 
 template <int R>
 struct LinkIO<float, R> {
     static constexpr int NQ = R / 4; // float4 planes: 4 (R18) or 3 (R12)
-    static __device__ __forceinline__ void load(const float* __restrict__ blk, size_t H, size_t h,
-                                                cx<float> (&u)[9])
+    static __device__ __forceinline__ void load(const float* blk, size_t H, size_t h, cx<float> (&u)[9], uint64_t pol)
     {
         const float4* p = reinterpret_cast<const float4*>(blk) + h;
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
-            float4 v = p[(size_t)q * H];
+            float4 v = ldg(p + (size_t)q * H, pol);
             u[2 * q] = {v.x, v.y};
             u[2 * q + 1] = {v.z, v.w};
         }
         if (R == 18) {
-            float2 v = reinterpret_cast<const float2*>(blk + 16 * H)[h];
+            float2 v = ldg(reinterpret_cast<const float2*>(blk + 16 * H) + h, pol);
             u[8] = {v.x, v.y};
         } else {
             rebuild_row2(u);
         }
     }
-    static __device__ __forceinline__ void store(float* __restrict__ blk, size_t H, size_t h,
-                                                 const cx<float> (&u)[9])
+    static __device__ __forceinline__ void store(float* blk, size_t H, size_t h, const cx<float> (&u)[9], uint64_t pol)
     {
         float4* p = reinterpret_cast<float4*>(blk) + h;
 #pragma unroll
         for (int q = 0; q < NQ; ++q)
-            p[(size_t)q * H] = make_float4(u[2 * q].re, u[2 * q].im, u[2 * q + 1].re, u[2 * q + 1].im);
-        if (R == 18) reinterpret_cast<float2*>(blk + 16 * H)[h] = make_float2(u[8].re, u[8].im);
+            stg(p + (size_t)q * H, make_float4(u[2 * q].re, u[2 * q].im, u[2 * q + 1].re, u[2 * q + 1].im), pol);
+        if (R == 18) stg(reinterpret_cast<float2*>(blk + 16 * H) + h, make_float2(u[8].re, u[8].im), pol);
     }
 };
 

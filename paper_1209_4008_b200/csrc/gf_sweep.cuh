@@ -25,6 +25,9 @@ struct SweepParams {
     int nd;         // directions entering K: 4 (Landau) or 3 (Coulomb, C12)
     int reunit;     // re-orthonormalise links on load (C15)
     int reverse;    // traverse blocks back to front (L2 reuse between consecutive half-sweeps)
+    int ld_policy;  // L2 policy of the link loads / stores (POLICY_*, gf_device.cuh)
+    int st_policy;
+    int pdl;        // launched with programmatic stream serialization: wait for the previous grid before loading
     double omega;   // overrelaxation parameter
     double T;       // heatbath temperature (C13)
     uint32_t key0, key1, step; // Philox key = seed, step = annealing step (C14)
@@ -172,15 +175,24 @@ struct SweepKernel {
         const size_t H = p.L.H;
         T* const base = reinterpret_cast<T*>(p.U);
 
+        const MemPolicy pol = {make_l2_policy(p.ld_policy), make_l2_policy(p.st_policy)};
         cx<T> F[NMU][9], B[NMU][9];
         unsigned hb[NMU];
+#pragma unroll
+        for (int m = 0; m < NMU; ++m) hb[m] = backward_neighbour(p.L, s, lane_mu0 + m);
+        // Programmatic dependent launch: this grid may become resident while the previous half-sweep drains
+        // (its index arithmetic above overlaps that tail); links are touched only after the previous grid
+        // has completed and flushed.  Letting the next grid launch early is always safe for the same reason.
+        if (p.pdl) {
+            cudaTriggerProgrammaticLaunchCompletion();
+            cudaGridDependencySynchronize();
+        }
         // issue every load before the first use
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
             const int mu = lane_mu0 + m;
-            hb[m] = backward_neighbour(p.L, s, mu);
-            IO::load(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m]);
-            IO::load(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m]);
+            IO::load(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.ld);
+            IO::load(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.ld);
         }
         if (p.reunit) {
 #pragma unroll
@@ -221,8 +233,8 @@ struct SweepKernel {
 #pragma unroll
             for (int m = 0; m < NMU; ++m) {
                 const int mu = lane_mu0 + m;
-                IO::store(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m]);
-                IO::store(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m]);
+                IO::store(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.st);
+                IO::store(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.st);
             }
         }
     }

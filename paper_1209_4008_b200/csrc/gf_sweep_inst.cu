@@ -45,8 +45,23 @@ cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParam
     if (fn == nullptr || block <= 0 || block > MAX_BLOCK || (block % 32) != 0) return cudaErrorInvalidValue;
     const unsigned long long threads = (unsigned long long)p.L.H * (unsigned long long)tps;
     const unsigned grid = (unsigned)((threads + (unsigned)block - 1ull) / (unsigned)block);
-    fn<<<grid, block, 0, stream>>>(p);
-    return cudaGetLastError();
+    if (!p.pdl) {
+        fn<<<grid, block, 0, stream>>>(p);
+        return cudaGetLastError();
+    }
+    // programmatic dependent launch: the grid may start while the previous kernel on the stream drains; the
+    // kernel itself waits (cudaGridDependencySynchronize) before it touches the field
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, fn, p);
 }
 
 cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, cudaFuncAttributes* attr)
