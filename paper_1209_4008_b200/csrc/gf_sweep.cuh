@@ -39,24 +39,26 @@ struct SweepParams {
 // second order and reprojection (reading C9):
 //   g = (k0,-k1,-k2,-k3)/|k|;  d = g0 - 1;  h0 = 1 + w d (1 + (w-1) g0);  hvec = w (1 + (w-1) d) gvec;  h /= |h|
 // ---------------------------------------------------------------------------------------------------------
+// Guards (C9) on the squared norms: |k|^2 below TinySq<T> takes G = 1 (the CPU oracle tests |k| < 1e-300; the
+// two differ only for |k| in [1e-300, 1e-150), fp32 [.., 1e-18) -- DESIGN.md "Differences").
 template <typename T> struct Tiny;
-template <> struct Tiny<float> { static constexpr float n = 1e-30f; };
-template <> struct Tiny<double> { static constexpr double n = 1e-300; };
+template <> struct Tiny<float> { static constexpr float n = 1e-30f; static constexpr float sq = 1e-36f; };
+template <> struct Tiny<double> { static constexpr double n = 1e-300; static constexpr double sq = 1e-300; };
 
 template <typename T>
 __device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[4])
 {
-    T n = gf_sqrt<T>(k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3]);
-    if (n < Tiny<T>::n) { h[0] = T(1); h[1] = h[2] = h[3] = T(0); return; }
-    T inv = T(1) / n;
-    T g0 = k[0] * inv, g1 = -k[1] * inv, g2 = -k[2] * inv, g3 = -k[3] * inv;
-    T d = g0 - T(1);
-    T h0 = T(1) + w * d * (T(1) + (w - T(1)) * g0);
-    T f = w * (T(1) + (w - T(1)) * d);
-    T h1 = f * g1, h2 = f * g2, h3 = f * g3;
-    T n2 = h0 * h0 + h1 * h1 + h2 * h2 + h3 * h3;
+    const T n2k = dot4(k[0], k[0], k[1], k[1], k[2], k[2], k[3], k[3]);
+    if (!(n2k >= Tiny<T>::sq)) { h[0] = T(1); h[1] = h[2] = h[3] = T(0); return; }
+    const T inv = gf_rsqrt<T>(n2k);
+    const T g0 = k[0] * inv, g1 = -k[1] * inv, g2 = -k[2] * inv, g3 = -k[3] * inv;
+    const T d = g0 - T(1);
+    const T h0 = T(1) + w * d * (T(1) + (w - T(1)) * g0);
+    const T f = w * (T(1) + (w - T(1)) * d);
+    const T h1 = f * g1, h2 = f * g2, h3 = f * g3;
+    const T n2 = dot4(h0, h0, h1, h1, h2, h2, h3, h3);
     if (n2 < T(1e-20)) { h[0] = g0; h[1] = g1; h[2] = g2; h[3] = g3; return; }
-    T hn = gf_rsqrt<T>(n2);
+    const T hn = gf_rsqrt<T>(n2);
     h[0] = h0 * hn; h[1] = h1 * hn; h[2] = h2 * hn; h[3] = h3 * hn;
 }
 
