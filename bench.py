@@ -303,8 +303,9 @@ def main():
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"),
-                    help="ncu dram bytes per launch per workload, written from profiles/ (optional)")
+    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r1_traffic.csv"),
+                    help="ncu dram__bytes_read.sum / dram__bytes_write.sum per launch of the half-sweep kernel, per "
+                         "workload, from one `ncu --set full` capture (profiles/r1_ncu_half_sweep.md)")
     args = ap.parse_args()
     w = WORKLOADS[args.workload]
 
@@ -333,9 +334,14 @@ def main():
     sweeps, steps, warmup = args.sweeps_per_step, args.steps, max(args.warmup, 3)
 
     traffic = {}
-    if os.path.exists(args.traffic_json):
-        with open(args.traffic_json) as fh:
-            traffic = json.load(fh)
+    if os.path.exists(args.traffic_csv):
+        import csv
+
+        acc = {}
+        with open(args.traffic_csv) as fh:
+            for row in csv.DictReader(fh):
+                acc.setdefault(row["workload"], []).append(float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]))
+        traffic = {k: int(sum(v) / len(v)) for k, v in acc.items()}
 
     def measure(name, wl, sampler=None, bar=None):
         U, gdims, tiled = base_field(wl)
