@@ -153,9 +153,11 @@ def site_overrelax(U, dims, s: int, omega: float, gauge: int = LANDAU) -> None:
     _load().orc_site_overrelax(N, gauge, _field(U, V), int(s), float(omega))
 
 
-def site_heatbath(U, dims, s: int, T: float, seed: int, step: int, gauge: int = LANDAU) -> np.ndarray:
+def site_heatbath(U, dims, s: int, T: float, seed: int, step: int, gauge: int = LANDAU, buf=None) -> np.ndarray:
+    """buf: optional (V, 3) int32 scratch for the trial counts, reused between calls on large lattices"""
     N, V = _dims(dims)
-    tr = np.zeros((V, 3), dtype=np.int32)
+    tr = np.zeros((V, 3), dtype=np.int32) if buf is None else buf
+    assert tr.shape == (V, 3) and tr.dtype == np.int32 and tr.flags.c_contiguous
     _load().orc_site_heatbath(N, gauge, _field(U, V), int(s), float(T), int(seed), int(step), tr.ctypes.data)
     return tr[s].copy()
 
