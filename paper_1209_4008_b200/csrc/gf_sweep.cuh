@@ -75,44 +75,72 @@ template <> struct KPMath<double> {
     static __device__ __forceinline__ double neglog(double u) { return -log(u); }
     // delta = (-ln u1 / alpha) cos^2 + (-ln u2 / alpha), in exactly this order, no FMA contraction: this
     // value decides acceptance and must follow the stated recipe operation by operation (C14)
-    static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha)
+    static __device__ __forceinline__ double inv(double) { return 0.0; } // unused: the fp64 draw divides (C14)
+    static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha, double)
     {
         return __dadd_rn(__dmul_rn(__ddiv_rn(l1, alpha), __dmul_rn(c, c)), __ddiv_rn(l2, alpha));
     }
     static __device__ __forceinline__ bool accept(double u4, double d) { return __dmul_rn(u4, u4) <= __dsub_rn(1.0, __dmul_rn(0.5, d)); }
 };
+// fp32: decision parity with the fp64 oracle cannot be exact (alpha itself differs at 1e-7, C14), so the draw uses
+// the SFU: u from the mantissa trick (exact), -ln u = -ln2 * lg2(u) (MUFU.LG2, abs. error ~4e-7), cos/sin by
+// MUFU.COS/SIN (abs. error ~5e-7), one reciprocal of alpha per subgroup instead of two divisions per trial.
+// A decision flips when u4^2 falls within ~1e-6/alpha of the threshold: ~1e-6 of the (site, subgroup) draws.
 template <> struct KPMath<float> {
-    static __device__ __forceinline__ float uni(uint32_t x) { return (float)(2u * (x >> 9) + 1u) * (1.0f / 16777216.0f); }
-    static __device__ __forceinline__ float cos2pi(float u) { return cospif(2.0f * u); }
-    static __device__ __forceinline__ float sin2pi(float u) { return sinpif(2.0f * u); }
-    static __device__ __forceinline__ float neglog(float u) { return -logf(u); }
-    static __device__ __forceinline__ float delta(float l1, float l2, float c, float alpha)
+    // (2 (x >> 9) + 1) 2^-24 = [1 + (x >> 9) 2^-23] - (1 - 2^-24): both terms and the result are fp32 numbers
+    static __device__ __forceinline__ float uni(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994039535522461f; }
+    static __device__ __forceinline__ float cos2pi(float u) { return __cosf(6.283185307179586f * u); }
+    static __device__ __forceinline__ float sin2pi(float u) { return __sinf(6.283185307179586f * u); }
+    static __device__ __forceinline__ float neglog(float u) { return -0.693147180559945f * __log2f(u); }
+    static __device__ __forceinline__ float inv(float alpha) { return 1.0f / alpha; }
+    static __device__ __forceinline__ float delta(float l1, float l2, float c, float alpha, float inv_alpha)
     {
-        return __fadd_rn(__fmul_rn(__fdiv_rn(l1, alpha), __fmul_rn(c, c)), __fdiv_rn(l2, alpha));
+        (void)alpha;
+        return fmaf(l1, c * c, l2) * inv_alpha;
     }
-    static __device__ __forceinline__ bool accept(float u4, float d) { return __fmul_rn(u4, u4) <= __fsub_rn(1.0f, __fmul_rn(0.5f, d)); }
+    static __device__ __forceinline__ bool accept(float u4, float d) { return u4 * u4 <= fmaf(-0.5f, d, 1.0f); }
 };
+
+// The Philox counters of a draw hold (site, step, parity, subgroup, trial) and no data, so the block of trial 0
+// and the direction block of each subgroup are generated up front, as six independent chains, while the thread's
+// link loads are in flight (EarlyRandom); only rejected trials call the generator inside the data-dependent loop.
+struct EarlyRandom {
+    uint32_t trial0[4]; // Philox block of trial 0: u1, u2, u3, u4
+    uint32_t dir[2];    // first two words of the direction block (counter word 3 = 0x80000000)
+};
+
+__device__ __forceinline__ void early_random(uint32_t key0, uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2,
+                                             EarlyRandom& e)
+{
+    uint32_t x[4];
+    philox4x32_10(c0, c1, c2, 0u, key0, key1, e.trial0);
+    philox4x32_10(c0, c1, c2, 0x80000000u, key0, key1, x);
+    e.dir[0] = x[0];
+    e.dir[1] = x[1];
+}
 
 // returns the number of trials used (0: degenerate block, identity taken; 4097: cap hit)
 template <typename T>
 __device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T temperature, uint32_t key0,
                                                       uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2,
-                                                      T (&g)[4])
+                                                      const EarlyRandom& early, T (&g)[4])
 {
     using M = KPMath<T>;
     T n = gf_sqrt<T>(k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3]);
     if (n < Tiny<T>::n) { g[0] = T(1); g[1] = g[2] = g[3] = T(0); return 0u; }
-    T alpha = n / temperature;
-    T kc0 = k[0] / n, kc1 = -k[1] / n, kc2 = -k[2] / n, kc3 = -k[3] / n; // conj(khat)
-    uint32_t x[4];
+    const T alpha = n / temperature;
+    const T inv_alpha = M::inv(alpha);
+    const T inv_n = T(1) / n;
+    const T kc0 = k[0] * inv_n, kc1 = -k[1] * inv_n, kc2 = -k[2] * inv_n, kc3 = -k[3] * inv_n; // conj(khat)
+    uint32_t x[4] = {early.trial0[0], early.trial0[1], early.trial0[2], early.trial0[3]};
     T h0 = T(1);
     bool accepted = false;
     unsigned trial = 0;
     for (; trial < 4096u; ++trial) {
-        philox4x32_10(c0, c1, c2, trial, key0, key1, x);
+        if (trial > 0u) philox4x32_10(c0, c1, c2, trial, key0, key1, x);
         T u1 = M::uni(x[0]), u2 = M::uni(x[1]), u3 = M::uni(x[2]), u4 = M::uni(x[3]);
         T c = M::cos2pi(u3);
-        T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha);
+        T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha, inv_alpha);
         if (M::accept(u4, d)) { h0 = T(1) - d; accepted = true; break; }
     }
     if (!accepted) {
@@ -120,9 +148,8 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T tempera
         g[0] = kc0; g[1] = kc1; g[2] = kc2; g[3] = kc3;
         return 4097u;
     }
-    philox4x32_10(c0, c1, c2, 0x80000000u, key0, key1, x);
-    T cos_t = T(1) - T(2) * M::uni(x[0]);
-    T up = M::uni(x[1]);
+    T cos_t = T(1) - T(2) * M::uni(early.dir[0]);
+    T up = M::uni(early.dir[1]);
     T r = gf_sqrt<T>(fmax(T(0), T(1) - h0 * h0));
     T sin_t = gf_sqrt<T>(fmax(T(0), T(1) - cos_t * cos_t));
     T h1 = r * sin_t * M::cos2pi(up);
@@ -146,7 +173,8 @@ struct SweepKernel {
 
     template <int I, int J, int SUB>
     static __device__ __forceinline__ void subgroup(const SweepParams& p, cx<T> (&K)[9], cx<T> (&F)[NMU][9],
-                                                    cx<T> (&B)[NMU][9], uint32_t site_canon, bool record)
+                                                    cx<T> (&B)[NMU][9], uint32_t site_canon, bool record,
+                                                    const EarlyRandom& early)
     {
         T k[4], h[4];
         su2_project<I, J>(K, k);
@@ -154,7 +182,7 @@ struct SweepKernel {
             su2_overrelax_step<T>(k, (T)p.omega, h);
         } else {
             unsigned ntr = su2_heatbath_step<T>(k, (T)p.T, p.key0, p.key1, site_canon, p.step,
-                                                ((uint32_t)p.parity << 2) | (uint32_t)SUB, h);
+                                                ((uint32_t)p.parity << 2) | (uint32_t)SUB, early, h);
             if (record && p.trials != nullptr) p.trials[3u * (size_t)site_canon + SUB] = ntr;
         }
         const cx<T> a = {h[0], h[3]}, b = {h[2], h[1]}; // C4
@@ -196,6 +224,20 @@ struct SweepKernel {
             IO::load(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.ld);
             IO::load(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.ld);
         }
+        // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
+        const uint32_t sc = canonical_index(s);
+        EarlyRandom early[3];
+        if (MODE == MODE_HEATBATH) {
+#pragma unroll
+            for (int sub = 0; sub < 3; ++sub)
+                early_random(p.key0, p.key1, sc, p.step, ((uint32_t)p.parity << 2) | (uint32_t)sub, early[sub]);
+            // pin the 18 words here, before the first use of a loaded link: volatile asm statements keep their
+            // order, so the generator runs between the issue of the loads and their consumption
+#pragma unroll
+            for (int sub = 0; sub < 3; ++sub)
+                asm volatile("" :: "r"(early[sub].trial0[0]), "r"(early[sub].trial0[1]), "r"(early[sub].trial0[2]),
+                             "r"(early[sub].trial0[3]), "r"(early[sub].dir[0]), "r"(early[sub].dir[1]));
+        }
         if (p.reunit) {
 #pragma unroll
             for (int m = 0; m < NMU; ++m) { reunitarise(F[m]); reunitarise(B[m]); }
@@ -225,11 +267,10 @@ struct SweepKernel {
             }
         }
 
-        const uint32_t sc = canonical_index(s);
         const bool record = active && (lane_mu0 == 0);
-        subgroup<0, 1, 0>(p, K, F, B, sc, record); // Cabibbo-Marinari subgroups in the order of C4
-        subgroup<0, 2, 1>(p, K, F, B, sc, record);
-        subgroup<1, 2, 2>(p, K, F, B, sc, record);
+        subgroup<0, 1, 0>(p, K, F, B, sc, record, early[0]); // Cabibbo-Marinari subgroups in the order of C4
+        subgroup<0, 2, 1>(p, K, F, B, sc, record, early[1]);
+        subgroup<1, 2, 2>(p, K, F, B, sc, record, early[2]);
 
         if (active) {
 #pragma unroll
