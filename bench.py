@@ -214,6 +214,23 @@ def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None):
             "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
 
 
+def max_over_ranks(seconds: float, device) -> float:
+    """N > 1: the timed region of the job is the slowest rank's (the only collective on this path: replicas only)"""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return seconds
+    tt = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(world: int, V: int, sweeps: int, steps: int, seconds: float) -> float:
+    """site-updates/s of the whole job: every rank sweeps its own replica (weak scaling, no data-path collective)"""
+    return world * V * sweeps * steps / seconds
+
+
 def time_e2e(gfm, w, U_host_pinned, sweeps, steps, warmup):
     """the host-buffer C-ABI call: H2D of the canonical field, pack, sweeps, F, theta, unpack, D2H -- all inside"""
     import torch
@@ -359,13 +376,9 @@ def main():
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
     m = measure(args.workload, w, sampler, barrier)
-    total = m["total"]
-    if world > 1:
-        tt = torch.tensor([total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total = float(tt.item())
+    total = max_over_ranks(m["total"], "cuda")
     V = volume(w["dims"])
-    value = world * V * sweeps * steps / total
+    value = whole_job_value(world, V, sweeps, steps, total)
 
     if world > 1:
         dist.barrier()
