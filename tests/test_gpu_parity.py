@@ -314,3 +314,30 @@ def test_host_buffer_path(gfm, precision):
     assert np.abs(U - ref).max() <= TOL_LINK[precision] * 2
     assert F == pytest.approx(oracle.functional(ref, dims), rel=TOL_F[precision])
     assert th == pytest.approx(oracle.theta(ref, dims), rel=1e-6 if precision == "fp64" else 1e-3)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# launch-time options change scheduling and caching, never a bit of the result
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,R", [("fp64", 18), ("fp32", 12)])
+def test_pdl_l2_policy_and_reversal_are_bit_neutral(gfm, precision, R):
+    dims = (8, 6, 4, 10)
+    U = gf_inputs.smooth_random(dims, 0.4, 31)
+    results = []
+    for pdl, ld, st, rev in ((0, 0, 0, 0), (1, 0, 2, 1), (1, 1, 2, 0), (0, 2, 1, 1)):
+        fx = _fixer(gfm, dims, precision, R=R)
+        gfm.gf_set_pdl(fx.ctx, pdl)
+        gfm.gf_set_l2_policy(fx.ctx, ld, st)
+        gfm.gf_set_l2_reversal(fx.ctx, rev)
+        fx.load(U)
+        fx.overrelax(1.7, 3)
+        fx.anneal(0.5, 0.3, 2, 9)
+        results.append(fx.download())
+        fx.close()
+    for r in results[1:]:
+        assert np.array_equal(r, results[0])
+    ctx = gfm.gf_create(4, 4, 4, 4)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_set_l2_policy(ctx, 3, 0)
+    gfm.gf_destroy(ctx)
