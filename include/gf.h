@@ -128,6 +128,10 @@ int gf_set_l2_policy(gf_ctx* ctx, int load_policy, int store_policy);
 /* Programmatic dependent launch of consecutive half-sweeps (1 = on, default): the next half-sweep's grid becomes
  * resident while the current one drains and waits on the device before it touches the field. */
 int gf_set_pdl(gf_ctx* ctx, int on);
+/* L2 prefetch distance of the sweep kernels, in sites along the traversal direction: every thread prefetches
+ * into L2 the lines that the thread `sites` further on will load.  0 = off, -1 = automatic (default; chosen per
+ * precision / storage / sweep kind from the measurements in profiles/). */
+int gf_set_prefetch(gf_ctx* ctx, int sites);
 /* Optional debug output of gf_anneal: d_trials (device, V*3 unsigned, index 3*s + subgroup) receives the
  * number of Kennedy-Pendleton trials of every (site, subgroup) of the LAST step; NULL switches it off. */
 int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);

@@ -47,6 +47,7 @@ SIGNATURES = {
     "gf_set_l2_reversal": (_i, [_vp, _i]),
     "gf_set_l2_policy": (_i, [_vp, _i, _i]),
     "gf_set_pdl": (_i, [_vp, _i]),
+    "gf_set_prefetch": (_i, [_vp, _i]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
     "gf_launch_count": (_ull, [_vp]),
     "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
@@ -189,6 +190,10 @@ def gf_set_l2_policy(ctx, load_policy: int, store_policy: int) -> None:
 
 def gf_set_pdl(ctx, on: bool) -> None:
     _check(ctx, load_library().gf_set_pdl(ctx, int(bool(on))))
+
+
+def gf_set_prefetch(ctx, sites: int) -> None:
+    _check(ctx, load_library().gf_set_prefetch(ctx, int(sites)))
 
 
 def gf_set_trial_buffer(ctx, d_trials) -> None:

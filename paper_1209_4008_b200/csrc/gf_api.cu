@@ -20,6 +20,7 @@ struct gf_ctx {
     int l2_reversal;
     int ld_policy, st_policy;         // L2 eviction policy of the sweep's link loads / stores
     int pdl;                          // programmatic dependent launch of consecutive half-sweeps
+    int prefetch;                     // L2 prefetch distance of the sweep kernels, in sites (0 = off)
     unsigned long long sweeps_done;   // overrelaxation sweeps since creation (cadence of the fp32 reunitarisation)
     unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
     unsigned long long launches;
@@ -86,6 +87,7 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->l2_reversal = 1;
     c->ld_policy = POLICY_NORMAL; c->st_policy = POLICY_EVICT_LAST; // measured best: profiles/r1_variants.md
     c->pdl = 1;
+    c->prefetch = -1; // automatic
     c->sweeps_done = 0; c->half_sweeps = 0; c->launches = 0;
     c->d_trials = nullptr; c->last_stream = nullptr;
     c->d_canon = nullptr; c->d_native = nullptr;
@@ -172,6 +174,14 @@ extern "C" int gf_set_pdl(gf_ctx* c, int on)
     return GF_OK;
 }
 
+extern "C" int gf_set_prefetch(gf_ctx* c, int sites)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (sites < -1) return fail(c, GF_EINVAL, "gf_set_prefetch: distance must be >= 0, or -1 for automatic");
+    c->prefetch = sites;
+    return GF_OK;
+}
+
 extern "C" int gf_set_trial_buffer(gf_ctx* c, unsigned* d_trials)
 {
     if (c == nullptr) return GF_EINVAL;
@@ -192,11 +202,22 @@ static int auto_tps(const gf_ctx* c, int mode)
     if (c->precision == GF_FP64) return 2;
     return c->R == 18 ? 1 : 2;
 }
+// L2 prefetch distance (sites), from the sweep in profiles/r1_variants.md: a quarter of a wave ahead helps the
+// variants with more arithmetic per byte (R = 12: +2..3 %, heatbath: +1.5 %); the R = 18 overrelaxation kernels
+// already saturate the memory system with their own outstanding loads (fp32: -1 % with prefetch, fp64: neutral).
+static int auto_prefetch(const gf_ctx* c, int mode)
+{
+    if (c->prefetch >= 0) return c->prefetch;
+    if (mode == MODE_HEATBATH) return 7104;
+    return c->R == 12 ? 4736 : 0;
+}
 static int auto_block(const gf_ctx* c) { return c->block ? c->block : 32; }
 
-static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p, cudaStream_t st)
+static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p_in, cudaStream_t st)
 {
     const int tps = auto_tps(c, mode), block = auto_block(c);
+    SweepParams p = p_in;
+    p.prefetch = (unsigned)auto_prefetch(c, mode);
     if (c->precision == GF_FP32) return c->R == 18 ? launch_sweep_f32_r18(tps, mode, block, p, st) : launch_sweep_f32_r12(tps, mode, block, p, st);
     return c->R == 18 ? launch_sweep_f64_r18(tps, mode, block, p, st) : launch_sweep_f64_r12(tps, mode, block, p, st);
 }

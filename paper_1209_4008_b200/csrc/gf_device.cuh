@@ -209,6 +209,9 @@ __device__ __forceinline__ void stg(double2* p, double2 v, uint64_t pol)
     asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
 }
 
+// L2 prefetch of the 128-byte line holding p (a hint: no register, no scoreboard)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
+
 template <typename T, int R> struct LinkIO;
 
 template <int R>
@@ -224,6 +227,12 @@ struct LinkIO<double, R> {
             u[e] = {v.x, v.y};
         }
         if (R == 12) rebuild_row2(u);
+    }
+    static __device__ __forceinline__ void prefetch(const double* blk, size_t H, size_t h)
+    {
+        const double2* p = reinterpret_cast<const double2*>(blk) + h;
+#pragma unroll
+        for (int e = 0; e < NE; ++e) prefetch_l2(p + (size_t)e * H);
     }
     static __device__ __forceinline__ void store(double* blk, size_t H, size_t h, const cx<double> (&u)[9], uint64_t pol)
     {
@@ -251,6 +260,13 @@ struct LinkIO<float, R> {
         } else {
             rebuild_row2(u);
         }
+    }
+    static __device__ __forceinline__ void prefetch(const float* blk, size_t H, size_t h)
+    {
+        const float4* p = reinterpret_cast<const float4*>(blk) + h;
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) prefetch_l2(p + (size_t)q * H);
+        if (R == 18) prefetch_l2(reinterpret_cast<const float2*>(blk + 16 * H) + h);
     }
     static __device__ __forceinline__ void store(float* blk, size_t H, size_t h, const cx<float> (&u)[9], uint64_t pol)
     {

@@ -28,6 +28,7 @@ struct SweepParams {
     int ld_policy;  // L2 policy of the link loads / stores (POLICY_*, gf_device.cuh)
     int st_policy;
     int pdl;        // launched with programmatic stream serialization: wait for the previous grid before loading
+    unsigned prefetch; // L2 prefetch distance in sites along the traversal direction (0 = off)
     double omega;   // overrelaxation parameter
     double T;       // heatbath temperature (C13)
     uint32_t key0, key1, step; // Philox key = seed, step = annealing step (C14)
@@ -216,6 +217,23 @@ struct SweepKernel {
         if (p.pdl) {
             cudaTriggerProgrammaticLaunchCompletion();
             cudaGridDependencySynchronize();
+        }
+        // L2 prefetch for the block that runs `prefetch` sites further along the traversal: the few fat warps of
+        // an SM cannot keep enough bytes in flight while they compute, prefetches hold no register and no
+        // scoreboard entry, and the 126 MB L2 is the staging buffer.  Addresses are those of this thread shifted
+        // by the distance (exact for forward links, exact up to the periodic wrap for backward links: a hint).
+        if (p.prefetch) {
+            const long long d = p.reverse ? -(long long)p.prefetch : (long long)p.prefetch;
+            const long long hf = (long long)s.h + d;
+            if (hf >= 0 && hf < (long long)H) {
+#pragma unroll
+                for (int m = 0; m < NMU; ++m) {
+                    const int mu = lane_mu0 + m;
+                    const long long hbd = (long long)hb[m] + d;
+                    IO::prefetch(base + (size_t)(p.parity * 4 + mu) * R * H, H, (size_t)hf);
+                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, (size_t)hbd);
+                }
+            }
         }
         // issue every load before the first use
 #pragma unroll

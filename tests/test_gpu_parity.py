@@ -325,11 +325,12 @@ def test_pdl_l2_policy_and_reversal_are_bit_neutral(gfm, precision, R):
     dims = (8, 6, 4, 10)
     U = gf_inputs.smooth_random(dims, 0.4, 31)
     results = []
-    for pdl, ld, st, rev in ((0, 0, 0, 0), (1, 0, 2, 1), (1, 1, 2, 0), (0, 2, 1, 1)):
+    for pdl, ld, st, rev, pf in ((0, 0, 0, 0, 0), (1, 0, 2, 1, -1), (1, 1, 2, 0, 100), (0, 2, 1, 1, 7)):
         fx = _fixer(gfm, dims, precision, R=R)
         gfm.gf_set_pdl(fx.ctx, pdl)
         gfm.gf_set_l2_policy(fx.ctx, ld, st)
         gfm.gf_set_l2_reversal(fx.ctx, rev)
+        gfm.gf_set_prefetch(fx.ctx, pf)
         fx.load(U)
         fx.overrelax(1.7, 3)
         fx.anneal(0.5, 0.3, 2, 9)
