@@ -66,6 +66,11 @@ def _load():
         "orc_kp_draw": (_int, [_dbl, _vp, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32, _vp]),
         "orc_site_heatbath": (None, [N, _int, _vp, ctypes.c_long, _dbl, ctypes.c_uint64, ctypes.c_uint32, _vp]),
         "orc_anneal": (None, [N, _int, _vp, _dbl, _dbl, _int, ctypes.c_uint64, _vp]),
+        "orc_su2_overrelax1": (None, [_vp, _dbl, _vp]),
+        "orc_su2_square": (None, [_vp, _vp]),
+        "orc_site_relax": (None, [N, _int, _vp, ctypes.c_long, _int, _dbl, ctypes.c_uint64, ctypes.c_uint32, _vp]),
+        "orc_relax": (None, [N, _int, _vp, _int, _dbl, _int, ctypes.c_uint64, _vp]),
+        "orc_anneal_micro": (None, [N, _int, _vp, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -121,6 +126,43 @@ def anneal(U, dims, T_start: float, T_end: float, nsteps: int, seed: int, gauge:
     _load().orc_anneal(N, gauge, _field(U, V), float(T_start), float(T_end), int(nsteps), int(seed),
                        tr.ctypes.data if trials else None)
     return tr
+
+
+UPDATE_OVERRELAX2, UPDATE_OVERRELAX1, UPDATE_STOCHASTIC = 0, 1, 2
+
+
+def relax(U, dims, update: int, param: float, nsweeps: int, seed: int = 0, gauge: int = LANDAU, squared: bool = False):
+    """update variants (C17, C18): second / first order overrelaxation (param = omega), stochastic relaxation
+    (param = p).  squared=True returns the (V, 3) array of g^2 decisions of the last sweep."""
+    N, V = _dims(dims)
+    sq = np.zeros((V, 3), dtype=np.int32) if squared else None
+    _load().orc_relax(N, gauge, _field(U, V), int(update), float(param), int(nsweeps), int(seed),
+                      sq.ctypes.data if squared else None)
+    return sq
+
+
+def anneal_micro(U, dims, T_start: float, T_end: float, nsteps: int, n_micro: int, seed: int, gauge: int = LANDAU,
+                 trials: bool = False):
+    """annealing with n_micro microcanonical (g -> g^2) sweeps after every heatbath sweep (C19)"""
+    N, V = _dims(dims)
+    tr = np.zeros((V, 3), dtype=np.int32) if trials else None
+    _load().orc_anneal_micro(N, gauge, _field(U, V), float(T_start), float(T_end), int(nsteps), int(n_micro),
+                             int(seed), tr.ctypes.data if trials else None)
+    return tr
+
+
+def su2_overrelax1(g, omega: float) -> np.ndarray:
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    h = np.zeros(4)
+    _load().orc_su2_overrelax1(g.ctypes.data, float(omega), h.ctypes.data)
+    return h
+
+
+def su2_square(g) -> np.ndarray:
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    h = np.zeros(4)
+    _load().orc_su2_square(g.ctypes.data, h.ctypes.data)
+    return h
 
 
 def functional(U, dims, gauge: int = LANDAU) -> float:

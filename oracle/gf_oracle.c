@@ -483,3 +483,97 @@ void orc_anneal(const int N[4], int gauge, double *U, double T_start, double T_e
         }
     }
 }
+
+/* ------------------------------------------------------------------------------------------------ */
+/* Update variants of the relaxation family ("Besides the standard relaxation algorithm */
+/* [3] our program supports overrelaxation [4] and stochastic relaxation [5]"; "the      */
+/* exponentiation of the gauge transformation is done to first or second order").  The paper gives   */
+/* no formulas; readings C17-C19 of DESIGN.md:                                                       */
+/*   C17 first order:  g^w ~ 1 + w (g - 1)  =>  h = (1 + w d, w gvec) / |.|,  d = g0 - 1             */
+/*   C18 stochastic relaxation [5]: g -> g^2 with probability p, else g (plain relaxation);          */
+/*       g^2 = (2 g0^2 - 1, 2 g0 gvec); decision: u < p with u = uniform24(x0) of the Philox block    */
+/*       key = seed, counter = (site, sweep, parity<<2 | subgroup, 0x40000000)                       */
+/*   C19 microcanonical sweep: g -> g^2 always (leaves F unchanged), n_micro of them after every     */
+/*       heatbath sweep of the annealing                                                             */
+/* ------------------------------------------------------------------------------------------------ */
+enum { ORC_UPDATE_OVERRELAX2 = 0, ORC_UPDATE_OVERRELAX1 = 1, ORC_UPDATE_STOCHASTIC = 2 };
+
+void orc_su2_overrelax1(const double g[4], double omega, double h[4])
+{
+    double d = g[0] - 1.0;
+    double h0 = 1.0 + omega * d;
+    double h1 = omega * g[1], h2 = omega * g[2], h3 = omega * g[3];
+    double n2 = h0 * h0 + h1 * h1 + h2 * h2 + h3 * h3;
+    if (n2 < 1e-20) { h[0] = g[0]; h[1] = g[1]; h[2] = g[2]; h[3] = g[3]; return; }
+    double n = sqrt(n2);
+    h[0] = h0 / n; h[1] = h1 / n; h[2] = h2 / n; h[3] = h3 / n;
+}
+
+void orc_su2_square(const double g[4], double h[4])
+{
+    double t = 2.0 * g[0];
+    h[0] = t * g[0] - 1.0; h[1] = t * g[1]; h[2] = t * g[2]; h[3] = t * g[3];
+}
+
+/* one site update with the chosen variant.  squared (may be NULL): 3 ints per site, 1 where g^2 was taken */
+void orc_site_relax(const int N[4], int gauge, double *U_, long s, int update, double param, uint64_t seed,
+                    uint32_t sweep, int *squared)
+{
+    cplx *U = (cplx *)U_;
+    cplx K[9], G[9];
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    const uint32_t parity = (uint32_t)lat_parity(N, s);
+    orc_build_K(N, gauge, U_, s, (double *)K);
+    for (int sub = 0; sub < 3; ++sub) {
+        const int i = SUBGROUP[sub][0], j = SUBGROUP[sub][1];
+        double k[4], g[4], h[4];
+        int sq = 0;
+        orc_su2_project((const double *)K, i, j, k);
+        orc_su2_maximiser(k, g);
+        if (update == ORC_UPDATE_OVERRELAX1) {
+            orc_su2_overrelax1(g, param, h);
+        } else if (update == ORC_UPDATE_STOCHASTIC) {
+            uint32_t ctr[4] = { (uint32_t)s, sweep, (parity << 2) | (uint32_t)sub, 0x40000000u }, x[4];
+            orc_philox4x32_10(ctr, key, x);
+            sq = uniform24(x[0]) < param;
+            if (sq) orc_su2_square(g, h);
+            else { h[0] = g[0]; h[1] = g[1]; h[2] = g[2]; h[3] = g[3]; }
+        } else {
+            orc_su2_overrelax(g, param, h);
+        }
+        if (squared) squared[3 * s + sub] = sq;
+        orc_su2_embed(h, i, j, (double *)G);
+        apply_G_to_links(N, U, s, G);
+        m_mul(G, K, K);
+    }
+}
+
+/* nsweeps sweeps (RED then BLACK) with the chosen variant; the sweep counter of the random decisions starts at 0 */
+void orc_relax(const int N[4], int gauge, double *U, int update, double param, int nsweeps, uint64_t seed,
+               int *squared)
+{
+    const long V = lat_volume(N);
+    for (int sweep = 0; sweep < nsweeps; ++sweep)
+        for (int parity = 0; parity < 2; ++parity) {
+#pragma omp parallel for schedule(static)
+            for (long s = 0; s < V; ++s)
+                if (lat_parity(N, s) == parity)
+                    orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)sweep, squared);
+        }
+}
+
+/* annealing with n_micro microcanonical sweeps after every heatbath sweep (C19) */
+void orc_anneal_micro(const int N[4], int gauge, double *U, double T_start, double T_end, int nsteps,
+                      int n_micro, uint64_t seed, int *trials)
+{
+    const long V = lat_volume(N);
+    for (int step = 0; step < nsteps; ++step) {
+        double T = (nsteps > 1) ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
+        for (int parity = 0; parity < 2; ++parity) {
+#pragma omp parallel for schedule(static)
+            for (long s = 0; s < V; ++s)
+                if (lat_parity(N, s) == parity) orc_site_heatbath(N, gauge, U, s, T, seed, (uint32_t)step, trials);
+        }
+        orc_relax(N, gauge, U, ORC_UPDATE_STOCHASTIC, 2.0, n_micro, seed, NULL); /* p = 2 > u always: g^2 */
+    }
+}

@@ -1,0 +1,137 @@
+"""Pins of the oracle's update variants (readings C17-C19): first-order overrelaxation, stochastic
+relaxation, microcanonical sweeps.  Each against a closed form, an invariant or an independent restatement."""
+import numpy as np
+import pytest
+
+import gf_inputs
+import oracle
+
+import np_lattice as npl
+
+
+def _unit_quat(rng):
+    q = rng.normal(size=4)
+    return q / np.linalg.norm(q)
+
+
+def _exact_power(g, w):
+    """exact g^w of the SU(2) element g = (cos phi, sin phi n)"""
+    phi = np.arccos(np.clip(g[0], -1, 1))
+    n = g[1:] / max(np.linalg.norm(g[1:]), 1e-300)
+    return np.concatenate([[np.cos(w * phi)], np.sin(w * phi) * n])
+
+
+def test_first_order_closed_forms():
+    """C17: h = g at omega = 1; direction of hvec unchanged; matches exact g^omega to O(phi^2):
+    |h - g^w| <= w (w - 1) / 2 * phi^2 (1 + O(phi)) for small rotation angle phi"""
+    rng = np.random.default_rng(1)
+    for _ in range(50):
+        g = _unit_quat(rng)
+        assert np.allclose(oracle.su2_overrelax1(g, 1.0), g, atol=1e-15)
+        h = oracle.su2_overrelax1(g, 1.6)
+        assert abs(np.linalg.norm(h) - 1) < 1e-15
+        assert np.allclose(np.cross(h[1:], g[1:]), 0, atol=1e-15) and np.dot(h[1:], g[1:]) > 0
+    for phi in (1e-3, 1e-2, 5e-2):
+        n = _unit_quat(rng)[1:]
+        n /= np.linalg.norm(n)
+        g = np.concatenate([[np.cos(phi)], np.sin(phi) * n])
+        for w in (1.3, 1.7, 1.9):
+            err = np.linalg.norm(oracle.su2_overrelax1(g, w) - _exact_power(g, w))
+            # after normalisation the first-order form is a rotation by atan(w tan(phi) / ...) ~ w phi (1 + O(phi^2)):
+            # the angle error is cubic, bounded by w (w^2 - 1) / 3 * phi^3
+            assert err <= w * (w * w - 1) / 3 * phi**3 * 1.5 + 1e-15
+    # explicit value: g0 = 0, omega = 1.5: h = (1 - 1.5, 1.5 gvec) / sqrt(0.25 + 2.25)
+    g = np.array([0.0, 0.0, 1.0, 0.0])
+    assert np.allclose(oracle.su2_overrelax1(g, 1.5), np.array([-0.5, 0, 1.5, 0]) / np.sqrt(2.5), atol=1e-15)
+
+
+def test_square_is_exact_double_rotation():
+    """C18/C19: g^2 equals the exact power at omega = 2 and the quaternion product g (x) g"""
+    rng = np.random.default_rng(2)
+    for _ in range(50):
+        g = _unit_quat(rng)
+        sq = oracle.su2_square(g)
+        assert np.allclose(sq, oracle.quat_mul(g, g), atol=1e-15)
+        assert np.allclose(sq, _exact_power(g, 2.0), atol=1e-12)
+        assert np.allclose(sq, oracle.su2_overrelax(g, 2.0), atol=1e-14)  # the 2nd-order form is exact at omega = 2
+
+
+@pytest.mark.parametrize("gauge,nd", [(oracle.LANDAU, 4), (oracle.COULOMB, 3)])
+def test_microcanonical_sweeps_conserve_F(gauge, nd):
+    """C19: g -> g^2 leaves Re tr[g K] at its old value in every subgroup step, so F is unchanged by whole sweeps
+    (p = 1 stochastic relaxation); the field does change; plaquette and unitarity are preserved"""
+    dims = (4, 6, 4, 4)
+    U = gf_inputs.smooth_random(dims, 0.5, 41)
+    U0 = U.copy()
+    F0, P0 = npl.functional(U, dims, nd), npl.plaquette(U, dims)
+    oracle.relax(U, dims, oracle.UPDATE_STOCHASTIC, 1.0, 3, 5, gauge)
+    assert np.abs(U - U0).max() > 0.1
+    assert abs(npl.functional(U, dims, nd) - F0) < 1e-13
+    assert abs(npl.plaquette(U, dims) - P0) < 1e-13
+    uu, det = oracle.unitarity_defect(U, dims)
+    assert uu < 1e-13 and det < 1e-13
+
+
+def test_stochastic_limits_and_rate():
+    """C18: p = 0 is plain relaxation (omega = 1, up to the renormalisation rounding of the latter); decisions follow the stated Philox recipe and their
+    rate is p within 4 sigma; same seed -> same decisions, other seed -> others"""
+    dims = (4, 4, 4, 6)
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.4, 42)
+    a, b = U.copy(), U.copy()
+    oracle.relax(a, dims, oracle.UPDATE_STOCHASTIC, 0.0, 2, 9)
+    oracle.overrelax(b, dims, 1.0, 2)
+    assert np.abs(a - b).max() < 1e-13
+    p = 0.3
+    c = U.copy()
+    sq = oracle.relax(c, dims, oracle.UPDATE_STOCHASTIC, p, 1, 9, squared=True)
+    n = sq.size
+    assert abs(sq.mean() - p) < 4 * np.sqrt(p * (1 - p) / n)
+    # the recipe, restated: counter (site, sweep, parity << 2 | subgroup, 0x40000000), key = seed, first word
+    for s in (0, 17, V - 1):
+        x = s % 4 + (s // 4) % 4 + (s // 16) % 4 + s // 64
+        for sub in range(3):
+            w = oracle.philox4x32_10([s, 0, ((x & 1) << 2) | sub, 0x40000000], [9, 0])[0]
+            u = (2 * (int(w) >> 9) + 1) / 2**24
+            assert sq[s, sub] == int(u < p)
+    d = U.copy()
+    assert np.array_equal(oracle.relax(d, dims, oracle.UPDATE_STOCHASTIC, p, 1, 9, squared=True), sq)
+    e = U.copy()
+    assert not np.array_equal(oracle.relax(e, dims, oracle.UPDATE_STOCHASTIC, p, 1, 10, squared=True), sq)
+
+
+def test_variants_converge_on_trivial_orbit():
+    """first-order overrelaxation and stochastic relaxation are gauge-fixing algorithms: on the trivial orbit
+    (config 1) theta -> 0 and F -> 1 (P1 for the variants)"""
+    dims = (4, 4, 4, 4)
+    U0 = gf_inputs.trivial_orbit(dims, 1)
+    for update, param in ((oracle.UPDATE_OVERRELAX1, 1.3), (oracle.UPDATE_OVERRELAX1, 1.6),
+                          (oracle.UPDATE_STOCHASTIC, 0.3), (oracle.UPDATE_STOCHASTIC, 0.7)):
+        U = U0.copy()
+        oracle.relax(U, dims, update, param, 300, 3)
+        assert oracle.theta(U, dims) < 1e-14, (update, param)
+        assert abs(oracle.functional(U, dims) - 1) < 1e-12, (update, param)
+
+
+def test_second_order_variant_is_the_overrelax_call():
+    dims = (4, 4, 2, 6)
+    U = gf_inputs.smooth_random(dims, 0.4, 43)
+    a, b = U.copy(), U.copy()
+    oracle.relax(a, dims, oracle.UPDATE_OVERRELAX2, 1.7, 2, 0, oracle.COULOMB)
+    oracle.overrelax(b, dims, 1.7, 2, oracle.COULOMB)
+    assert np.array_equal(a, b)
+
+
+def test_anneal_micro_reduces_to_anneal_and_conserves_between_heatbath():
+    dims = (4, 4, 4, 4)
+    U = gf_inputs.smooth_random(dims, 0.5, 44)
+    a, b = U.copy(), U.copy()
+    oracle.anneal_micro(a, dims, 1.0, 0.5, 3, 0, 7)
+    oracle.anneal(b, dims, 1.0, 0.5, 3, 7)
+    assert np.array_equal(a, b)
+    # one heatbath sweep then 2 microcanonical sweeps: F equals F after the heatbath sweep alone
+    c, d = U.copy(), U.copy()
+    oracle.anneal_micro(c, dims, 0.8, 0.8, 1, 2, 7)
+    oracle.anneal(d, dims, 0.8, 0.8, 1, 7)
+    assert np.abs(c - d).max() > 0.05
+    assert abs(npl.functional(c, dims, 4) - npl.functional(d, dims, 4)) < 1e-13
