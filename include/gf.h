@@ -87,6 +87,22 @@ int gf_overrelax(gf_ctx* ctx, void* U_native_dev, double omega, int nsweeps, voi
 int gf_anneal(gf_ctx* ctx, void* U_native_dev, double T_start, double T_end, int nsteps,
               unsigned long long seed, void* stream);
 
+/* The other members of the paper's "family of relaxation algorithms", same sweep, other SU(2) step:
+ *   GF_UPDATE_OVERRELAX2: gf_overrelax (param = omega, second-order g^omega);
+ *   GF_UPDATE_OVERRELAX1: g^omega "to first order" (C17): h = (1 + omega (g0 - 1), omega gvec) / |.|;
+ *   GF_UPDATE_STOCHASTIC: stochastic relaxation (PAPER.md:33 ref. [5]; C18): g -> g^2 with probability param = p in
+ *     [0,1], else g; decision u < p from Philox4x32-10 keyed by (seed; site, sweep, parity, subgroup), the sweep
+ *     counter restarting at 0 with every call.  p = 0 is plain relaxation [3], p = 1 a microcanonical sweep.
+ * GF_EINVAL: unknown update, omega outside [1,2), p outside [0,1], nsweeps < 0, NULL U. */
+enum { GF_UPDATE_OVERRELAX2 = 0, GF_UPDATE_OVERRELAX1 = 1, GF_UPDATE_STOCHASTIC = 2 };
+int gf_relax(gf_ctx* ctx, void* U_native_dev, int update, double param, int nsweeps, unsigned long long seed,
+             void* stream);
+
+/* gf_anneal with n_micro microcanonical sweeps (g -> g^2 in every subgroup: F unchanged, C19) after every heatbath
+ * sweep.  n_micro = 0 is gf_anneal. */
+int gf_anneal_micro(gf_ctx* ctx, void* U_native_dev, double T_start, double T_end, int nsteps, int n_micro,
+                    unsigned long long seed, void* stream);
+
 /* ---- the reductions (device field -> host scalar; these calls synchronise) ------------------------------- */
 
 /* F = Re sum_{x, mu < Nd} tr U_mu(x) / (N_c * Nd * V)  (eq. 2.1, C1), Nd = 4 (Landau) or 3

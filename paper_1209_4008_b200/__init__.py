@@ -17,6 +17,7 @@ import os
 GF_FP32, GF_FP64 = 0, 1
 GF_LANDAU, GF_COULOMB = 0, 1
 GF_OK, GF_EINVAL, GF_ECUDA, GF_ENOMEM = 0, -1, -2, -3
+GF_UPDATE_OVERRELAX2, GF_UPDATE_OVERRELAX1, GF_UPDATE_STOCHASTIC = 0, 1, 2
 
 # paper flop model, Alg. 1: 60 + 19 + 4*(84+84) = 751 per subgroup, 2253 per site
 FLOP_PER_SITE = 3 * (60 + 19 + 4 * (84 + 84))
@@ -38,6 +39,8 @@ SIGNATURES = {
     "gf_unpack": (_i, [_vp, _vp, _vp, _vp]),
     "gf_overrelax": (_i, [_vp, _vp, _d, _i, _vp]),
     "gf_anneal": (_i, [_vp, _vp, _d, _d, _i, _ull, _vp]),
+    "gf_relax": (_i, [_vp, _vp, _i, _d, _i, _ull, _vp]),
+    "gf_anneal_micro": (_i, [_vp, _vp, _d, _d, _i, _i, _ull, _vp]),
     "gf_functional": (_i, [_vp, _vp, _pd]),
     "gf_theta": (_i, [_vp, _vp, _pd]),
     "gf_theta_slices": (_i, [_vp, _vp, _pd]),
@@ -143,6 +146,16 @@ def gf_overrelax(ctx, U, omega: float, nsweeps: int, stream=None) -> None:
 def gf_anneal(ctx, U, T_start: float, T_end: float, nsteps: int, seed: int, stream=None) -> None:
     _check(ctx, load_library().gf_anneal(ctx, _ptr(U), float(T_start), float(T_end), int(nsteps), int(seed),
                                         _stream(stream)))
+
+
+def gf_relax(ctx, U, update: int, param: float, nsweeps: int, seed: int = 0, stream=None) -> None:
+    _check(ctx, load_library().gf_relax(ctx, _ptr(U), int(update), float(param), int(nsweeps), int(seed),
+                                       _stream(stream)))
+
+
+def gf_anneal_micro(ctx, U, T_start: float, T_end: float, nsteps: int, n_micro: int, seed: int, stream=None) -> None:
+    _check(ctx, load_library().gf_anneal_micro(ctx, _ptr(U), float(T_start), float(T_end), int(nsteps), int(n_micro),
+                                              int(seed), _stream(stream)))
 
 
 def gf_functional(ctx, U) -> float:
@@ -269,8 +282,11 @@ class GaugeFixer:
     def overrelax(self, omega: float, nsweeps: int, stream=None):
         gf_overrelax(self.ctx, self.U, omega, nsweeps, stream)
 
-    def anneal(self, T_start: float, T_end: float, nsteps: int, seed: int, stream=None):
-        gf_anneal(self.ctx, self.U, T_start, T_end, nsteps, seed, stream)
+    def anneal(self, T_start: float, T_end: float, nsteps: int, seed: int, stream=None, n_micro: int = 0):
+        gf_anneal_micro(self.ctx, self.U, T_start, T_end, nsteps, n_micro, seed, stream)
+
+    def relax(self, update: int, param: float, nsweeps: int, seed: int = 0, stream=None):
+        gf_relax(self.ctx, self.U, update, param, nsweeps, seed, stream)
 
     def functional(self) -> float:
         return gf_functional(self.ctx, self.U)

@@ -274,24 +274,25 @@ extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* str
     return GF_OK;
 }
 
-extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void* stream)
+// nsweeps sweeps (RED then BLACK) of one member of the relaxation family on `st`
+static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
+                      cudaStream_t st, const char* who)
 {
-    if (c == nullptr) return GF_EINVAL;
-    if (U == nullptr) return fail(c, GF_EINVAL, "gf_overrelax: U is NULL");
-    if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_overrelax: omega = %g outside [1,2) (PAPER.md:63)", omega);
-    if (nsweeps < 0) return fail(c, GF_EINVAL, "gf_overrelax: nsweeps = %d < 0", nsweeps);
-    cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     SweepParams p = base_params(c, U);
-    p.omega = omega;
+    p.omega = param;
+    p.variant = variant;
+    p.key0 = (uint32_t)seed;
+    p.key1 = (uint32_t)(seed >> 32);
     for (int sweep = 0; sweep < nsweeps; ++sweep) {
         const bool reunit = c->reunit_every > 0 && ((c->sweeps_done + 1) % (unsigned long long)c->reunit_every) == 0;
+        p.step = (uint32_t)sweep; // sweep counter of the random decisions (C18): restarts at 0 with every call
         for (int parity = 0; parity < 2; ++parity) { // RED, BLACK
             p.parity = parity;
             p.reunit = (reunit && parity == 0) ? 1 : 0; // every link is loaded once per half-sweep (C6)
             p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
-            cudaError_t e = launch_sweep(c, MODE_OVERRELAX, p, st);
-            if (e != cudaSuccess) return cuda_fail(c, e, "gf_overrelax: kernel launch");
+            cudaError_t e = launch_sweep(c, mode, p, st);
+            if (e != cudaSuccess) return cuda_fail(c, e, who);
             c->half_sweeps += 1;
             c->launches += 1;
         }
@@ -300,12 +301,43 @@ extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void*
     return GF_OK;
 }
 
-extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, unsigned long long seed, void* stream)
+extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (U == nullptr) return fail(c, GF_EINVAL, "gf_overrelax: U is NULL");
+    if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_overrelax: omega = %g outside [1,2) (PAPER.md:63)", omega);
+    if (nsweeps < 0) return fail(c, GF_EINVAL, "gf_overrelax: nsweeps = %d < 0", nsweeps);
+    return run_sweeps(c, U, MODE_OVERRELAX, 0, omega, nsweeps, 0ull, (cudaStream_t)stream, "gf_overrelax: kernel launch");
+}
+
+extern "C" int gf_relax(gf_ctx* c, void* U, int update, double param, int nsweeps, unsigned long long seed, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (U == nullptr) return fail(c, GF_EINVAL, "gf_relax: U is NULL");
+    if (nsweeps < 0) return fail(c, GF_EINVAL, "gf_relax: nsweeps = %d < 0", nsweeps);
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (update) {
+    case GF_UPDATE_OVERRELAX2:
+        return gf_overrelax(c, U, param, nsweeps, stream);
+    case GF_UPDATE_OVERRELAX1:
+        if (!(param >= 1.0 && param < 2.0)) return fail(c, GF_EINVAL, "gf_relax: omega = %g outside [1,2) (PAPER.md:63)", param);
+        return run_sweeps(c, U, MODE_VARIANT, VARIANT_OVERRELAX1, param, nsweeps, seed, st, "gf_relax: kernel launch");
+    case GF_UPDATE_STOCHASTIC:
+        if (!(param >= 0.0 && param <= 1.0)) return fail(c, GF_EINVAL, "gf_relax: probability p = %g outside [0,1]", param);
+        return run_sweeps(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, param, nsweeps, seed, st, "gf_relax: kernel launch");
+    default:
+        return fail(c, GF_EINVAL, "gf_relax: unknown update %d", update);
+    }
+}
+
+extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, int n_micro,
+                               unsigned long long seed, void* stream)
 {
     if (c == nullptr) return GF_EINVAL;
     if (U == nullptr) return fail(c, GF_EINVAL, "gf_anneal: U is NULL");
     if (!(T_start > 0.0) || !(T_end > 0.0)) return fail(c, GF_EINVAL, "gf_anneal: temperatures must be > 0 (got %g, %g)", T_start, T_end);
     if (nsteps < 0) return fail(c, GF_EINVAL, "gf_anneal: nsteps = %d < 0", nsteps);
+    if (n_micro < 0) return fail(c, GF_EINVAL, "gf_anneal_micro: n_micro = %d < 0", n_micro);
     cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     SweepParams p = base_params(c, U);
@@ -324,8 +356,18 @@ extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int n
             c->half_sweeps += 1;
             c->launches += 1;
         }
+        // microcanonical sweeps g -> g^2 (C19): stochastic relaxation with p = 2 > u, i.e. always
+        if (n_micro > 0) {
+            int rc = run_sweeps(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, seed, st, "gf_anneal_micro: kernel launch");
+            if (rc != GF_OK) return rc;
+        }
     }
     return GF_OK;
+}
+
+extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, unsigned long long seed, void* stream)
+{
+    return gf_anneal_micro(c, U, T_start, T_end, nsteps, 0, seed, stream);
 }
 
 // runs one reduction on last_stream and brings the Nt+2 results to h_out

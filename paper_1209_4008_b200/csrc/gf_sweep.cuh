@@ -15,7 +15,10 @@
 
 namespace gf {
 
-enum { MODE_OVERRELAX = 0, MODE_HEATBATH = 1 };
+enum { MODE_OVERRELAX = 0, MODE_HEATBATH = 1, MODE_VARIANT = 2 };
+// MODE_VARIANT picks the SU(2) step at run time (SweepParams::variant): the update variants the paper's package
+// offers beside second-order overrelaxation (readings C17, C18)
+enum { VARIANT_OVERRELAX1 = 1, VARIANT_STOCHASTIC = 2 };
 constexpr int MAX_BLOCK = 256;
 
 struct SweepParams {
@@ -29,7 +32,8 @@ struct SweepParams {
     int st_policy;
     int pdl;        // launched with programmatic stream serialization: wait for the previous grid before loading
     unsigned prefetch; // L2 prefetch distance in sites along the traversal direction (0 = off)
-    double omega;   // overrelaxation parameter
+    double omega;   // overrelaxation parameter; MODE_VARIANT: omega (first order) or probability p
+    int variant;    // MODE_VARIANT: VARIANT_*
     double T;       // heatbath temperature (C13)
     uint32_t key0, key1, step; // Philox key = seed, step = annealing step (C14)
     unsigned* trials;          // optional: KP trial counts, index 3*s + subgroup
@@ -57,6 +61,39 @@ __device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[
     const T h0 = T(1) + w * d * (T(1) + (w - T(1)) * g0);
     const T f = w * (T(1) + (w - T(1)) * d);
     const T h1 = f * g1, h2 = f * g2, h3 = f * g3;
+    const T n2 = dot4(h0, h0, h1, h1, h2, h2, h3, h3);
+    if (n2 < T(1e-20)) { h[0] = g0; h[1] = g1; h[2] = g2; h[3] = g3; return; }
+    const T hn = gf_rsqrt<T>(n2);
+    h[0] = h0 * hn; h[1] = h1 * hn; h[2] = h2 * hn; h[3] = h3 * hn;
+}
+
+// SU(2) step of the variants.  First order (C17): g^w ~ 1 + w (g - 1), reprojected.  Stochastic relaxation (C18):
+// g^2 = (2 g0^2 - 1, 2 g0 gvec) with probability p, else g; the decision u < p is taken in double on
+// u = (2 (x >> 9) + 1) 2^-24 (exact), x the first word of the Philox block (site, sweep, parity<<2|subgroup,
+// 0x40000000), so fp32 and fp64 kernels decide exactly like the oracle.
+template <typename T>
+__device__ __forceinline__ void su2_variant_step(const T (&k)[4], int variant, double param, uint32_t key0,
+                                                 uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2, T (&h)[4])
+{
+    const T n2k = dot4(k[0], k[0], k[1], k[1], k[2], k[2], k[3], k[3]);
+    if (!(n2k >= Tiny<T>::sq)) { h[0] = T(1); h[1] = h[2] = h[3] = T(0); return; }
+    const T inv = gf_rsqrt<T>(n2k);
+    const T g0 = k[0] * inv, g1 = -k[1] * inv, g2 = -k[2] * inv, g3 = -k[3] * inv;
+    if (variant == VARIANT_STOCHASTIC) {
+        uint32_t x[4];
+        philox4x32_10(c0, c1, c2, 0x40000000u, key0, key1, x);
+        const double u = (double)(2u * (x[0] >> 9) + 1u) * (1.0 / 16777216.0);
+        if (u < param) {
+            const T t = T(2) * g0;
+            h[0] = gf_fma(t, g0, T(-1)); h[1] = t * g1; h[2] = t * g2; h[3] = t * g3;
+        } else {
+            h[0] = g0; h[1] = g1; h[2] = g2; h[3] = g3;
+        }
+        return;
+    }
+    const T w = (T)param;
+    const T h0 = gf_fma(w, g0 - T(1), T(1));
+    const T h1 = w * g1, h2 = w * g2, h3 = w * g3;
     const T n2 = dot4(h0, h0, h1, h1, h2, h2, h3, h3);
     if (n2 < T(1e-20)) { h[0] = g0; h[1] = g1; h[2] = g2; h[3] = g3; return; }
     const T hn = gf_rsqrt<T>(n2);
@@ -181,6 +218,10 @@ struct SweepKernel {
         su2_project<I, J>(K, k);
         if (MODE == MODE_OVERRELAX) {
             su2_overrelax_step<T>(k, (T)p.omega, h);
+        } else if (MODE == MODE_VARIANT) {
+            su2_variant_step<T>(k, p.variant, p.omega, p.key0, p.key1, site_canon, p.step,
+                                ((uint32_t)p.parity << 2) | (uint32_t)SUB, h);
+            (void)early;
         } else {
             unsigned ntr = su2_heatbath_step<T>(k, (T)p.T, p.key0, p.key1, site_canon, p.step,
                                                 ((uint32_t)p.parity << 2) | (uint32_t)SUB, early, h);

@@ -1,6 +1,6 @@
 // gf_sweep_inst.cu -- one translation unit per (precision, reals-per-link): compiled four times by build.py with
 //   -DGF_INST_FP64={0,1} -DGF_INST_R={12,18}
-// so the twenty-four half-sweep kernels build in parallel.  Each unit exports one launcher and one
+// so the thirty-six half-sweep kernels build in parallel.  Each unit exports one launcher and one
 // attribute query, declared in gf_internal.h.
 #include "gf_internal.h"
 #include "gf_sweep.cuh"
@@ -31,6 +31,10 @@ static sweep_fn pick(int tps, int mode)
         if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX>;
         if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX>;
         if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_OVERRELAX>;
+    } else if (mode == MODE_VARIANT) {
+        if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_VARIANT>;
+        if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_VARIANT>;
+        if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_VARIANT>;
     } else if (mode == MODE_HEATBATH) {
         if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_HEATBATH>;
         if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_HEATBATH>;

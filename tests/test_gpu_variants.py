@@ -1,0 +1,122 @@
+"""CUDA path vs oracle for the update variants (gf_relax: first-order overrelaxation, stochastic relaxation;
+gf_anneal_micro: microcanonical sweeps inside the annealing).  Tolerances as for the second-order sweep
+(north_star): per link 1e-12 (fp64) / 5e-5 (fp32) after one sweep; decisions (g^2 taken or not) are taken in
+double on both sides from the same Philox word, so they must be identical in fp32 too."""
+import numpy as np
+import pytest
+
+import gf_inputs
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL_LINK = {"fp64": 1e-12, "fp32": 5e-5}
+ORC_GAUGE = {"landau": oracle.LANDAU, "coulomb": oracle.COULOMB}
+
+
+@pytest.fixture(scope="module")
+def gfm():
+    import torch
+
+    assert torch.cuda.is_available()
+    import paper_1209_4008_b200 as m
+
+    m.load_library()
+    return m
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("R", [18, 12])
+@pytest.mark.parametrize("tps", [0, 1, 2, 4])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("update,param", [(1, 1.6), (2, 0.35)])
+def test_one_sweep_links(gfm, precision, R, tps, gauge, update, param):
+    dims = (8, 6, 4, 10)
+    U = gf_inputs.smooth_random(dims, 0.4, 51)
+    fx = gfm.GaugeFixer(dims, precision=precision, gauge=gauge, reals_per_link=R)
+    gfm.gf_set_tuning(fx.ctx, tps, 0 if tps == 0 else 64)
+    fx.load(U)
+    ref = fx.download() if precision == "fp32" and update == 2 else U.copy()
+    fx.relax(update, param, 1, seed=13)
+    got = fx.download()
+    oracle.relax(ref, dims, update, param, 1, 13, ORC_GAUGE[gauge])
+    assert np.abs(got - ref).max() <= TOL_LINK[precision]
+    fx.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_stochastic_sweep_counter_and_limits(gfm, precision):
+    """three sweeps in one call use sweep counters 0,1,2 (as the oracle); p = 1 conserves F (C19); p = 0 is
+    relaxation; the update 0 of gf_relax is gf_overrelax"""
+    dims = (6, 4, 4, 8)
+    U = gf_inputs.smooth_random(dims, 0.4, 52)
+    fx = gfm.GaugeFixer(dims, precision=precision)
+    fx.load(U)
+    ref = fx.download()
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 0.5, 3, seed=2**40 + 5)
+    oracle.relax(ref, dims, oracle.UPDATE_STOCHASTIC, 0.5, 3, 2**40 + 5)
+    assert np.abs(fx.download() - ref).max() <= 3 * TOL_LINK[precision]
+    F0 = fx.functional()
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 1.0, 2, seed=1)
+    assert abs(fx.functional() - F0) < (1e-13 if precision == "fp64" else 2e-6)
+    a = fx.download()
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 0.0, 1, seed=1)
+    b = a.copy()
+    oracle.overrelax(b, dims, 1.0, 1)
+    assert np.abs(fx.download() - b).max() <= TOL_LINK[precision]
+    fx.load(U)
+    fx.relax(gfm.GF_UPDATE_OVERRELAX2, 1.7, 2)
+    c = fx.download()
+    fx.load(U)
+    fx.overrelax(1.7, 2)
+    assert np.array_equal(c, fx.download())
+    fx.close()
+
+
+def test_first_order_fixes_the_gauge(gfm):
+    """config 1 with the first-order update: theta < 1e-14 and F -> 1 (P1), per-sweep parity with the oracle"""
+    dims = (4, 4, 4, 4)
+    U = gf_inputs.trivial_orbit(dims, 1)
+    fx = gfm.GaugeFixer(dims, precision="fp64")
+    fx.load(U)
+    for sweep in range(300):
+        fx.relax(gfm.GF_UPDATE_OVERRELAX1, 1.3, 1)
+        oracle.relax(U, dims, oracle.UPDATE_OVERRELAX1, 1.3, 1)
+        if sweep < 20:
+            assert np.abs(fx.download() - U).max() <= 1e-12
+        if fx.theta() < 1e-14:
+            break
+    assert fx.theta() < 1e-14 and abs(fx.functional() - 1.0) < 1e-12
+    assert fx.theta() == pytest.approx(oracle.theta(U, dims), rel=1e-6, abs=1e-24)
+    fx.close()
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_anneal_micro_decisions_fp64(gfm, gauge):
+    import torch
+
+    dims = (6, 4, 4, 8)
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.5, 53)
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge=gauge)
+    trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
+    gfm.gf_set_trial_buffer(fx.ctx, trials)
+    fx.load(U)
+    fx.anneal(1.2, 0.3, 2, 7, n_micro=2)
+    ref_trials = oracle.anneal_micro(U, dims, 1.2, 0.3, 2, 2, 7, ORC_GAUGE[gauge], trials=True)
+    assert np.array_equal(trials.cpu().numpy().reshape(V, 3), ref_trials)
+    # 2 heatbath + 4 microcanonical sweeps; the g^2 sweeps do not damp rounding differences (they grow by
+    # roughly 5x per sweep from 1e-14), so the bar after 6 sweeps is 1e-10
+    assert np.abs(fx.download() - U).max() <= 1e-10
+    fx.close()
+
+
+def test_argument_errors(gfm):
+    ctx = gfm.gf_create(4, 4, 4, 4)
+    for args in ((1234, 1, 2.0, 1), (1234, 1, 0.5, 1), (1234, 2, 1.5, 1), (1234, 2, -0.1, 1), (1234, 3, 1.5, 1),
+                 (1234, 1, 1.5, -1), (0, 1, 1.5, 1)):
+        with pytest.raises(gfm.GFError):
+            gfm.gf_relax(ctx, *args)
+    with pytest.raises(gfm.GFError):
+        gfm.gf_anneal_micro(ctx, 1234, 1.0, 1.0, 1, -1, 1)
+    gfm.gf_destroy(ctx)
