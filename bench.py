@@ -50,7 +50,9 @@ WORKLOADS = {
     "48^3x64-f32-r18-coulomb-anneal": dict(dims=(48, 48, 48, 64), precision="fp32", R=18, gauge="coulomb",
                                            omega=1.7, eps=0.5, seed=5, anneal=True),
 }
-ALSO_DEFAULT = ["32^4-f32-r12", "32^4-f64-r18"]
+# further workloads timed after the main one in the default run (lattices above 32^4: at most 3 steps each)
+ALSO_DEFAULT = ["32^4-f32-r12", "32^4-f64-r18", "32^4-f64-r12", "64^4-f32-r18", "64^4-f64-r18",
+                "48^3x64-f32-r18-coulomb", "48^3x64-f32-r18-coulomb-anneal"]
 
 
 def volume(dims):
@@ -360,7 +362,7 @@ def main():
                 acc.setdefault(row["workload"], []).append(float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]))
         traffic = {k: int(sum(v) / len(v)) for k, v in acc.items()}
 
-    def measure(name, wl, sampler=None, bar=None):
+    def measure(name, wl, sampler=None, bar=None, steps=steps):
         U, gdims, tiled = base_field(wl)
         canon = device_canonical(U, gdims, wl["dims"], tiled)
         fx = make_fixer(gfm, wl, canon)
@@ -370,6 +372,8 @@ def main():
         total, in_sw, launches, F, th, clocks = time_device(gfm, fx, wl, sweeps, steps, warmup, stream, bar, sampler)
         regs, spill = gfm.gf_kernel_info(fx.ctx, 1 if wl.get("anneal") else 0)
         fx.close()
+        del fx
+        torch.cuda.empty_cache()
         return dict(U=U if not tiled else None, total=total, in_sweeps=in_sw, launches=launches, F=F, theta=th,
                     clocks=clocks, regs=regs, spill=spill, tiled=tiled, gdims=gdims,
                     roofline=roofline_entry(wl, sweeps, steps, in_sw, traffic.get(name)))
@@ -406,11 +410,12 @@ def main():
     also = []
     for name in [n for n in args.also.split(",") if n and n != args.workload]:
         wl = WORKLOADS[name]
-        a = measure(name, wl)
         Va = volume(wl["dims"])
-        va = Va * sweeps * steps / a["total"]
+        a_steps = steps if Va <= 32**4 else min(steps, 3)
+        a = measure(name, wl, steps=a_steps)
+        va = Va * sweeps * a_steps / a["total"]
         also.append({"workload": name, "value": va, "unit": "site-updates/s", "gflops_paper_model": va * FLOP_PER_SITE / 1e9,
-                     "ms_per_step": a["total"] / steps * 1e3, "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
+                     "steps": a_steps, "ms_per_step": a["total"] / a_steps * 1e3, "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
                      "regs_per_thread": a["regs"], "spill_bytes": a["spill"]})
 
     cpu = None
