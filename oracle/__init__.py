@@ -70,6 +70,7 @@ def _load():
         "orc_su2_square": (None, [_vp, _vp]),
         "orc_site_relax": (None, [N, _int, _vp, ctypes.c_long, _int, _dbl, ctypes.c_uint64, ctypes.c_uint32, _vp]),
         "orc_relax": (None, [N, _int, _vp, _int, _dbl, _int, ctypes.c_uint64, _vp]),
+        "orc_fix": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp]),
         "orc_anneal_micro": (None, [N, _int, _vp, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp]),
     }
     for name, (res, args) in sig.items():
@@ -139,6 +140,16 @@ def relax(U, dims, update: int, param: float, nsweeps: int, seed: int = 0, gauge
     _load().orc_relax(N, gauge, _field(U, V), int(update), float(param), int(nsweeps), int(seed),
                       sq.ctypes.data if squared else None)
     return sq
+
+
+def fix(U, dims, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int, seed: int = 0,
+        gauge: int = LANDAU):
+    """Alg. 1 outer loop: returns (sweeps done, theta, F)"""
+    N, V = _dims(dims)
+    th, F = ctypes.c_double(), ctypes.c_double()
+    n = _load().orc_fix(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
+                        int(max_sweeps), int(seed), ctypes.byref(th), ctypes.byref(F))
+    return int(n), th.value, F.value
 
 
 def anneal_micro(U, dims, T_start: float, T_end: float, nsteps: int, n_micro: int, seed: int, gauge: int = LANDAU,

@@ -577,3 +577,26 @@ void orc_anneal_micro(const int N[4], int gauge, double *U, double T_start, doub
         orc_relax(N, gauge, U, ORC_UPDATE_STOCHASTIC, 2.0, n_micro, seed, NULL); /* p = 2 > u always: g^2 */
     }
 }
+
+/* ------------------------------------------------------------------------------------------------ */
+/* Alg. 1 outer loop ("while precision theta not reached"), with the paper's cadence of   */
+/* the check (F and theta are evaluated after every `check_every`-th iteration; C11):    */
+/* sweep in chunks of check_every (the last chunk is cut at max_sweeps) until theta < theta_tol        */
+/* (Coulomb: max over timeslices, C12).  Each chunk is one orc_relax call, so the sweep counter of the */
+/* stochastic decisions restarts with every chunk.  Returns the number of sweeps done.                 */
+/* ------------------------------------------------------------------------------------------------ */
+int orc_fix(const int N[4], int gauge, double *U, int update, double param, double theta_tol, int check_every,
+            int max_sweeps, uint64_t seed, double *theta_out, double *F_out)
+{
+    int done = 0;
+    double th = orc_theta_report(N, gauge, U);
+    while (th >= theta_tol && done < max_sweeps) {
+        int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
+        orc_relax(N, gauge, U, update, param, n, seed, NULL);
+        done += n;
+        th = orc_theta_report(N, gauge, U);
+    }
+    if (theta_out) *theta_out = th;
+    if (F_out) *F_out = orc_functional(N, gauge, U);
+    return done;
+}

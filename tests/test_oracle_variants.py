@@ -135,3 +135,28 @@ def test_anneal_micro_reduces_to_anneal_and_conserves_between_heatbath():
     oracle.anneal(d, dims, 0.8, 0.8, 1, 7)
     assert np.abs(c - d).max() > 0.05
     assert abs(npl.functional(c, dims, 4) - npl.functional(d, dims, 4)) < 1e-13
+
+
+def test_fix_loop_config1_and_cadence():
+    """Alg. 1 outer loop: config 1 (golden/config1_expectation.txt) stops below theta_tol with F = 1; the number of
+    sweeps is the first multiple of check_every at which a sweep-by-sweep run is below the tolerance; max_sweeps
+    cuts the last chunk; an already fixed field needs 0 sweeps"""
+    dims = (4, 4, 4, 4)
+    U0 = gf_inputs.trivial_orbit(dims, 1)
+    U = U0.copy()
+    first = None
+    for n in range(1, 501):
+        oracle.overrelax(U, dims, 1.7, 1)
+        if oracle.theta(U, dims) < 1e-14:
+            first = n
+            break
+    assert first is not None
+    for every in (1, 7, 100):
+        V = U0.copy()
+        n, th, F = oracle.fix(V, dims, oracle.UPDATE_OVERRELAX2, 1.7, 1e-14, every, 500)
+        assert n == -(-first // every) * every and th < 1e-14 and abs(F - 1) < 1e-12
+    V = U0.copy()
+    n, th, F = oracle.fix(V, dims, oracle.UPDATE_OVERRELAX2, 1.7, 1e-14, 7, 10)
+    assert n == 10 and th == oracle.theta(V, dims) and F == oracle.functional(V, dims)
+    n, th, F = oracle.fix(U, dims, oracle.UPDATE_OVERRELAX2, 1.7, 1e-14, 5, 10)
+    assert n == 0
