@@ -115,6 +115,17 @@ int gf_theta(gf_ctx* ctx, const void* U_native_dev, double* theta_host);
 /* per-timeslice theta_t = (1 / (V_s N_c)) sum_{x in slice t} tr[Delta Delta^dagger]; theta_host_Nt: Nt doubles */
 int gf_theta_slices(gf_ctx* ctx, const void* U_native_dev, double* theta_host_Nt);
 
+/* ---- Alg. 1 with its stop rule -------------------------------------------------------------------------------- */
+
+/* "while precision theta not reached do" with the check after every `check_every`-th sweep
+ * (C11): gf_theta; while theta >= theta_tol and fewer than max_sweeps sweeps done: gf_relax(update,
+ * param, min(check_every, max_sweeps - done), seed); gf_theta.  Coulomb: theta = max over timeslices (C12).
+ * sweeps_done / theta_host / F_host (each may be NULL) receive the number of sweeps, the last theta and F.
+ * Synchronises at every check.  Errors as gf_relax; GF_EINVAL also for check_every < 1, max_sweeps < 0. */
+int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double theta_tol, int check_every,
+           int max_sweeps, unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host,
+           void* stream);
+
 /* ---- host-buffer convenience path (what a user with a configuration in host memory calls) ---------------- */
 
 /* U_canon_host (canonical fp64, V*72 doubles) is copied to the device, packed, swept `nsweeps` times at

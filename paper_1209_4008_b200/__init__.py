@@ -41,6 +41,7 @@ SIGNATURES = {
     "gf_anneal": (_i, [_vp, _vp, _d, _d, _i, _ull, _vp]),
     "gf_relax": (_i, [_vp, _vp, _i, _d, _i, _ull, _vp]),
     "gf_anneal_micro": (_i, [_vp, _vp, _d, _d, _i, _i, _ull, _vp]),
+    "gf_fix": (_i, [_vp, _vp, _i, _d, _d, _i, _i, _ull, _pi, _pd, _pd, _vp]),
     "gf_functional": (_i, [_vp, _vp, _pd]),
     "gf_theta": (_i, [_vp, _vp, _pd]),
     "gf_theta_slices": (_i, [_vp, _vp, _pd]),
@@ -156,6 +157,16 @@ def gf_relax(ctx, U, update: int, param: float, nsweeps: int, seed: int = 0, str
 def gf_anneal_micro(ctx, U, T_start: float, T_end: float, nsteps: int, n_micro: int, seed: int, stream=None) -> None:
     _check(ctx, load_library().gf_anneal_micro(ctx, _ptr(U), float(T_start), float(T_end), int(nsteps), int(n_micro),
                                               int(seed), _stream(stream)))
+
+
+def gf_fix(ctx, U, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int, seed: int = 0,
+           stream=None):
+    """Alg. 1 with its stop rule; returns (sweeps done, theta, F)"""
+    n, th, F = ctypes.c_int(), ctypes.c_double(), ctypes.c_double()
+    _check(ctx, load_library().gf_fix(ctx, _ptr(U), int(update), float(param), float(theta_tol), int(check_every),
+                                     int(max_sweeps), int(seed), ctypes.byref(n), ctypes.byref(th), ctypes.byref(F),
+                                     _stream(stream)))
+    return n.value, th.value, F.value
 
 
 def gf_functional(ctx, U) -> float:
@@ -284,6 +295,10 @@ class GaugeFixer:
 
     def anneal(self, T_start: float, T_end: float, nsteps: int, seed: int, stream=None, n_micro: int = 0):
         gf_anneal_micro(self.ctx, self.U, T_start, T_end, nsteps, n_micro, seed, stream)
+
+    def fix(self, theta_tol: float, update: int = GF_UPDATE_OVERRELAX2, param: float = 1.7, check_every: int = 100,
+            max_sweeps: int = 100000, seed: int = 0, stream=None):
+        return gf_fix(self.ctx, self.U, update, param, theta_tol, check_every, max_sweeps, seed, stream)
 
     def relax(self, update: int, param: float, nsweeps: int, seed: int = 0, stream=None):
         gf_relax(self.ctx, self.U, update, param, nsweeps, seed, stream)

@@ -416,6 +416,32 @@ extern "C" int gf_theta_slices(gf_ctx* c, const void* U, double* theta_host_Nt)
     return GF_OK;
 }
 
+extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta_tol, int check_every, int max_sweeps,
+                      unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (U == nullptr) return fail(c, GF_EINVAL, "gf_fix: U is NULL");
+    if (check_every < 1) return fail(c, GF_EINVAL, "gf_fix: check_every = %d < 1", check_every);
+    if (max_sweeps < 0) return fail(c, GF_EINVAL, "gf_fix: max_sweeps = %d < 0", max_sweeps);
+    if (!(theta_tol >= 0.0)) return fail(c, GF_EINVAL, "gf_fix: theta_tol = %g < 0", theta_tol);
+    c->last_stream = (cudaStream_t)stream;
+    int done = 0;
+    double th = 0.0;
+    int rc = gf_theta(c, U, &th);
+    // Alg. 1: "while precision theta not reached", checked every check_every-th sweep
+    while (rc == GF_OK && th >= theta_tol && done < max_sweeps) {
+        const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
+        rc = gf_relax(c, U, update, param, n, seed, stream);
+        done += n;
+        if (rc == GF_OK) rc = gf_theta(c, U, &th);
+    }
+    if (rc != GF_OK) return rc;
+    if (sweeps_done) *sweeps_done = done;
+    if (theta_host) *theta_host = th;
+    if (F_host) return gf_functional(c, U, F_host);
+    return GF_OK;
+}
+
 extern "C" int gf_overrelax_host(gf_ctx* c, double* U_host, double omega, int nsweeps, double* F_host, double* theta_host)
 {
     if (c == nullptr) return GF_EINVAL;

@@ -120,3 +120,34 @@ def test_argument_errors(gfm):
     with pytest.raises(gfm.GFError):
         gfm.gf_anneal_micro(ctx, 1234, 1.0, 1.0, 1, -1, 1)
     gfm.gf_destroy(ctx)
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_fix_loop_matches_oracle(gfm, gauge):
+    """Alg. 1 with its stop rule (gf_fix vs orc_fix): same number of sweeps, theta within 1e-6 relative"""
+    dims = (6, 6, 6, 4)
+    U = gf_inputs.smooth_random(dims, 0.3, 54)
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge=gauge)
+    fx.load(U)
+    n, th, F = fx.fix(1e-10, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=10, max_sweeps=2000)
+    n_ref, th_ref, F_ref = oracle.fix(U, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-10, 10, 2000, 0, ORC_GAUGE[gauge])
+    assert n == n_ref and 0 < n < 2000 and th < 1e-10
+    assert th == pytest.approx(th_ref, rel=1e-6) and F == pytest.approx(F_ref, rel=1e-10)
+    if gauge == "coulomb":
+        assert max(fx.theta_slices()) == th
+    # cut by max_sweeps; zero sweeps when already fixed
+    assert fx.fix(1e-10, max_sweeps=50)[0] == 0
+    assert fx.fix(0.0, check_every=7, max_sweeps=10)[0] == 10
+    with pytest.raises(gfm.GFError):
+        fx.fix(1e-10, check_every=0)
+    fx.close()
+
+
+def test_fix_config1_fp32_and_stochastic(gfm):
+    dims = (4, 4, 4, 4)
+    U = gf_inputs.trivial_orbit(dims, 1)
+    fx = gfm.GaugeFixer(dims, precision="fp32")
+    fx.load(U)
+    n, th, F = fx.fix(1e-11, gfm.GF_UPDATE_STOCHASTIC, 0.6, check_every=5, max_sweeps=1000, seed=3)
+    assert n < 1000 and th < 1e-11 and abs(F - 1) < 1e-5
+    fx.close()
