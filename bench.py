@@ -240,16 +240,17 @@ def time_e2e(gfm, w, U_host_pinned, sweeps, steps, warmup):
     prec = gfm.GF_FP64 if w["precision"] == "fp64" else gfm.GF_FP32
     ctx = gfm.gf_create(*w["dims"], prec, gfm.GF_COULOMB if w["gauge"] == "coulomb" else gfm.GF_LANDAU)
     gfm.gf_set_storage(ctx, w["R"])
+    call = gfm.gf_overrelax_host_f32 if U_host_pinned.dtype == torch.float32 else gfm.gf_overrelax_host
     for _ in range(warmup):
-        gfm.gf_overrelax_host(ctx, U_host_pinned, w["omega"], sweeps)
+        call(ctx, U_host_pinned, w["omega"], sweeps)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(steps):
-        gfm.gf_overrelax_host(ctx, U_host_pinned, w["omega"], sweeps)
+        call(ctx, U_host_pinned, w["omega"], sweeps)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     gfm.gf_destroy(ctx)
-    nbytes = volume(w["dims"]) * 72 * 8
+    nbytes = U_host_pinned.numel() * U_host_pinned.element_size()
     return dt, nbytes, nbytes + 16
 
 
@@ -399,12 +400,18 @@ def main():
 
             Nx, Ny, Nz, Nt = m["gdims"]
             U = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(-1, 4, 3, 3)
-        host = torch.from_numpy(U.view("float64").reshape(-1)).pin_memory()
+        # an fp32 context takes its configuration as float (gf_overrelax_host_f32), an fp64 one as double
+        host = torch.from_numpy(U.view("float64").reshape(-1))
+        if w["precision"] == "fp32":
+            host = host.to(torch.float32)
+        host = host.pin_memory()
         e_steps = max(1, min(steps, 5))
         dt, h2d, d2h = time_e2e(gfm, w, host, sweeps, e_steps, 1)
         e2e = {"value": world * V * sweeps * e_steps / dt, "unit": "site-updates/s", "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": e_steps, "ms_per_step": dt / e_steps * 1e3,
-               "call": "gf_overrelax_host (canonical fp64 field in pinned host memory in, fixed field + F + theta out)"}
+               "call": ("gf_overrelax_host_f32" if w["precision"] == "fp32" else "gf_overrelax_host") +
+                       " (canonical field in pinned host memory in, fixed field + F + theta out; element type = the "
+                       "context's precision)"}
         del host
 
     also = []

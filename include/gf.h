@@ -135,6 +135,11 @@ int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double the
 int gf_overrelax_host(gf_ctx* ctx, double* U_canon_host, double omega, int nsweeps, double* F_host,
                       double* theta_host);
 
+/* The same with the canonical field held as float (V*72 floats, same element order): what a user of an fp32
+ * context has in memory; halves the bytes over PCIe.  Works for fp64 contexts too (the field is widened on pack). */
+int gf_overrelax_host_f32(gf_ctx* ctx, float* U_canon_host, double omega, int nsweeps, double* F_host,
+                          double* theta_host);
+
 /* ---- tuning and diagnostics ------------------------------------------------------------------------------ */
 
 /* Launch shape of the sweep kernels: threads_per_site in {1,2,4} (1: one thread holds all 8 links of a site;

@@ -46,6 +46,7 @@ SIGNATURES = {
     "gf_theta": (_i, [_vp, _vp, _pd]),
     "gf_theta_slices": (_i, [_vp, _vp, _pd]),
     "gf_overrelax_host": (_i, [_vp, _vp, _d, _i, _pd, _pd]),
+    "gf_overrelax_host_f32": (_i, [_vp, _vp, _d, _i, _pd, _pd]),
     "gf_set_tuning": (_i, [_vp, _i, _i]),
     "gf_set_reunit": (_i, [_vp, _i]),
     "gf_set_l2_reversal": (_i, [_vp, _i]),
@@ -193,6 +194,14 @@ def gf_overrelax_host(ctx, U_canon_host, omega: float, nsweeps: int):
     F, th = ctypes.c_double(), ctypes.c_double()
     _check(ctx, load_library().gf_overrelax_host(ctx, _ptr(U_canon_host), float(omega), int(nsweeps),
                                                 ctypes.byref(F), ctypes.byref(th)))
+    return F.value, th.value
+
+
+def gf_overrelax_host_f32(ctx, U_canon_host, omega: float, nsweeps: int):
+    """as gf_overrelax_host with the canonical field held as float32 (numpy complex64 (V,4,3,3) or pinned tensor)"""
+    F, th = ctypes.c_double(), ctypes.c_double()
+    _check(ctx, load_library().gf_overrelax_host_f32(ctx, _ptr(U_canon_host), float(omega), int(nsweeps),
+                                                    ctypes.byref(F), ctypes.byref(th)))
     return F.value, th.value
 
 

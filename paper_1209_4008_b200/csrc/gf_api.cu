@@ -442,23 +442,49 @@ extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta
     return GF_OK;
 }
 
-extern "C" int gf_overrelax_host(gf_ctx* c, double* U_host, double omega, int nsweeps, double* F_host, double* theta_host)
+// host-buffer path, canonical field in host memory as double (elem = 8) or float (elem = 4)
+static int overrelax_host_impl(gf_ctx* c, void* U_host, size_t elem, double omega, int nsweeps, double* F_host,
+                               double* theta_host, const char* who)
 {
     if (c == nullptr) return GF_EINVAL;
-    if (U_host == nullptr) return fail(c, GF_EINVAL, "gf_overrelax_host: U_canon_host is NULL");
-    const size_t canon_bytes = (size_t)c->L.H * 2 * 72 * sizeof(double);
+    if (U_host == nullptr) return fail(c, GF_EINVAL, "%s: U_canon_host is NULL", who);
+    const size_t canon_bytes = (size_t)c->L.H * 2 * 72 * sizeof(double); // staging sized for the larger element
+    const size_t copy_bytes = (size_t)c->L.H * 2 * 72 * elem;
     cudaError_t e;
-    if (c->d_canon == nullptr && (e = cudaMalloc(&c->d_canon, canon_bytes)) != cudaSuccess) { c->d_canon = nullptr; return cuda_fail(c, e, "gf_overrelax_host: staging allocation"); }
-    if (c->d_native == nullptr && (e = cudaMalloc(&c->d_native, gf_field_bytes(c))) != cudaSuccess) { c->d_native = nullptr; return cuda_fail(c, e, "gf_overrelax_host: staging allocation"); }
+    if (c->d_canon == nullptr && (e = cudaMalloc(&c->d_canon, canon_bytes)) != cudaSuccess) { c->d_canon = nullptr; return cuda_fail(c, e, "host path: staging allocation"); }
+    if (c->d_native == nullptr && (e = cudaMalloc(&c->d_native, gf_field_bytes(c))) != cudaSuccess) { c->d_native = nullptr; return cuda_fail(c, e, "host path: staging allocation"); }
     cudaStream_t st = c->last_stream;
-    if ((e = cudaMemcpyAsync(c->d_canon, U_host, canon_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(c, e, "gf_overrelax_host: H2D copy");
-    int rc = gf_pack(c, c->d_canon, c->d_native, st);
+    if ((e = cudaMemcpyAsync(c->d_canon, U_host, copy_bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(c, e, "host path: H2D copy");
+    int rc;
+    if (elem == 8) rc = gf_pack(c, c->d_canon, c->d_native, st);
+    else {
+        e = launch_pack_f32(c->precision, c->R, c->L, (const float*)c->d_canon, c->d_native, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "host path: pack");
+        c->launches += 1;
+        rc = GF_OK;
+    }
     if (rc == GF_OK) rc = gf_overrelax(c, c->d_native, omega, nsweeps, st);
-    if (rc == GF_OK) rc = gf_unpack(c, c->d_native, c->d_canon, st);
     if (rc != GF_OK) return rc;
-    if ((e = cudaMemcpyAsync(U_host, c->d_canon, canon_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(c, e, "gf_overrelax_host: D2H copy");
+    if (elem == 8) rc = gf_unpack(c, c->d_native, c->d_canon, st);
+    else {
+        e = launch_unpack_f32(c->precision, c->R, c->L, c->d_native, (float*)c->d_canon, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "host path: unpack");
+        c->launches += 1;
+    }
+    if (rc != GF_OK) return rc;
+    if ((e = cudaMemcpyAsync(U_host, c->d_canon, copy_bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(c, e, "host path: D2H copy");
     if (F_host != nullptr && (rc = gf_functional(c, c->d_native, F_host)) != GF_OK) return rc;
     if (theta_host != nullptr && (rc = gf_theta(c, c->d_native, theta_host)) != GF_OK) return rc;
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(c, e, "gf_overrelax_host: synchronise");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(c, e, "host path: synchronise");
     return GF_OK;
+}
+
+extern "C" int gf_overrelax_host(gf_ctx* c, double* U_host, double omega, int nsweeps, double* F_host, double* theta_host)
+{
+    return overrelax_host_impl(c, U_host, sizeof(double), omega, nsweeps, F_host, theta_host, "gf_overrelax_host");
+}
+
+extern "C" int gf_overrelax_host_f32(gf_ctx* c, float* U_host, double omega, int nsweeps, double* F_host, double* theta_host)
+{
+    return overrelax_host_impl(c, U_host, sizeof(float), omega, nsweeps, F_host, theta_host, "gf_overrelax_host_f32");
 }

@@ -12,23 +12,23 @@ constexpr int AUX_BLOCK = 256;
 // ---------------------------------------------------------------------------------------------------------
 // pack / unpack.  One thread per (half-site h, link block l = parity*4 + mu).
 // ---------------------------------------------------------------------------------------------------------
-template <typename T, int R>
-__global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, const double* __restrict__ canon, T* __restrict__ native)
+template <typename T, int R, typename S>
+__global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, const S* __restrict__ canon, T* __restrict__ native)
 {
     const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (unsigned long long)L.H * 8ull) return;
     const unsigned h = (unsigned)(gid % L.H);
     const int l = (int)(gid / L.H), parity = l >> 2, mu = l & 3;
     const Site s = decode_site(L, h, parity);
-    const double* src = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
+    const S* src = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
     cx<T> u[9];
 #pragma unroll
     for (int e = 0; e < 9; ++e) u[e] = {(T)src[2 * e], (T)src[2 * e + 1]};
     LinkIO<T, R>::store(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
 }
 
-template <typename T, int R>
-__global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* __restrict__ native, double* __restrict__ canon)
+template <typename T, int R, typename S>
+__global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* __restrict__ native, S* __restrict__ canon)
 {
     const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (unsigned long long)L.H * 8ull) return;
@@ -37,33 +37,53 @@ __global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* _
     const Site s = decode_site(L, h, parity);
     cx<T> u[9];
     LinkIO<T, R>::load(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
-    double* dst = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
+    S* dst = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
 #pragma unroll
-    for (int e = 0; e < 9; ++e) { dst[2 * e] = (double)u[e].re; dst[2 * e + 1] = (double)u[e].im; }
+    for (int e = 0; e < 9; ++e) { dst[2 * e] = (S)u[e].re; dst[2 * e + 1] = (S)u[e].im; }
+}
+
+// canon_f32: the canonical field holds float instead of double (host-buffer path of fp32 contexts)
+template <typename S>
+static cudaError_t launch_pack_t(int prec, int R, const Lattice& L, const S* canon, void* native, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (prec == 0 && R == 18) pack_kernel<float, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
+    else if (prec == 0 && R == 12) pack_kernel<float, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
+    else if (prec == 1 && R == 18) pack_kernel<double, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
+    else if (prec == 1 && R == 12) pack_kernel<double, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+template <typename S>
+static cudaError_t launch_unpack_t(int prec, int R, const Lattice& L, const void* native, S* canon, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (prec == 0 && R == 18) unpack_kernel<float, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
+    else if (prec == 0 && R == 12) unpack_kernel<float, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
+    else if (prec == 1 && R == 18) unpack_kernel<double, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
+    else if (prec == 1 && R == 12) unpack_kernel<double, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
 }
 
 cudaError_t launch_pack(int prec, int R, const Lattice& L, int, const double* canon, void* native, cudaStream_t st)
 {
-    const unsigned long long n = (unsigned long long)L.H * 8ull;
-    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
-    if (prec == 0 && R == 18) pack_kernel<float, 18><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
-    else if (prec == 0 && R == 12) pack_kernel<float, 12><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
-    else if (prec == 1 && R == 18) pack_kernel<double, 18><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
-    else if (prec == 1 && R == 12) pack_kernel<double, 12><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
-    else return cudaErrorInvalidValue;
-    return cudaGetLastError();
+    return launch_pack_t<double>(prec, R, L, canon, native, st);
 }
-
 cudaError_t launch_unpack(int prec, int R, const Lattice& L, int, const void* native, double* canon, cudaStream_t st)
 {
-    const unsigned long long n = (unsigned long long)L.H * 8ull;
-    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
-    if (prec == 0 && R == 18) unpack_kernel<float, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
-    else if (prec == 0 && R == 12) unpack_kernel<float, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
-    else if (prec == 1 && R == 18) unpack_kernel<double, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
-    else if (prec == 1 && R == 12) unpack_kernel<double, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
-    else return cudaErrorInvalidValue;
-    return cudaGetLastError();
+    return launch_unpack_t<double>(prec, R, L, native, canon, st);
+}
+cudaError_t launch_pack_f32(int prec, int R, const Lattice& L, const float* canon, void* native, cudaStream_t st)
+{
+    return launch_pack_t<float>(prec, R, L, canon, native, st);
+}
+cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, const void* native, float* canon, cudaStream_t st)
+{
+    return launch_unpack_t<float>(prec, R, L, native, canon, st);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -103,11 +123,8 @@ __global__ void __launch_bounds__(AUX_BLOCK) functional_kernel(Lattice L, int nd
     const uint64_t pol = make_l2_policy(POLICY_NORMAL);
     if (local < Hs) {
         const unsigned h = (unsigned)t * Hs + local;
-        for (int mu = 0; mu < nd; ++mu) {
-            cx<T> u[9];
-            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, h, u, pol);
-            acc += (double)u[0].re + (double)u[4].re + (double)u[8].re;
-        }
+        for (int mu = 0; mu < nd; ++mu)
+            acc += (double)LinkIO<T, R>::trace_re(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, h, pol);
     }
     block_sum_to(acc, partials + (size_t)blockIdx.y * gridDim.x + blockIdx.x);
 }

@@ -228,6 +228,15 @@ struct LinkIO<double, R> {
         }
         if (R == 12) rebuild_row2(u);
     }
+    // Re tr U from the diagonal planes alone (R = 12: rows 0,1 in full, entry (2,2) rebuilt)
+    static __device__ __forceinline__ double trace_re(const double* blk, size_t H, size_t h, uint64_t pol)
+    {
+        const double2* p = reinterpret_cast<const double2*>(blk) + h;
+        if (R == 18) return ldg(p, pol).x + ldg(p + 4 * H, pol).x + ldg(p + 8 * H, pol).x;
+        cx<double> u[9];
+        load(blk, H, h, u, pol);
+        return u[0].re + u[4].re + u[8].re;
+    }
     static __device__ __forceinline__ void prefetch(const double* blk, size_t H, size_t h)
     {
         const double2* p = reinterpret_cast<const double2*>(blk) + h;
@@ -260,6 +269,17 @@ struct LinkIO<float, R> {
         } else {
             rebuild_row2(u);
         }
+    }
+    static __device__ __forceinline__ double trace_re(const float* blk, size_t H, size_t h, uint64_t pol)
+    {
+        if (R == 18) {
+            const float4* p = reinterpret_cast<const float4*>(blk) + h;
+            return (double)ldg(p, pol).x + (double)ldg(p + 2 * H, pol).x +
+                   (double)ldg(reinterpret_cast<const float2*>(blk + 16 * H) + h, pol).x;
+        }
+        cx<float> u[9];
+        load(blk, H, h, u, pol);
+        return (double)u[0].re + (double)u[4].re + (double)u[8].re;
     }
     static __device__ __forceinline__ void prefetch(const float* blk, size_t H, size_t h)
     {

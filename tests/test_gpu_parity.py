@@ -316,6 +316,29 @@ def test_host_buffer_path(gfm, precision):
     assert th == pytest.approx(oracle.theta(ref, dims), rel=1e-6 if precision == "fp64" else 1e-3)
 
 
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_host_buffer_path_f32(gfm, precision):
+    """canonical field held as float: fp32 contexts give the same links as the double-buffer call bit for bit
+    (the pack rounds to the same fp32 numbers); fp64 contexts start from the widened floats"""
+    dims = (8, 4, 4, 6)
+    U = gf_inputs.smooth_random(dims, 0.4, 30)
+    U32 = U.astype(np.complex64)
+    prec = gfm.GF_FP64 if precision == "fp64" else gfm.GF_FP32
+    ref = U32.astype(np.complex128)  # the input as the library sees it
+    ctx = gfm.gf_create(*dims, prec, gfm.GF_LANDAU)
+    F, th = gfm.gf_overrelax_host_f32(ctx, U32, 1.7, 2)
+    gfm.gf_destroy(ctx)
+    if precision == "fp32":
+        ctx = gfm.gf_create(*dims, prec, gfm.GF_LANDAU)
+        Ud = U.copy()
+        F2, th2 = gfm.gf_overrelax_host(ctx, Ud, 1.7, 2)
+        gfm.gf_destroy(ctx)
+        assert np.array_equal(Ud.astype(np.complex64), U32) and F == F2 and th == th2
+    oracle.overrelax(ref, dims, 1.7, 2)
+    assert np.abs(U32.astype(np.complex128) - ref).max() <= 2 * TOL_LINK["fp32"]  # output is float either way
+    assert F == pytest.approx(oracle.functional(ref, dims), rel=TOL_F[precision])
+
+
 # ---------------------------------------------------------------------------------------------------------
 # launch-time options change scheduling and caching, never a bit of the result
 # ---------------------------------------------------------------------------------------------------------
