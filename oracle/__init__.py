@@ -71,6 +71,7 @@ def _load():
         "orc_site_relax": (None, [N, _int, _vp, ctypes.c_long, _int, _dbl, ctypes.c_uint64, ctypes.c_uint32, _vp]),
         "orc_relax": (None, [N, _int, _vp, _int, _dbl, _int, ctypes.c_uint64, _vp]),
         "orc_fix": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp]),
+        "orc_fix_slices": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp, _vp]),
         "orc_anneal_micro": (None, [N, _int, _vp, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp]),
     }
     for name, (res, args) in sig.items():
@@ -150,6 +151,17 @@ def fix(U, dims, update: int, param: float, theta_tol: float, check_every: int, 
     n = _load().orc_fix(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
                         int(max_sweeps), int(seed), ctypes.byref(th), ctypes.byref(F))
     return int(n), th.value, F.value
+
+
+def fix_slices(U, dims, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int, seed: int = 0,
+               gauge: int = COULOMB):
+    """Alg. 1 with the stop rule per timeslice (C20): returns (max sweeps, theta = max_t theta_t, F, sweeps per slice)"""
+    N, V = _dims(dims)
+    th, F = ctypes.c_double(), ctypes.c_double()
+    per = np.zeros(int(dims[3]), dtype=np.int32)
+    n = _load().orc_fix_slices(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
+                               int(max_sweeps), int(seed), per.ctypes.data, ctypes.byref(th), ctypes.byref(F))
+    return int(n), th.value, F.value, per
 
 
 def anneal_micro(U, dims, T_start: float, T_end: float, nsteps: int, n_micro: int, seed: int, gauge: int = LANDAU,

@@ -600,3 +600,58 @@ int orc_fix(const int N[4], int gauge, double *U, int update, double param, doub
     if (F_out) *F_out = orc_functional(N, gauge, U);
     return done;
 }
+
+/* ------------------------------------------------------------------------------------------------ */
+/* Coulomb gauge, "each timeslice fixed independently" (BASELINE.json configs[4]; C12, C20): K, F and  */
+/* theta of a site use the spatial links of its own timeslice only, so a timeslice whose theta_t is    */
+/* below the tolerance can be frozen: its sites are no longer updated (its theta_t then never changes,  */
+/* sweeps of the neighbouring slices only multiply the temporal links between them).                   */
+/* orc_relax_slices: as orc_relax, restricted to the sites of the timeslices with active[t] != 0.      */
+/* orc_fix_slices: Alg. 1 with the stop rule per timeslice: after every check_every sweeps the slices   */
+/* with theta_t < theta_tol are frozen for good; ends when none is active or at max_sweeps.            */
+/* sweeps_per_slice (Nt ints, may be NULL) receives the sweeps each slice got; returns their maximum.   */
+/* ------------------------------------------------------------------------------------------------ */
+void orc_relax_slices(const int N[4], int gauge, double *U, int update, double param, int nsweeps, uint64_t seed,
+                      const unsigned char *active)
+{
+    const long V = lat_volume(N);
+    const long Vs = (long)N[0] * N[1] * N[2];
+    for (int sweep = 0; sweep < nsweeps; ++sweep)
+        for (int parity = 0; parity < 2; ++parity) {
+#pragma omp parallel for schedule(static)
+            for (long s = 0; s < V; ++s)
+                if (active[s / Vs] && lat_parity(N, s) == parity)
+                    orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)sweep, NULL);
+        }
+}
+
+int orc_fix_slices(const int N[4], int gauge, double *U, int update, double param, double theta_tol, int check_every,
+                   int max_sweeps, uint64_t seed, int *sweeps_per_slice, double *theta_out, double *F_out)
+{
+    const int Nt = N[3];
+    unsigned char *active = (unsigned char *)malloc((size_t)Nt);
+    double *sl = (double *)malloc(sizeof(double) * (size_t)Nt);
+    int *count = (int *)calloc((size_t)Nt, sizeof(int));
+    int done = 0, any = 0;
+    orc_theta(N, gauge, U, sl);
+    for (int t = 0; t < Nt; ++t) { active[t] = sl[t] >= theta_tol; any |= active[t]; }
+    while (any && done < max_sweeps) {
+        int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
+        orc_relax_slices(N, gauge, U, update, param, n, seed, active);
+        done += n;
+        orc_theta(N, gauge, U, sl);
+        any = 0;
+        for (int t = 0; t < Nt; ++t) {
+            if (active[t]) count[t] += n;
+            active[t] = active[t] && sl[t] >= theta_tol; /* frozen slices stay frozen */
+            any |= active[t];
+        }
+    }
+    double m = sl[0];
+    for (int t = 1; t < Nt; ++t) if (sl[t] > m) m = sl[t];
+    if (theta_out) *theta_out = m;
+    if (F_out) *F_out = orc_functional(N, gauge, U);
+    if (sweeps_per_slice) memcpy(sweeps_per_slice, count, sizeof(int) * (size_t)Nt);
+    free(active); free(sl); free(count);
+    return done;
+}

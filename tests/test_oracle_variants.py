@@ -160,3 +160,30 @@ def test_fix_loop_config1_and_cadence():
     assert n == 10 and th == oracle.theta(V, dims) and F == oracle.functional(V, dims)
     n, th, F = oracle.fix(U, dims, oracle.UPDATE_OVERRELAX2, 1.7, 1e-14, 5, 10)
     assert n == 0
+
+
+def test_fix_slices_freezes_timeslices_independently():
+    """C20 (Coulomb, per-timeslice stop rule): every slice ends below the tolerance; slices need different numbers
+    of sweeps; the spatial links of slice t are exactly those of plain all-slice sweeping after n_t sweeps (the
+    slices decouple, C12); the result is still a gauge transform of the input (plaquette)"""
+    dims = (6, 6, 6, 8)
+    Vs = 6 * 6 * 6
+    U0 = gf_inputs.smooth_random(dims, 0.5, 45)
+    U = U0.copy()
+    n, th, F, per = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 5, 3000)
+    sl = oracle.theta_slices(U, dims, oracle.COULOMB)
+    assert n == per.max() and n < 3000 and th == sl.max() and (sl < 1e-9).all()
+    assert len(set(per.tolist())) > 1 and (per % 5 == 0).all() and per.min() > 0
+    assert abs(npl.plaquette(U, dims) - npl.plaquette(U0, dims)) < 1e-12
+    ref = U0.copy()
+    done = 0
+    for nt in sorted(set(per.tolist())):
+        oracle.overrelax(ref, dims, 1.5, nt - done, oracle.COULOMB)
+        done = nt
+        for t in np.nonzero(per == nt)[0]:
+            a = U[t * Vs:(t + 1) * Vs, :3]
+            b = ref[t * Vs:(t + 1) * Vs, :3]
+            assert np.array_equal(a, b), (t, nt)
+    # nothing to do on a fixed field
+    n2, _, _, per2 = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 5, 3000)
+    assert n2 == 0 and per2.max() == 0
