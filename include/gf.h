@@ -126,6 +126,14 @@ int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double the
            int max_sweeps, unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host,
            void* stream);
 
+/* Coulomb gauge, "each timeslice fixed independently" (C12, C20): as gf_fix, but a timeslice whose theta_t is below
+ * theta_tol at a check is frozen for good (its sites are no longer updated; K, F and theta_t of a slice depend on
+ * the spatial links of that slice alone), and the loop ends when no slice is active.  sweeps_done = sweeps of the
+ * slowest slice; sweeps_per_slice (Nt ints, may be NULL) the sweeps every slice got.  GF_EINVAL for a Landau ctx. */
+int gf_fix_slices(gf_ctx* ctx, void* U_native_dev, int update, double param, double theta_tol, int check_every,
+                  int max_sweeps, unsigned long long seed, int* sweeps_done, int* sweeps_per_slice,
+                  double* theta_host, double* F_host, void* stream);
+
 /* ---- host-buffer convenience path (what a user with a configuration in host memory calls) ---------------- */
 
 /* U_canon_host (canonical fp64, V*72 doubles) is copied to the device, packed, swept `nsweeps` times at

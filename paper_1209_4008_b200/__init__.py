@@ -42,6 +42,7 @@ SIGNATURES = {
     "gf_relax": (_i, [_vp, _vp, _i, _d, _i, _ull, _vp]),
     "gf_anneal_micro": (_i, [_vp, _vp, _d, _d, _i, _i, _ull, _vp]),
     "gf_fix": (_i, [_vp, _vp, _i, _d, _d, _i, _i, _ull, _pi, _pd, _pd, _vp]),
+    "gf_fix_slices": (_i, [_vp, _vp, _i, _d, _d, _i, _i, _ull, _pi, _pi, _pd, _pd, _vp]),
     "gf_functional": (_i, [_vp, _vp, _pd]),
     "gf_theta": (_i, [_vp, _vp, _pd]),
     "gf_theta_slices": (_i, [_vp, _vp, _pd]),
@@ -168,6 +169,17 @@ def gf_fix(ctx, U, update: int, param: float, theta_tol: float, check_every: int
                                      int(max_sweeps), int(seed), ctypes.byref(n), ctypes.byref(th), ctypes.byref(F),
                                      _stream(stream)))
     return n.value, th.value, F.value
+
+
+def gf_fix_slices(ctx, U, Nt: int, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int,
+                  seed: int = 0, stream=None):
+    """Coulomb gauge, stop rule per timeslice; returns (max sweeps, theta, F, list of sweeps per slice)"""
+    n, th, F = ctypes.c_int(), ctypes.c_double(), ctypes.c_double()
+    per = (ctypes.c_int * Nt)()
+    _check(ctx, load_library().gf_fix_slices(ctx, _ptr(U), int(update), float(param), float(theta_tol),
+                                            int(check_every), int(max_sweeps), int(seed), ctypes.byref(n), per,
+                                            ctypes.byref(th), ctypes.byref(F), _stream(stream)))
+    return n.value, th.value, F.value, list(per)
 
 
 def gf_functional(ctx, U) -> float:
@@ -308,6 +320,11 @@ class GaugeFixer:
     def fix(self, theta_tol: float, update: int = GF_UPDATE_OVERRELAX2, param: float = 1.7, check_every: int = 100,
             max_sweeps: int = 100000, seed: int = 0, stream=None):
         return gf_fix(self.ctx, self.U, update, param, theta_tol, check_every, max_sweeps, seed, stream)
+
+    def fix_slices(self, theta_tol: float, update: int = GF_UPDATE_OVERRELAX2, param: float = 1.7,
+                   check_every: int = 100, max_sweeps: int = 100000, seed: int = 0, stream=None):
+        return gf_fix_slices(self.ctx, self.U, self.dims[3], update, param, theta_tol, check_every, max_sweeps, seed,
+                             stream)
 
     def relax(self, update: int, param: float, nsweeps: int, seed: int = 0, stream=None):
         gf_relax(self.ctx, self.U, update, param, nsweeps, seed, stream)

@@ -246,6 +246,8 @@ static SweepParams base_params(gf_ctx* c, void* U)
     p.nd = c->gauge == GF_COULOMB ? 3 : 4;
     p.omega = 1.0;
     p.T = 1.0;
+    p.h_begin = 0;
+    p.h_count = c->L.H;
     p.ld_policy = c->ld_policy;
     p.st_policy = c->st_policy;
     p.pdl = c->pdl;
@@ -275,8 +277,10 @@ extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* str
 }
 
 // nsweeps sweeps (RED then BLACK) of one member of the relaxation family on `st`
+// active (may be NULL = all): Nt flags; only the sites of the flagged timeslices are updated, one launch per
+// maximal run of consecutive flagged slices (their half-site indices are contiguous) -- C20
 static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
-                      cudaStream_t st, const char* who)
+                      cudaStream_t st, const char* who, const unsigned char* active = nullptr)
 {
     c->last_stream = st;
     SweepParams p = base_params(c, U);
@@ -291,10 +295,25 @@ static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, i
             p.parity = parity;
             p.reunit = (reunit && parity == 0) ? 1 : 0; // every link is loaded once per half-sweep (C6)
             p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
-            cudaError_t e = launch_sweep(c, mode, p, st);
-            if (e != cudaSuccess) return cuda_fail(c, e, who);
+            if (active == nullptr) {
+                cudaError_t e = launch_sweep(c, mode, p, st);
+                if (e != cudaSuccess) return cuda_fail(c, e, who);
+                c->launches += 1;
+            } else {
+                const unsigned Hs = c->L.H / (unsigned)c->Nt; // half-sites per timeslice
+                for (int t = 0; t < c->Nt;) {
+                    if (!active[t]) { ++t; continue; }
+                    int t1 = t;
+                    while (t1 < c->Nt && active[t1]) ++t1;
+                    p.h_begin = (unsigned)t * Hs;
+                    p.h_count = (unsigned)(t1 - t) * Hs;
+                    cudaError_t e = launch_sweep(c, mode, p, st);
+                    if (e != cudaSuccess) return cuda_fail(c, e, who);
+                    c->launches += 1;
+                    t = t1;
+                }
+            }
             c->half_sweeps += 1;
-            c->launches += 1;
         }
         c->sweeps_done += 1;
     }
@@ -440,6 +459,58 @@ extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta
     if (theta_host) *theta_host = th;
     if (F_host) return gf_functional(c, U, F_host);
     return GF_OK;
+}
+
+extern "C" int gf_fix_slices(gf_ctx* c, void* U, int update, double param, double theta_tol, int check_every,
+                             int max_sweeps, unsigned long long seed, int* sweeps_done, int* sweeps_per_slice,
+                             double* theta_host, double* F_host, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (c->gauge != GF_COULOMB) return fail(c, GF_EINVAL, "gf_fix_slices: timeslices decouple in Coulomb gauge only (C12)");
+    if (U == nullptr) return fail(c, GF_EINVAL, "gf_fix_slices: U is NULL");
+    if (check_every < 1) return fail(c, GF_EINVAL, "gf_fix_slices: check_every = %d < 1", check_every);
+    if (max_sweeps < 0) return fail(c, GF_EINVAL, "gf_fix_slices: max_sweeps = %d < 0", max_sweeps);
+    if (!(theta_tol >= 0.0)) return fail(c, GF_EINVAL, "gf_fix_slices: theta_tol = %g < 0", theta_tol);
+    int mode, variant = 0;
+    switch (update) {
+    case GF_UPDATE_OVERRELAX2: mode = MODE_OVERRELAX; break;
+    case GF_UPDATE_OVERRELAX1: mode = MODE_VARIANT; variant = VARIANT_OVERRELAX1; break;
+    case GF_UPDATE_STOCHASTIC: mode = MODE_VARIANT; variant = VARIANT_STOCHASTIC; break;
+    default: return fail(c, GF_EINVAL, "gf_fix_slices: unknown update %d", update);
+    }
+    if (update == GF_UPDATE_STOCHASTIC ? !(param >= 0.0 && param <= 1.0) : !(param >= 1.0 && param < 2.0))
+        return fail(c, GF_EINVAL, "gf_fix_slices: parameter %g out of range for update %d", param, update);
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    const int Nt = c->Nt;
+    unsigned char* active = new (std::nothrow) unsigned char[Nt];
+    int* count = new (std::nothrow) int[Nt];
+    if (active == nullptr || count == nullptr) { delete[] active; delete[] count; return fail(c, GF_ENOMEM, "gf_fix_slices: host allocation"); }
+    int done = 0, any = 0;
+    int rc = reduce_to_host(c, U, true, "gf_fix_slices");
+    for (int t = 0; t < Nt && rc == GF_OK; ++t) { count[t] = 0; active[t] = c->h_out[2 + t] >= theta_tol; any |= active[t]; }
+    // Alg. 1 with the stop rule per timeslice: a slice below the tolerance at a check is frozen for good
+    while (rc == GF_OK && any && done < max_sweeps) {
+        const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
+        rc = run_sweeps(c, U, mode, variant, param, n, seed, st, "gf_fix_slices: kernel launch", active);
+        done += n;
+        if (rc == GF_OK) rc = reduce_to_host(c, U, true, "gf_fix_slices");
+        any = 0;
+        for (int t = 0; t < Nt && rc == GF_OK; ++t) {
+            if (active[t]) count[t] += n;
+            active[t] = active[t] && c->h_out[2 + t] >= theta_tol;
+            any |= active[t];
+        }
+    }
+    if (rc == GF_OK) {
+        if (sweeps_done) *sweeps_done = done;
+        if (sweeps_per_slice) memcpy(sweeps_per_slice, count, sizeof(int) * (size_t)Nt);
+        if (theta_host) *theta_host = c->h_out[1];
+        if (F_host) rc = gf_functional(c, U, F_host);
+    }
+    delete[] active;
+    delete[] count;
+    return rc;
 }
 
 // host-buffer path, canonical field in host memory as double (elem = 8) or float (elem = 4)

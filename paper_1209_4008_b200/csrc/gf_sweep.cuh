@@ -31,6 +31,7 @@ struct SweepParams {
     int ld_policy;  // L2 policy of the link loads / stores (POLICY_*, gf_device.cuh)
     int st_policy;
     int pdl;        // launched with programmatic stream serialization: wait for the previous grid before loading
+    unsigned h_begin, h_count; // half-site range updated by this launch (whole lattice: 0, H; a run of timeslices: C20)
     unsigned prefetch; // L2 prefetch distance in sites along the traversal direction (0 = off)
     double omega;   // overrelaxation parameter; MODE_VARIANT: omega (first order) or probability p
     int variant;    // MODE_VARIANT: VARIANT_*
@@ -240,9 +241,9 @@ struct SweepKernel {
     {
         const unsigned blk = p.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
         const unsigned gtid = blk * blockDim.x + threadIdx.x;
-        const unsigned slot = gtid / TPS;
+        const unsigned slot = p.h_begin + gtid / TPS;
         const int lane_mu0 = (int)(gtid % TPS) * NMU; // first direction this thread owns
-        const bool active = slot < p.L.H;             // inactive threads shadow site 0 and store nothing,
+        const bool active = slot < p.h_begin + p.h_count; // inactive threads shadow site 0 and store nothing,
         const Site s = decode_site(p.L, active ? slot : 0u, p.parity); // so warp shuffles stay converged
         const size_t H = p.L.H;
         T* const base = reinterpret_cast<T*>(p.U);

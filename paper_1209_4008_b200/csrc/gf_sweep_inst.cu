@@ -47,7 +47,8 @@ cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParam
 {
     sweep_fn fn = pick(tps, mode);
     if (fn == nullptr || block <= 0 || block > MAX_BLOCK || (block % 32) != 0) return cudaErrorInvalidValue;
-    const unsigned long long threads = (unsigned long long)p.L.H * (unsigned long long)tps;
+    const unsigned long long threads = (unsigned long long)p.h_count * (unsigned long long)tps;
+    if (p.h_count == 0) return cudaSuccess;
     const unsigned grid = (unsigned)((threads + (unsigned)block - 1ull) / (unsigned)block);
     if (!p.pdl) {
         fn<<<grid, block, 0, stream>>>(p);

@@ -151,3 +151,30 @@ def test_fix_config1_fp32_and_stochastic(gfm):
     n, th, F = fx.fix(1e-11, gfm.GF_UPDATE_STOCHASTIC, 0.6, check_every=5, max_sweeps=1000, seed=3)
     assert n < 1000 and th < 1e-11 and abs(F - 1) < 1e-5
     fx.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_fix_slices_matches_oracle(gfm, precision):
+    """Coulomb gauge, stop rule per timeslice (C20): gf_fix_slices vs orc_fix_slices -- the same sweeps for every
+    slice (fp64), every slice below the tolerance, links of the fp64 run within the N-sweep growth of 1e-12"""
+    dims = (6, 6, 6, 8)
+    U = gf_inputs.smooth_random(dims, 0.5, 45)
+    fx = gfm.GaugeFixer(dims, precision=precision, gauge="coulomb")
+    fx.load(U)
+    tol = 1e-9 if precision == "fp64" else 1e-8
+    n, th, F, per = fx.fix_slices(tol, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=5, max_sweeps=3000)
+    n_ref, th_ref, F_ref, per_ref = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, tol, 5, 3000)
+    sl = fx.theta_slices()
+    assert max(sl) < tol and th == max(sl) and n == max(per) and len(set(per)) > 1
+    if precision == "fp64":
+        assert per == per_ref.tolist() and n == n_ref
+        assert th == pytest.approx(th_ref, rel=1e-5) and F == pytest.approx(F_ref, rel=1e-10)
+        assert np.abs(fx.download() - U).max() < 1e-9
+    else:
+        assert abs(n - n_ref) <= 10 and F == pytest.approx(F_ref, rel=1e-5)
+    assert fx.fix_slices(tol, check_every=5)[0] == 0  # already fixed
+    fx.close()
+    lx = gfm.GaugeFixer(dims, precision=precision, gauge="landau")
+    with pytest.raises(gfm.GFError):
+        lx.fix_slices(1e-9)
+    lx.close()
