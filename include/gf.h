@@ -67,6 +67,12 @@ int gf_pack(gf_ctx* ctx, const double* U_canon_dev, void* U_native_dev, void* st
 /* native (device) -> canonical fp64 (device).  R12: row 2 is rebuilt from rows 0,1 (C16). */
 int gf_unpack(gf_ctx* ctx, const void* U_native_dev, double* U_canon_dev, void* stream);
 
+/* native field of `src` (its precision and storage) -> native field of `dst` (same lattice, any precision / storage):
+ * fp32 sweeps followed by an fp64 polish, or 18- <-> 12-real storage (row 2 rebuilt / dropped).  The gauge of the
+ * two contexts may differ.  Widening (fp32 -> fp64) re-orthonormalises every link in fp64 (rows 0,1 Gram-Schmidt,
+ * row 2 rebuilt), so the result is unitary to fp64 rounding.  GF_EINVAL: different extents, NULL or identical buffers. */
+int gf_convert(gf_ctx* src, const void* U_src_native_dev, gf_ctx* dst, void* U_dst_native_dev, void* stream);
+
 /* ---- the sweeps (device, in place, asynchronous on `stream`) --------------------------------------------- */
 
 /* `nsweeps` iterations of Alg. 1: for sublattice = RED (parity 0), BLACK (parity 1): for

@@ -37,6 +37,7 @@ SIGNATURES = {
     "gf_field_bytes": (_sz, [_vp]),
     "gf_pack": (_i, [_vp, _vp, _vp, _vp]),
     "gf_unpack": (_i, [_vp, _vp, _vp, _vp]),
+    "gf_convert": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "gf_overrelax": (_i, [_vp, _vp, _d, _i, _vp]),
     "gf_anneal": (_i, [_vp, _vp, _d, _d, _i, _ull, _vp]),
     "gf_relax": (_i, [_vp, _vp, _i, _d, _i, _ull, _vp]),
@@ -140,6 +141,10 @@ def gf_pack(ctx, U_canon_dev, U_native_dev, stream=None) -> None:
 
 def gf_unpack(ctx, U_native_dev, U_canon_dev, stream=None) -> None:
     _check(ctx, load_library().gf_unpack(ctx, _ptr(U_native_dev), _ptr(U_canon_dev), _stream(stream)))
+
+
+def gf_convert(src_ctx, U_src, dst_ctx, U_dst, stream=None) -> None:
+    _check(dst_ctx, load_library().gf_convert(src_ctx, _ptr(U_src), dst_ctx, _ptr(U_dst), _stream(stream)))
 
 
 def gf_overrelax(ctx, U, omega: float, nsweeps: int, stream=None) -> None:
@@ -309,6 +314,14 @@ class GaugeFixer:
         dev = torch.empty(self.V * 72, dtype=torch.float64, device="cuda")
         gf_unpack(self.ctx, self.U, dev)
         return dev.cpu().numpy().view("complex128").reshape(self.V, 4, 3, 3)
+
+    def convert_to(self, precision=None, gauge=None, reals_per_link=None) -> "GaugeFixer":
+        """a new GaugeFixer holding this field in another precision / storage (mixed-precision fixing)"""
+        other = GaugeFixer(self.dims, self.precision if precision is None else precision,
+                           self.gauge if gauge is None else gauge,
+                           self.R if reals_per_link is None else reals_per_link)
+        gf_convert(self.ctx, self.U, other.ctx, other.U)
+        return other
 
     # the method
     def overrelax(self, omega: float, nsweeps: int, stream=None):

@@ -320,6 +320,20 @@ static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, i
     return GF_OK;
 }
 
+extern "C" int gf_convert(gf_ctx* src, const void* U_src, gf_ctx* dst, void* U_dst, void* stream)
+{
+    if (src == nullptr || dst == nullptr) return GF_EINVAL;
+    if (U_src == nullptr || U_dst == nullptr) return fail(dst, GF_EINVAL, "gf_convert: NULL field");
+    if (src->Nx != dst->Nx || src->Ny != dst->Ny || src->Nz != dst->Nz || src->Nt != dst->Nt)
+        return fail(dst, GF_EINVAL, "gf_convert: the two contexts describe different lattices");
+    if (U_src == U_dst) return fail(dst, GF_EINVAL, "gf_convert: source and destination must be different buffers");
+    dst->last_stream = (cudaStream_t)stream;
+    cudaError_t e = launch_convert(src->precision, src->R, dst->precision, dst->R, dst->L, U_src, U_dst, dst->last_stream);
+    if (e != cudaSuccess) return cuda_fail(dst, e, "gf_convert");
+    dst->launches += 1;
+    return GF_OK;
+}
+
 extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void* stream)
 {
     if (c == nullptr) return GF_EINVAL;

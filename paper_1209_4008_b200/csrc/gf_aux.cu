@@ -86,6 +86,48 @@ cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, const void* nat
     return launch_unpack_t<float>(prec, R, L, native, canon, st);
 }
 
+// native -> native between precisions / storage formats (mixed-precision fixing: fp32 sweeps, fp64 polish)
+template <typename TS, int RS, typename TD, int RD>
+__global__ void __launch_bounds__(AUX_BLOCK) convert_kernel(Lattice L, const TS* __restrict__ src, TD* __restrict__ dst)
+{
+    const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (unsigned long long)L.H * 8ull) return;
+    const unsigned h = (unsigned)(gid % L.H);
+    const int l = (int)(gid / L.H);
+    const uint64_t pol = make_l2_policy(POLICY_NORMAL);
+    cx<TS> u[9];
+    LinkIO<TS, RS>::load(src + (size_t)l * RS * L.H, L.H, h, u, pol);
+    cx<TD> v[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) v[e] = {(TD)u[e].re, (TD)u[e].im};
+    // widening: the fp32 links are unitary to 1e-7 only; Gram-Schmidt in the wider type makes the fp64 field an
+    // SU(3) field to rounding, so that the polish starts from a proper configuration (C15)
+    if (sizeof(TD) > sizeof(TS)) reunitarise(v);
+    LinkIO<TD, RD>::store(dst + (size_t)l * RD * L.H, L.H, h, v, pol);
+}
+
+template <typename TS, int RS>
+static cudaError_t launch_convert_from(int dprec, int dR, const Lattice& L, const void* src, void* dst, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (dprec == 0 && dR == 18) convert_kernel<TS, RS, float, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (const TS*)src, (float*)dst);
+    else if (dprec == 0 && dR == 12) convert_kernel<TS, RS, float, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (const TS*)src, (float*)dst);
+    else if (dprec == 1 && dR == 18) convert_kernel<TS, RS, double, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (const TS*)src, (double*)dst);
+    else if (dprec == 1 && dR == 12) convert_kernel<TS, RS, double, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (const TS*)src, (double*)dst);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_convert(int sprec, int sR, int dprec, int dR, const Lattice& L, const void* src, void* dst, cudaStream_t st)
+{
+    if (sprec == 0 && sR == 18) return launch_convert_from<float, 18>(dprec, dR, L, src, dst, st);
+    if (sprec == 0 && sR == 12) return launch_convert_from<float, 12>(dprec, dR, L, src, dst, st);
+    if (sprec == 1 && sR == 18) return launch_convert_from<double, 18>(dprec, dR, L, src, dst, st);
+    if (sprec == 1 && sR == 12) return launch_convert_from<double, 12>(dprec, dR, L, src, dst, st);
+    return cudaErrorInvalidValue;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // reductions.  Grid (bx, 2*Nt): blockIdx.y = 2*t + parity, so every block lies inside one timeslice and the
 // Coulomb per-timeslice theta (C12) falls out of the same partials.

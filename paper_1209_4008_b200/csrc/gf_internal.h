@@ -26,6 +26,9 @@ cudaError_t launch_unpack(int prec, int R, const Lattice& L, int Nx, const void*
 cudaError_t launch_pack_f32(int prec, int R, const Lattice& L, const float* canon, void* native, cudaStream_t stream);
 cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, const void* native, float* canon, cudaStream_t stream);
 
+cudaError_t launch_convert(int sprec, int sR, int dprec, int dR, const Lattice& L, const void* src, void* dst,
+                           cudaStream_t stream);
+
 // Reduction scratch (device): partial sums per block, then a deterministic fixed-order final pass.
 //   functional: out[0] = sum_{x, mu<nd} Re tr U_mu(x) / (3 nd V)
 //   theta:      out[0] = theta over the whole lattice (eq. 2.5); out[1] = max_t theta_t; out[2+t] = theta_t

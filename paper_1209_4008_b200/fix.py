@@ -39,6 +39,8 @@ def main():
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--check-every", type=int, default=100)
     ap.add_argument("--max-sweeps", type=int, default=100000)
+    ap.add_argument("--polish", type=float, default=0.0, help="mixed precision: after the fp32 run, convert to fp64 "
+                    "(gf_convert) and continue to this tolerance")
     ap.add_argument("--all-slices", action="store_true", help="Coulomb: sweep every timeslice until the slowest is fixed")
     args = ap.parse_args()
 
@@ -89,6 +91,12 @@ def main():
         (n, th, F), sec = timed(lambda: fx.fix(args.tol, update, args.omega, args.check_every, args.max_sweeps, 1))
         print(f"relaxation ({args.update} {args.omega}): {n} sweeps in {sec:.3f} s ({V * max(n, 1) / sec:.3e} site-updates/s): "
               f"F = {F:.12f} theta = {th:.6e}")
+    if args.polish > 0.0 and args.precision == "fp32":
+        wide = fx.convert_to(precision="fp64")
+        fx.close()
+        fx = wide
+        (n, th, F), sec = timed(lambda: fx.fix(args.polish, update, args.omega, args.check_every, args.max_sweeps, 1))
+        print(f"fp64 polish ({args.update} {args.omega}): {n} sweeps in {sec:.3f} s: F = {F:.12f} theta = {th:.6e}")
     if args.out:
         gfm.gf_unpack(fx.ctx, fx.U, canon)
         np.save(args.out, canon.cpu().numpy().view("complex128").reshape(V, 4, 3, 3))

@@ -178,3 +178,41 @@ def test_fix_slices_matches_oracle(gfm, precision):
     with pytest.raises(gfm.GFError):
         lx.fix_slices(1e-9)
     lx.close()
+
+
+def test_convert_and_mixed_precision_fixing(gfm):
+    """gf_convert: fp64 -> fp32 rounds like gf_pack, fp32 -> fp64 re-orthonormalises in fp64, R18 <-> R12 rebuilds row 2; fp32 sweeps
+    followed by an fp64 polish reach theta < 1e-13 in few fp64 sweeps and the same maximum as the pure fp64 run"""
+    dims = (8, 8, 8, 8)
+    U = gf_inputs.smooth_random(dims, 0.3, 55)
+    a = gfm.GaugeFixer(dims, precision="fp64")
+    a.load(U)
+    b = a.convert_to(precision="fp32", reals_per_link=12)
+    c = gfm.GaugeFixer(dims, precision="fp32", reals_per_link=12)
+    c.load(U)
+    assert np.array_equal(b.download(), c.download())
+    d = b.convert_to(precision="fp64", reals_per_link=18)
+    wide = d.download()
+    assert np.abs(wide - b.download()).max() < 1e-6
+    uu, det = oracle.unitarity_defect(wide, dims)
+    assert uu < 1e-14 and det < 1e-14
+    c.close(); d.close()
+    # mixed precision
+    n32, th32, _ = b.fix(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=10, max_sweeps=5000)
+    e = b.convert_to(precision="fp64", reals_per_link=18)
+    n64, th64, F_mixed = e.fix(1e-13, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=10, max_sweeps=5000)
+    n_pure, th_pure, F_pure = a.fix(1e-13, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=10, max_sweeps=5000)
+    assert th32 < 1e-9 and th64 < 1e-13 and th_pure < 1e-13
+    assert n64 < n_pure / 2 and n32 + n64 <= n_pure + 40
+    assert F_mixed == pytest.approx(F_pure, rel=1e-6)
+    got = e.download()
+    uu, det = oracle.unitarity_defect(got, dims)
+    assert uu < 1e-12 and det < 1e-12  # widening re-orthonormalised the links
+    assert abs(oracle.plaquette(got, dims) - oracle.plaquette(U, dims)) < 1e-5
+    with pytest.raises(gfm.GFError):
+        other = gfm.gf_create(4, 4, 4, 4)
+        try:
+            gfm.gf_convert(a.ctx, a.U, other, a.U)
+        finally:
+            gfm.gf_destroy(other)
+    a.close(); b.close(); e.close()
