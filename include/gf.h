@@ -178,6 +178,13 @@ int gf_set_pdl(gf_ctx* ctx, int on);
  * into L2 the lines that the thread `sites` further on will load.  0 = off, -1 = automatic (default; chosen per
  * precision / storage / sweep kind from the measurements in profiles/). */
 int gf_set_prefetch(gf_ctx* ctx, int sites);
+/* Slab fusion of the two half-sweeps of a sweep through L2 (0 = off, default): RED and BLACK are launched as a
+ * wavefront over chunks of `chunk_slices` timeslices (BLACK on slice t after RED on t-1, t, t+1), so that BLACK
+ * finds the links RED has just written in L2.  Same updates, bit-identical results.  Used by gf_overrelax / gf_relax
+ * when Nt >= 4.  gf_fusion_schedule writes the launch order of one sweep as (parity, t_begin, t_end) triples
+ * (`backward`: walking t downwards) and returns their number (also when capacity is too small). */
+int gf_set_fusion(gf_ctx* ctx, int chunk_slices);
+int gf_fusion_schedule(int Nt, int chunk_slices, int backward, int* triples, int capacity);
 /* Optional debug output of gf_anneal: d_trials (device, V*3 unsigned, index 3*s + subgroup) receives the
  * number of Kennedy-Pendleton trials of every (site, subgroup) of the LAST step; NULL switches it off. */
 int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);

@@ -55,6 +55,8 @@ SIGNATURES = {
     "gf_set_l2_policy": (_i, [_vp, _i, _i]),
     "gf_set_pdl": (_i, [_vp, _i]),
     "gf_set_prefetch": (_i, [_vp, _i]),
+    "gf_set_fusion": (_i, [_vp, _i]),
+    "gf_fusion_schedule": (_i, [_i, _i, _i, _pi, _i]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
     "gf_launch_count": (_ull, [_vp]),
     "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
@@ -244,6 +246,21 @@ def gf_set_pdl(ctx, on: bool) -> None:
 
 def gf_set_prefetch(ctx, sites: int) -> None:
     _check(ctx, load_library().gf_set_prefetch(ctx, int(sites)))
+
+
+def gf_set_fusion(ctx, chunk_slices: int) -> None:
+    _check(ctx, load_library().gf_set_fusion(ctx, int(chunk_slices)))
+
+
+def gf_fusion_schedule(Nt: int, chunk_slices: int, backward: bool = False):
+    """launch order of one slab-fused sweep: list of (parity, t_begin, t_end)"""
+    lib = load_library()
+    n = lib.gf_fusion_schedule(int(Nt), int(chunk_slices), int(bool(backward)), None, 0)
+    if n < 0:
+        raise GFError(n, "gf_fusion_schedule: invalid arguments")
+    buf = (ctypes.c_int * (3 * n))()
+    lib.gf_fusion_schedule(int(Nt), int(chunk_slices), int(bool(backward)), buf, n)
+    return [(buf[3 * i], buf[3 * i + 1], buf[3 * i + 2]) for i in range(n)]
 
 
 def gf_set_trial_buffer(ctx, d_trials) -> None:

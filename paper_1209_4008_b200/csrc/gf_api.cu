@@ -21,6 +21,7 @@ struct gf_ctx {
     int ld_policy, st_policy;         // L2 eviction policy of the sweep's link loads / stores
     int pdl;                          // programmatic dependent launch of consecutive half-sweeps
     int prefetch;                     // L2 prefetch distance of the sweep kernels, in sites (0 = off)
+    int fuse_slices;                  // > 0: RED and BLACK of one sweep interleaved in chunks of that many timeslices
     unsigned long long sweeps_done;   // overrelaxation sweeps since creation (cadence of the fp32 reunitarisation)
     unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
     unsigned long long launches;
@@ -88,6 +89,7 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->ld_policy = POLICY_NORMAL; c->st_policy = POLICY_EVICT_LAST; // measured best: profiles/r1_variants.md
     c->pdl = 1;
     c->prefetch = -1; // automatic
+    c->fuse_slices = 0;
     c->sweeps_done = 0; c->half_sweeps = 0; c->launches = 0;
     c->d_trials = nullptr; c->last_stream = nullptr;
     c->d_canon = nullptr; c->d_native = nullptr;
@@ -276,6 +278,56 @@ extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* str
     return GF_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// L2 fusion of the two half-sweeps of one sweep.  BLACK on timeslice t needs
+// RED finished on t-1, t, t+1 (the only links a site shares with other timeslices are the temporal ones), so the
+// sweep can run as a wavefront in t: RED on a chunk of timeslices, then BLACK on the slices whose three RED
+// neighbours are done, and so on; the links BLACK reads were written by RED a moment ago and are still in L2,
+// and RED's dirty lines are overwritten by BLACK before they are written back.  Only the order of launches
+// changes: every (parity, site) is updated exactly once per sweep from the same inputs, results are bit-identical.
+// Schedule: triples (parity, t_begin, t_end) for one sweep; `backward` walks t from Nt-1 down (consecutive sweeps
+// alternate, so a sweep starts on the slices the previous one finished on).  Returns the number of triples.
+// ---------------------------------------------------------------------------------------------------------
+static int fusion_schedule(int Nt, int chunk, int backward, int* out, int cap)
+{
+    int n = 0;
+    auto emit = [&](int parity, int a, int b) { // slices [a, b) in walk coordinates
+        if (a >= b) return;
+        if (n < cap) {
+            out[3 * n] = parity;
+            out[3 * n + 1] = backward ? Nt - b : a;
+            out[3 * n + 2] = backward ? Nt - a : b;
+        }
+        ++n;
+    };
+    if (chunk < 1) chunk = 1;
+    int r = 0, b = 1; // RED done on walk slices [0, r); BLACK done on [1, b)
+    while (r < Nt) {
+        const int r1 = r + chunk < Nt ? r + chunk : Nt;
+        emit(0, r, r1);
+        r = r1;
+        const int b1 = r < Nt ? r - 1 : Nt; // BLACK on t needs RED on t+1; the last slice's t+1 is slice 0: done
+        if (b1 > b) { emit(1, b, b1); b = b1; }
+    }
+    if (Nt > 1) emit(1, 0, 1); // slice 0 needs RED on the last slice
+    else emit(1, 0, 1);
+    return n;
+}
+
+extern "C" int gf_fusion_schedule(int Nt, int chunk_slices, int backward, int* triples, int capacity)
+{
+    if (Nt < 1 || chunk_slices < 1 || capacity < 0 || (capacity > 0 && triples == nullptr)) return GF_EINVAL;
+    return fusion_schedule(Nt, chunk_slices, backward ? 1 : 0, triples, capacity);
+}
+
+extern "C" int gf_set_fusion(gf_ctx* c, int chunk_slices)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (chunk_slices < 0) return fail(c, GF_EINVAL, "gf_set_fusion: chunk_slices must be >= 0");
+    c->fuse_slices = chunk_slices;
+    return GF_OK;
+}
+
 // nsweeps sweeps (RED then BLACK) of one member of the relaxation family on `st`
 // active (may be NULL = all): Nt flags; only the sites of the flagged timeslices are updated, one launch per
 // maximal run of consecutive flagged slices (their half-site indices are contiguous) -- C20
@@ -291,6 +343,30 @@ static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, i
     for (int sweep = 0; sweep < nsweeps; ++sweep) {
         const bool reunit = c->reunit_every > 0 && ((c->sweeps_done + 1) % (unsigned long long)c->reunit_every) == 0;
         p.step = (uint32_t)sweep; // sweep counter of the random decisions (C18): restarts at 0 with every call
+        if (c->fuse_slices > 0 && active == nullptr && c->Nt >= 4) {
+            // slab-fused sweep: same updates, launched as a wavefront in t
+            int sched[3 * 260];
+            const int backward = (int)(c->sweeps_done & 1ull);
+            const int chunk = c->fuse_slices > c->Nt ? c->Nt : c->fuse_slices;
+            int n = fusion_schedule(c->Nt, chunk, backward, sched, 260);
+            if (n > 260) return fail(c, GF_EINVAL, "%s: fusion schedule too long (Nt = %d, chunk = %d)", who, c->Nt, chunk);
+            const unsigned Hs = c->L.H / (unsigned)c->Nt;
+            for (int i = 0; i < n; ++i) {
+                p.parity = sched[3 * i];
+                p.reunit = (reunit && p.parity == 0) ? 1 : 0;
+                p.reverse = backward;
+                p.h_begin = (unsigned)sched[3 * i + 1] * Hs;
+                p.h_count = (unsigned)(sched[3 * i + 2] - sched[3 * i + 1]) * Hs;
+                cudaError_t e = launch_sweep(c, mode, p, st);
+                if (e != cudaSuccess) return cuda_fail(c, e, who);
+                c->launches += 1;
+            }
+            p.h_begin = 0;
+            p.h_count = c->L.H;
+            c->half_sweeps += 2;
+            c->sweeps_done += 1;
+            continue;
+        }
         for (int parity = 0; parity < 2; ++parity) { // RED, BLACK
             p.parity = parity;
             p.reunit = (reunit && parity == 0) ? 1 : 0; // every link is loaded once per half-sweep (C6)

@@ -365,3 +365,23 @@ def test_pdl_l2_policy_and_reversal_are_bit_neutral(gfm, precision, R):
     with pytest.raises(gfm.GFError):
         gfm.gf_set_l2_policy(ctx, 3, 0)
     gfm.gf_destroy(ctx)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,R,gauge", [("fp64", 18, "landau"), ("fp32", 12, "coulomb"), ("fp32", 18, "landau")])
+@pytest.mark.parametrize("chunk", [1, 2, 3, 16])
+def test_slab_fusion_is_bit_neutral(gfm, precision, R, gauge, chunk):
+    """gf_set_fusion changes the order of launches only: every sweep variant gives the same bits as unfused"""
+    dims = (6, 4, 4, 10)
+    U = gf_inputs.smooth_random(dims, 0.4, 32)
+    outs = []
+    for fuse in (0, chunk):
+        fx = _fixer(gfm, dims, precision, gauge, R)
+        gfm.gf_set_fusion(fx.ctx, fuse)
+        fx.load(U)
+        fx.overrelax(1.7, 17)  # crosses the fp32 re-orthonormalisation at sweep 16
+        fx.relax(gfm.GF_UPDATE_STOCHASTIC, 0.4, 3, seed=5)
+        fx.relax(gfm.GF_UPDATE_OVERRELAX1, 1.5, 2)
+        outs.append(fx.download())
+        fx.close()
+    assert np.array_equal(outs[0], outs[1])
