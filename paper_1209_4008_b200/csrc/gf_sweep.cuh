@@ -243,7 +243,7 @@ struct SweepKernel {
         const unsigned gtid = blk * blockDim.x + threadIdx.x;
         const unsigned slot = p.h_begin + gtid / TPS;
         const int lane_mu0 = (int)(gtid % TPS) * NMU; // first direction this thread owns
-        const bool active = slot < p.h_begin + p.h_count; // inactive threads shadow site 0 and store nothing,
+        const bool active = gtid / TPS < p.h_count;        // inactive threads shadow site 0 and store nothing,
         const Site s = decode_site(p.L, active ? slot : 0u, p.parity); // so warp shuffles stay converged
         const size_t H = p.L.H;
         T* const base = reinterpret_cast<T*>(p.U);
