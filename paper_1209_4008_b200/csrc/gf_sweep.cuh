@@ -114,7 +114,15 @@ template <> struct KPMath<double> {
     static __device__ __forceinline__ double neglog(double u) { return -log(u); }
     // delta = (-ln u1 / alpha) cos^2 + (-ln u2 / alpha), in exactly this order, no FMA contraction: this
     // value decides acceptance and must follow the stated recipe operation by operation (C14)
-    static __device__ __forceinline__ double inv(double) { return 0.0; } // unused: the fp64 draw divides (C14)
+    // alpha = |k| / T exactly as the oracle forms it (sqrt, then division): it decides acceptance (C14)
+    static __device__ __forceinline__ void prep(double n2, double T, double& alpha, double& inv_alpha, double& inv_n)
+    {
+        const double n = sqrt(n2);
+        alpha = n / T;
+        inv_alpha = 0.0; // unused: the fp64 draw divides
+        inv_n = 1.0 / n;
+    }
+    static __device__ __forceinline__ double root(double x) { return sqrt(fmax(0.0, x)); }
     static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha, double)
     {
         return __dadd_rn(__dmul_rn(__ddiv_rn(l1, alpha), __dmul_rn(c, c)), __ddiv_rn(l2, alpha));
@@ -131,7 +139,14 @@ template <> struct KPMath<float> {
     static __device__ __forceinline__ float cos2pi(float u) { return __cosf(6.283185307179586f * u); }
     static __device__ __forceinline__ float sin2pi(float u) { return __sinf(6.283185307179586f * u); }
     static __device__ __forceinline__ float neglog(float u) { return -0.693147180559945f * __log2f(u); }
-    static __device__ __forceinline__ float inv(float alpha) { return 1.0f / alpha; }
+    // no division, no IEEE square root: 1/|k| by MUFU.RSQ + one Newton step, alpha and 1/alpha from it
+    static __device__ __forceinline__ void prep(float n2, float T, float& alpha, float& inv_alpha, float& inv_n)
+    {
+        inv_n = gf_rsqrt<float>(n2);
+        alpha = n2 * inv_n * __frcp_rn(T);
+        inv_alpha = T * inv_n;
+    }
+    static __device__ __forceinline__ float root(float x) { return x > 0.0f ? x * rsqrtf(x) : 0.0f; }
     static __device__ __forceinline__ float delta(float l1, float l2, float c, float alpha, float inv_alpha)
     {
         (void)alpha;
@@ -165,35 +180,46 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T tempera
                                                       const EarlyRandom& early, T (&g)[4])
 {
     using M = KPMath<T>;
-    T n = gf_sqrt<T>(k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3]);
-    if (n < Tiny<T>::n) { g[0] = T(1); g[1] = g[2] = g[3] = T(0); return 0u; }
-    const T alpha = n / temperature;
-    const T inv_alpha = M::inv(alpha);
-    const T inv_n = T(1) / n;
+    const T n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
+    if (!(n2 >= Tiny<T>::sq)) { g[0] = T(1); g[1] = g[2] = g[3] = T(0); return 0u; }
+    T alpha, inv_alpha, inv_n;
+    M::prep(n2, temperature, alpha, inv_alpha, inv_n);
     const T kc0 = k[0] * inv_n, kc1 = -k[1] * inv_n, kc2 = -k[2] * inv_n, kc3 = -k[3] * inv_n; // conj(khat)
-    uint32_t x[4] = {early.trial0[0], early.trial0[1], early.trial0[2], early.trial0[3]};
-    T h0 = T(1);
-    bool accepted = false;
+    // unit vector of the direction of hvec: data independent, computed ahead of the draw
+    const T cos_t = T(1) - T(2) * M::uni(early.dir[0]);
+    const T up = M::uni(early.dir[1]);
+    const T sin_t = M::root(T(1) - cos_t * cos_t);
+    const T e1 = sin_t * M::cos2pi(up), e2 = sin_t * M::sin2pi(up), e3 = cos_t;
+    // trial 0 from the words generated up front: straight-line code, so that it can be scheduled together with the
+    // link updates of the previous subgroup; only rejected lanes enter the loop
+    T h0;
     unsigned trial = 0;
-    for (; trial < 4096u; ++trial) {
-        if (trial > 0u) philox4x32_10(c0, c1, c2, trial, key0, key1, x);
-        T u1 = M::uni(x[0]), u2 = M::uni(x[1]), u3 = M::uni(x[2]), u4 = M::uni(x[3]);
-        T c = M::cos2pi(u3);
-        T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha, inv_alpha);
-        if (M::accept(u4, d)) { h0 = T(1) - d; accepted = true; break; }
+    bool accepted;
+    {
+        const T u1 = M::uni(early.trial0[0]), u2 = M::uni(early.trial0[1]), u3 = M::uni(early.trial0[2]),
+                u4 = M::uni(early.trial0[3]);
+        const T c = M::cos2pi(u3);
+        const T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha, inv_alpha);
+        accepted = M::accept(u4, d);
+        h0 = T(1) - d;
+    }
+    if (!accepted) {
+        uint32_t x[4];
+        for (trial = 1; trial < 4096u; ++trial) {
+            philox4x32_10(c0, c1, c2, trial, key0, key1, x);
+            const T u1 = M::uni(x[0]), u2 = M::uni(x[1]), u3 = M::uni(x[2]), u4 = M::uni(x[3]);
+            const T c = M::cos2pi(u3);
+            const T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha, inv_alpha);
+            if (M::accept(u4, d)) { h0 = T(1) - d; accepted = true; break; }
+        }
     }
     if (!accepted) {
         // h = identity  =>  g = conj(khat)
         g[0] = kc0; g[1] = kc1; g[2] = kc2; g[3] = kc3;
         return 4097u;
     }
-    T cos_t = T(1) - T(2) * M::uni(early.dir[0]);
-    T up = M::uni(early.dir[1]);
-    T r = gf_sqrt<T>(fmax(T(0), T(1) - h0 * h0));
-    T sin_t = gf_sqrt<T>(fmax(T(0), T(1) - cos_t * cos_t));
-    T h1 = r * sin_t * M::cos2pi(up);
-    T h2 = r * sin_t * M::sin2pi(up);
-    T h3 = r * cos_t;
+    const T r = M::root(T(1) - h0 * h0);
+    const T h1 = r * e1, h2 = r * e2, h3 = r * e3;
     // g = h (x) conj(khat):  (pq)_0 = p0 q0 - p.q,  (pq)_vec = p0 qvec + q0 pvec - pvec x qvec   (C13)
     g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3;
     g[1] = h0 * kc1 + kc0 * h1 - (h2 * kc3 - h3 * kc2);
