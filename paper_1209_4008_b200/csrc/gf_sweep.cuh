@@ -54,18 +54,23 @@ template <> struct Tiny<double> { static constexpr double n = 1e-300; static con
 template <typename T>
 __device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[4])
 {
+    // branch-free: the guards (C9) are selects at the end, so that the compiler can schedule this dependent chain
+    // together with the independent link updates of the previous subgroup
     const T n2k = dot4(k[0], k[0], k[1], k[1], k[2], k[2], k[3], k[3]);
-    if (!(n2k >= Tiny<T>::sq)) { h[0] = T(1); h[1] = h[2] = h[3] = T(0); return; }
-    const T inv = gf_rsqrt<T>(n2k);
+    const bool ok = n2k >= Tiny<T>::sq;
+    const T inv = gf_rsqrt<T>(ok ? n2k : T(1));
     const T g0 = k[0] * inv, g1 = -k[1] * inv, g2 = -k[2] * inv, g3 = -k[3] * inv;
     const T d = g0 - T(1);
     const T h0 = T(1) + w * d * (T(1) + (w - T(1)) * g0);
     const T f = w * (T(1) + (w - T(1)) * d);
     const T h1 = f * g1, h2 = f * g2, h3 = f * g3;
     const T n2 = dot4(h0, h0, h1, h1, h2, h2, h3, h3);
-    if (n2 < T(1e-20)) { h[0] = g0; h[1] = g1; h[2] = g2; h[3] = g3; return; }
-    const T hn = gf_rsqrt<T>(n2);
-    h[0] = h0 * hn; h[1] = h1 * hn; h[2] = h2 * hn; h[3] = h3 * hn;
+    const bool ok2 = n2 >= T(1e-20);
+    const T hn = gf_rsqrt<T>(ok2 ? n2 : T(1));
+    h[0] = ok ? (ok2 ? h0 * hn : g0) : T(1);
+    h[1] = ok ? (ok2 ? h1 * hn : g1) : T(0);
+    h[2] = ok ? (ok2 ? h2 * hn : g2) : T(0);
+    h[3] = ok ? (ok2 ? h3 * hn : g3) : T(0);
 }
 
 // SU(2) step of the variants.  First order (C17): g^w ~ 1 + w (g - 1), reprojected.  Stochastic relaxation (C18):
