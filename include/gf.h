@@ -161,8 +161,11 @@ int gf_overrelax_host_f32(gf_ctx* ctx, float* U_canon_host, double omega, int ns
  * shuffles), block = threads per block (multiple of 32, <= 256).  0 = automatic (the default): chosen per
  * (precision, storage) from the measurements in profiles/. */
 int gf_set_tuning(gf_ctx* ctx, int threads_per_site, int block);
-/* fp32 unitarity policy (C15): every `every`-th sweep the RED half-sweep re-orthonormalises rows 0,1 of each
- * link on load (and rebuilds row 2).  0 = never.  Default: 16 for fp32, 0 for fp64. */
+/* Unitarity policy (C15): every `every`-th sweep the RED half-sweep re-orthonormalises rows 0,1 of each link on load
+ * (and rebuilds row 2).  0 = never, -1 = automatic (default): 18-real storage fp32 every 16th sweep, fp64 never;
+ * 12-real storage (both precisions) every 16th overrelaxation sweep and every 4th heatbath / stochastic /
+ * microcanonical sweep -- with 12 reals the rebuilt row feeds norm errors back and they grow exponentially under
+ * large rotations. */
 int gf_set_reunit(gf_ctx* ctx, int every);
 /* Alternate the block traversal direction between consecutive half-sweeps so that the tail of one
  * half-sweep, still in L2, is what the next one reads first (1 = on, default; 0 = off). */

@@ -84,7 +84,7 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->L.Nxh = Nx / 2; c->L.Ny = Ny; c->L.Nz = Nz; c->L.Nt = Nt; c->L.H = (unsigned)(V / 2);
     c->tps = 0;   // 0 = automatic: resolved per (precision, storage, mode) by auto_tps()
     c->block = 0; // 0 = automatic
-    c->reunit_every = precision == GF_FP32 ? 16 : 0;
+    c->reunit_every = -1; // automatic: reunit_due()
     c->l2_reversal = 1;
     c->ld_policy = POLICY_NORMAL; c->st_policy = POLICY_EVICT_LAST; // measured best: profiles/r1_variants.md
     c->pdl = 1;
@@ -147,7 +147,7 @@ extern "C" int gf_set_tuning(gf_ctx* c, int tps, int block)
 extern "C" int gf_set_reunit(gf_ctx* c, int every)
 {
     if (c == nullptr) return GF_EINVAL;
-    if (every < 0) return fail(c, GF_EINVAL, "gf_set_reunit: every must be >= 0");
+    if (every < -1) return fail(c, GF_EINVAL, "gf_set_reunit: every must be >= 0, or -1 for automatic");
     c->reunit_every = every;
     return GF_OK;
 }
@@ -278,6 +278,19 @@ extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* str
     return GF_OK;
 }
 
+// Unitarity policy (C15).  Automatic cadence of the re-orthonormalisation on load (RED half-sweep, every link once):
+//   18-real storage: rounding makes the links drift linearly -- fp32 every 16th sweep, fp64 never;
+//   12-real storage: the rebuilt third row feeds the norm errors of rows 0,1 back into them, which grows
+//   EXPONENTIALLY under large rotations (measured x1.5-1.7 per heatbath sweep at T = 1, both precisions: fp32 loses
+//   unitarity after ~50 sweeps, fp64 after ~150) -- every 4th sweep for the hot updates (heatbath, stochastic /
+//   microcanonical), every 16th for overrelaxation, in fp32 and fp64.
+static bool reunit_due(const gf_ctx* c, bool hot)
+{
+    int every = c->reunit_every;
+    if (every < 0) every = c->R == 12 ? (hot ? 4 : 16) : (c->precision == GF_FP32 ? 16 : 0);
+    return every > 0 && ((c->sweeps_done + 1) % (unsigned long long)every) == 0;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // L2 fusion of the two half-sweeps of one sweep.  BLACK on timeslice t needs
 // RED finished on t-1, t, t+1 (the only links a site shares with other timeslices are the temporal ones), so the
@@ -341,7 +354,7 @@ static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, i
     p.key0 = (uint32_t)seed;
     p.key1 = (uint32_t)(seed >> 32);
     for (int sweep = 0; sweep < nsweeps; ++sweep) {
-        const bool reunit = c->reunit_every > 0 && ((c->sweeps_done + 1) % (unsigned long long)c->reunit_every) == 0;
+        const bool reunit = reunit_due(c, mode == MODE_VARIANT && variant == VARIANT_STOCHASTIC);
         p.step = (uint32_t)sweep; // sweep counter of the random decisions (C18): restarts at 0 with every call
         if (c->fuse_slices > 0 && active == nullptr && c->Nt >= 4) {
             // slab-fused sweep: same updates, launched as a wavefront in t
@@ -457,14 +470,17 @@ extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end,
         p.T = nsteps > 1 ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
         p.step = (uint32_t)step;
         p.trials = (step == nsteps - 1) ? c->d_trials : nullptr;
+        const bool reunit = reunit_due(c, true);
         for (int parity = 0; parity < 2; ++parity) {
             p.parity = parity;
+            p.reunit = (reunit && parity == 0) ? 1 : 0;
             p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
             cudaError_t e = launch_sweep(c, MODE_HEATBATH, p, st);
             if (e != cudaSuccess) return cuda_fail(c, e, "gf_anneal: kernel launch");
             c->half_sweeps += 1;
             c->launches += 1;
         }
+        c->sweeps_done += 1;
         // microcanonical sweeps g -> g^2 (C19): stochastic relaxation with p = 2 > u, i.e. always
         if (n_micro > 0) {
             int rc = run_sweeps(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, seed, st, "gf_anneal_micro: kernel launch");

@@ -216,3 +216,29 @@ def test_convert_and_mixed_precision_fixing(gfm):
         finally:
             gfm.gf_destroy(other)
     a.close(); b.close(); e.close()
+
+
+@pytest.mark.parametrize("precision,tol", [("fp32", 2e-5), ("fp64", 1e-12)])
+def test_r12_stays_unitary_under_hot_updates(gfm, precision, tol):
+    """12-real storage feeds norm errors of rows 0,1 back through the rebuilt row: without re-orthonormalisation
+    they grow exponentially under large rotations (measured: fp32 heatbath at T = 1 reaches O(1) after 60 sweeps,
+    fp64 diverges within a 200-step annealing).  With the automatic policy the links stay unitary and the plaquette
+    invariant; switching the policy off shows the growth."""
+    dims = (8, 8, 8, 8)
+    U = gf_inputs.smooth_random(dims, 0.4, 56)
+    P0 = oracle.plaquette(U, dims)
+    fx = gfm.GaugeFixer(dims, precision=precision, reals_per_link=12)
+    fx.load(U)
+    fx.anneal(1.0, 1.0, 60, 7)
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 1.0, 40, 3)
+    fx.anneal(1.4, 0.01, 100, 8, n_micro=1)
+    got = fx.download()
+    uu, det = oracle.unitarity_defect(got, dims)
+    assert uu < tol and det < tol
+    assert abs(oracle.plaquette(got, dims) - P0) < 20 * tol
+    gfm.gf_set_reunit(fx.ctx, 0)  # never: the instability shows
+    fx.load(U)
+    fx.anneal(1.0, 1.0, 60, 7)
+    uu_off, _ = oracle.unitarity_defect(fx.download(), dims)
+    assert uu_off > 1e3 * tol
+    fx.close()
