@@ -216,3 +216,30 @@ def test_config5_48x3x64_coulomb_anneal_sampled_sites(gfm):
     assert n_links_ok >= n_sites - 3, (n_links_ok, n_sites)
     fx.close()
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_config2_16x3x32_logs_every_100_sweeps(gfm, precision):
+    """BASELINE.json configs[1]: 16^3x32, eps 0.3, seed 2, omega 1.7, 1000 sweeps, F and theta logged every 100
+    sweeps -- the whole log against the oracle's.  F: relative 1e-10 (fp64) / 1e-5 (fp32); theta: relative 1e-6 in
+    fp64 while it is above the rounding floor (1e-24), fp32 within 5 % above its own floor (1e-13)."""
+    dims = (16, 16, 16, 32)
+    U = gf_inputs.smooth_random(dims, 0.3, 2)
+    fx = gfm.GaugeFixer(dims, precision=precision)
+    fx.load(U)
+    log, ref = [], []
+    for _ in range(10):
+        fx.overrelax(1.7, 100)
+        log.append((fx.functional(), fx.theta()))
+        oracle.overrelax(U, dims, 1.7, 100)
+        ref.append((oracle.functional(U, dims), oracle.theta(U, dims)))
+    for (F, th), (F_ref, th_ref) in zip(log, ref):
+        assert F == pytest.approx(F_ref, rel=TOL_F[precision])
+        if precision == "fp64":
+            assert th == pytest.approx(th_ref, rel=1e-6, abs=1e-24)
+        elif th_ref > 1e-13:
+            assert th == pytest.approx(th_ref, rel=5e-2)
+    assert ref[-1][1] < ref[0][1] * 1e-3  # theta falls by decades over the log
+    if precision == "fp64":
+        assert np.abs(fx.download() - U).max() < 1e-9
+    fx.close()
