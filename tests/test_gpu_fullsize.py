@@ -66,6 +66,28 @@ def test_config3_32x4_every_link_and_F_theta(gfm, field32, oracle32, precision, 
     fx.close()
 
 
+@pytest.fixture(scope="module")
+def oracle32_500(field32):
+    """the headline config run to its end by the oracle: 500 sweeps at omega = 1.7 (about 40 s on 16 cores)"""
+    dims = (32, 32, 32, 32)
+    U = field32.copy()
+    oracle.overrelax(U, dims, 1.7, 500)
+    return oracle.functional(U, dims), oracle.theta(U, dims)
+
+
+@pytest.mark.parametrize("precision,R", [("fp64", 18), ("fp32", 18), ("fp32", 12)])
+def test_config3_32x4_after_500_sweeps(gfm, field32, oracle32_500, precision, R):
+    """BASELINE.json configs[2] as stated: omega = 1.7, fixed 500 sweeps; F (relative 1e-10 fp64 / 1e-5 fp32) and
+    theta (relative 1e-6 fp64) against the oracle's"""
+    F_ref, th_ref = oracle32_500
+    fx = gfm.GaugeFixer((32, 32, 32, 32), precision=precision, reals_per_link=R)
+    fx.load(field32)
+    fx.overrelax(1.7, 500)
+    assert fx.functional() == pytest.approx(F_ref, rel=TOL_F[precision])
+    assert fx.theta() == pytest.approx(th_ref, rel=1e-6 if precision == "fp64" else 5e-2)
+    fx.close()
+
+
 def _tiled_device(U, gdims):
     import torch
 
