@@ -187,7 +187,9 @@ __global__ void __launch_bounds__(AUX_BLOCK) theta_kernel(Lattice L, int nd, con
         cx<double> K[9];
 #pragma unroll
         for (int e = 0; e < 9; ++e) K[e] = {0.0, 0.0};
-        for (int mu = 0; mu < nd; ++mu) {
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) { // unrolled: the loads of all directions are in flight together
+            if (mu >= nd) break;
             cx<T> f[9], b[9];
             LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, s.h, f, pol);
             LinkIO<T, R>::load(native + (size_t)((1 - parity) * 4 + mu) * R * L.H, L.H, backward_neighbour(L, s, mu), b, pol);
