@@ -181,6 +181,13 @@ int gf_set_pdl(gf_ctx* ctx, int on);
  * into L2 the lines that the thread `sites` further on will load.  0 = off, -1 = automatic (default; chosen per
  * precision / storage / sweep kind from the measurements in profiles/). */
 int gf_set_prefetch(gf_ctx* ctx, int sites);
+/* Coulomb gauge, treatment of the temporal links (C12): 0 = reading A: every half-sweep moves and multiplies all 8
+ * links of a site; 1 = reading B; -1 = automatic (default): B in fp32 (+14 % at one thread per site), A in fp64, and
+ * A when the site field cannot be allocated.  Reading B: the relaxation sweeps (gf_overrelax / gf_relax / gf_fix / gf_fix_slices)
+ * leave the temporal links in memory, accumulate g(x) in a site field owned by the context (V * 18 reals) and
+ * transform the temporal links once at the end of each call -- 14/16 of the bytes, same result up to rounding.
+ * Annealing sweeps always use reading A.  GF_EINVAL for a Landau context. */
+int gf_set_coulomb_reading(gf_ctx* ctx, int reading_b);
 /* Slab fusion of the two half-sweeps of a sweep through L2 (0 = off, default): RED and BLACK are launched as a
  * wavefront over chunks of `chunk_slices` timeslices (BLACK on slice t after RED on t-1, t, t+1), so that BLACK
  * finds the links RED has just written in L2.  Same updates, bit-identical results.  Used by gf_overrelax / gf_relax

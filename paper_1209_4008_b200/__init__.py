@@ -55,6 +55,7 @@ SIGNATURES = {
     "gf_set_l2_policy": (_i, [_vp, _i, _i]),
     "gf_set_pdl": (_i, [_vp, _i]),
     "gf_set_prefetch": (_i, [_vp, _i]),
+    "gf_set_coulomb_reading": (_i, [_vp, _i]),
     "gf_set_fusion": (_i, [_vp, _i]),
     "gf_fusion_schedule": (_i, [_i, _i, _i, _pi, _i]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
@@ -246,6 +247,10 @@ def gf_set_pdl(ctx, on: bool) -> None:
 
 def gf_set_prefetch(ctx, sites: int) -> None:
     _check(ctx, load_library().gf_set_prefetch(ctx, int(sites)))
+
+
+def gf_set_coulomb_reading(ctx, reading_b: bool) -> None:
+    _check(ctx, load_library().gf_set_coulomb_reading(ctx, -1 if reading_b is None else int(bool(reading_b))))
 
 
 def gf_set_fusion(ctx, chunk_slices: int) -> None:

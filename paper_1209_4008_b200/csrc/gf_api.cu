@@ -21,6 +21,8 @@ struct gf_ctx {
     int ld_policy, st_policy;         // L2 eviction policy of the sweep's link loads / stores
     int pdl;                          // programmatic dependent launch of consecutive half-sweeps
     int prefetch;                     // L2 prefetch distance of the sweep kernels, in sites (0 = off)
+    int coulomb_b;                    // Coulomb reading B: temporal links transformed once per call (C12)
+    void* d_gfield;                   // its accumulated g(x): V links of 18 reals
     int fuse_slices;                  // > 0: RED and BLACK of one sweep interleaved in chunks of that many timeslices
     unsigned long long sweeps_done;   // overrelaxation sweeps since creation (cadence of the fp32 reunitarisation)
     unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
@@ -90,6 +92,7 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->pdl = 1;
     c->prefetch = -1; // automatic
     c->fuse_slices = 0;
+    c->coulomb_b = -1; c->d_gfield = nullptr; // automatic: reading B in fp32, A in fp64 (uses_reading_b)
     c->sweeps_done = 0; c->half_sweeps = 0; c->launches = 0;
     c->d_trials = nullptr; c->last_stream = nullptr;
     c->d_canon = nullptr; c->d_native = nullptr;
@@ -116,6 +119,7 @@ extern "C" void gf_destroy(gf_ctx* c)
     if (c->h_out) cudaFreeHost(c->h_out);
     if (c->d_canon) cudaFree(c->d_canon);
     if (c->d_native) cudaFree(c->d_native);
+    if (c->d_gfield) cudaFree(c->d_gfield);
     delete c;
 }
 
@@ -197,9 +201,18 @@ extern "C" unsigned long long gf_launch_count(const gf_ctx* c) { return c ? c->l
 // bound and wants as many bytes in flight per SM as the register file allows -- few, fat threads in one-warp
 // blocks.  fp32 R18: one thread per site (8 links = 144 reals in registers); fp32 R12 and fp64: two threads per
 // site (forward+backward links of two directions each), K combined with one warp shuffle.
+// Coulomb reading B pays where one thread holds all links of a site (fp32: +14 % at R = 18, +4 % at R = 12); with two
+// threads per site the thread that drops the temporal links idles (fp64: -2 %), so automatic = fp32 only.
+static bool uses_reading_b(const gf_ctx* c, int mode)
+{
+    if (c->gauge != GF_COULOMB || mode == MODE_HEATBATH) return false;
+    return c->coulomb_b < 0 ? c->precision == GF_FP32 : c->coulomb_b != 0;
+}
+
 static int auto_tps(const gf_ctx* c, int mode)
 {
     if (c->tps) return c->tps;
+    if (c->precision == GF_FP32 && uses_reading_b(c, mode)) return 1;
     if (c->precision == GF_FP64) return 2;
     if (mode == MODE_HEATBATH) return 1; // the draw is done once per thread: one thread per site (R12: 0.83 vs 0.65)
     return c->R == 18 ? 1 : 2;
@@ -333,6 +346,14 @@ extern "C" int gf_fusion_schedule(int Nt, int chunk_slices, int backward, int* t
     return fusion_schedule(Nt, chunk_slices, backward ? 1 : 0, triples, capacity);
 }
 
+extern "C" int gf_set_coulomb_reading(gf_ctx* c, int reading_b)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (c->gauge != GF_COULOMB) return fail(c, GF_EINVAL, "gf_set_coulomb_reading: the context is not in Coulomb gauge");
+    c->coulomb_b = reading_b < 0 ? -1 : (reading_b ? 1 : 0);
+    return GF_OK;
+}
+
 extern "C" int gf_set_fusion(gf_ctx* c, int chunk_slices)
 {
     if (c == nullptr) return GF_EINVAL;
@@ -344,11 +365,12 @@ extern "C" int gf_set_fusion(gf_ctx* c, int chunk_slices)
 // nsweeps sweeps (RED then BLACK) of one member of the relaxation family on `st`
 // active (may be NULL = all): Nt flags; only the sites of the flagged timeslices are updated, one launch per
 // maximal run of consecutive flagged slices (their half-site indices are contiguous) -- C20
-static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
-                      cudaStream_t st, const char* who, const unsigned char* active = nullptr)
+static int run_sweeps_core(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
+                           cudaStream_t st, const char* who, const unsigned char* active, void* gfield)
 {
     c->last_stream = st;
     SweepParams p = base_params(c, U);
+    p.G = gfield;
     p.omega = param;
     p.variant = variant;
     p.key0 = (uint32_t)seed;
@@ -420,6 +442,31 @@ extern "C" int gf_convert(gf_ctx* src, const void* U_src, gf_ctx* dst, void* U_d
     cudaError_t e = launch_convert(src->precision, src->R, dst->precision, dst->R, dst->L, U_src, U_dst, dst->last_stream);
     if (e != cudaSuccess) return cuda_fail(dst, e, "gf_convert");
     dst->launches += 1;
+    return GF_OK;
+}
+
+// Coulomb reading B (gf_set_coulomb_reading): G = 1, the sweeps leave the temporal links alone and accumulate g(x) in
+// G, then one pass transforms the temporal links.  Reading A otherwise.
+static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
+                      cudaStream_t st, const char* who, const unsigned char* active = nullptr)
+{
+    if (!uses_reading_b(c, mode) || nsweeps == 0)
+        return run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, nullptr);
+    cudaError_t e;
+    if (c->d_gfield == nullptr && (e = cudaMalloc(&c->d_gfield, (size_t)c->L.H * 2 * 18 * real_size(c))) != cudaSuccess) {
+        c->d_gfield = nullptr;
+        (void)cudaGetLastError();
+        if (c->coulomb_b < 0) { // automatic choice and no room for the g(x) field: reading A needs none
+            c->coulomb_b = 0;
+            return run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, nullptr);
+        }
+        return cuda_fail(c, e, "Coulomb reading B: allocation of the g(x) field");
+    }
+    if ((e = launch_coulomb_init(c->precision, c->L, c->d_gfield, st)) != cudaSuccess) return cuda_fail(c, e, who);
+    int rc = run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, c->d_gfield);
+    if (rc != GF_OK) return rc;
+    if ((e = launch_coulomb_finish(c->precision, c->R, c->L, U, c->d_gfield, st)) != cudaSuccess) return cuda_fail(c, e, who);
+    c->launches += 2;
     return GF_OK;
 }
 

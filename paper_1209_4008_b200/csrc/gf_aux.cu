@@ -128,6 +128,71 @@ cudaError_t launch_convert(int sprec, int sR, int dprec, int dR, const Lattice& 
     return cudaErrorInvalidValue;
 }
 
+// Coulomb reading B (C12): G(x) = 1 before the sweeps; afterwards U_t(x) <- G(x) U_t(x) G(x+t)^dagger for every site.
+// G: 2 parity blocks of H links in the 18-real layout.
+template <typename T>
+__global__ void __launch_bounds__(AUX_BLOCK) coulomb_init_kernel(Lattice L, T* __restrict__ G)
+{
+    const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (unsigned long long)L.H * 2ull) return;
+    const unsigned h = (unsigned)(gid % L.H);
+    const int parity = (int)(gid / L.H);
+    cx<T> u[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) u[e] = {(e % 4 == 0) ? T(1) : T(0), T(0)};
+    LinkIO<T, 18>::store(G + (size_t)parity * 18 * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
+}
+
+template <typename T, int R>
+__global__ void __launch_bounds__(AUX_BLOCK) coulomb_finish_kernel(Lattice L, T* __restrict__ native, const T* __restrict__ G)
+{
+    const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (unsigned long long)L.H * 2ull) return;
+    const unsigned h = (unsigned)(gid % L.H);
+    const int parity = (int)(gid / L.H);
+    const uint64_t pol = make_l2_policy(POLICY_NORMAL);
+    const Site s = decode_site(L, h, parity);
+    // x + t_hat: other parity block, one timeslice up (periodic)
+    const unsigned st = (unsigned)L.Nxh * (unsigned)L.Ny * (unsigned)L.Nz;
+    const unsigned hf = s.t == L.Nt - 1 ? h - st * (unsigned)(L.Nt - 1) : h + st;
+    cx<T> u[9], g[9], gn[9], t[9];
+    T* blk = native + (size_t)(parity * 4 + 3) * R * L.H;
+    LinkIO<T, R>::load(blk, L.H, h, u, pol);
+    LinkIO<T, 18>::load(G + (size_t)parity * 18 * L.H, L.H, h, g, pol);
+    LinkIO<T, 18>::load(G + (size_t)(1 - parity) * 18 * L.H, L.H, hf, gn, pol);
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) t[3 * r + c] = g[3 * r] * u[c] + g[3 * r + 1] * u[3 + c] + g[3 * r + 2] * u[6 + c];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            u[3 * r + c] = cmul_cb(t[3 * r], gn[3 * c]) + cmul_cb(t[3 * r + 1], gn[3 * c + 1]) + cmul_cb(t[3 * r + 2], gn[3 * c + 2]);
+    LinkIO<T, R>::store(blk, L.H, h, u, pol);
+}
+
+cudaError_t launch_coulomb_init(int prec, const Lattice& L, void* G, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 2ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (prec == 0) coulomb_init_kernel<float><<<grid, AUX_BLOCK, 0, st>>>(L, (float*)G);
+    else coulomb_init_kernel<double><<<grid, AUX_BLOCK, 0, st>>>(L, (double*)G);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_coulomb_finish(int prec, int R, const Lattice& L, void* native, const void* G, cudaStream_t st)
+{
+    const unsigned long long n = (unsigned long long)L.H * 2ull;
+    const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
+    if (prec == 0 && R == 18) coulomb_finish_kernel<float, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (float*)native, (const float*)G);
+    else if (prec == 0 && R == 12) coulomb_finish_kernel<float, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (float*)native, (const float*)G);
+    else if (prec == 1 && R == 18) coulomb_finish_kernel<double, 18><<<grid, AUX_BLOCK, 0, st>>>(L, (double*)native, (const double*)G);
+    else if (prec == 1 && R == 12) coulomb_finish_kernel<double, 12><<<grid, AUX_BLOCK, 0, st>>>(L, (double*)native, (const double*)G);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // reductions.  Grid (bx, 2*Nt): blockIdx.y = 2*t + parity, so every block lies inside one timeslice and the
 // Coulomb per-timeslice theta (C12) falls out of the same partials.

@@ -29,6 +29,10 @@ cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, const void* nat
 cudaError_t launch_convert(int sprec, int sR, int dprec, int dR, const Lattice& L, const void* src, void* dst,
                            cudaStream_t stream);
 
+// Coulomb reading B: G(x) = 1; U_t(x) <- G(x) U_t(x) G(x+t)^dagger
+cudaError_t launch_coulomb_init(int prec, const Lattice& L, void* G, cudaStream_t stream);
+cudaError_t launch_coulomb_finish(int prec, int R, const Lattice& L, void* native, const void* G, cudaStream_t stream);
+
 // Reduction scratch (device): partial sums per block, then a deterministic fixed-order final pass.
 //   functional: out[0] = sum_{x, mu<nd} Re tr U_mu(x) / (3 nd V)
 //   theta:      out[0] = theta over the whole lattice (eq. 2.5); out[1] = max_t theta_t; out[2+t] = theta_t

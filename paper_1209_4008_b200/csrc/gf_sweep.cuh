@@ -38,6 +38,7 @@ struct SweepParams {
     double T;       // heatbath temperature (C13)
     uint32_t key0, key1, step; // Philox key = seed, step = annealing step (C14)
     unsigned* trials;          // optional: KP trial counts, index 3*s + subgroup
+    void* G;                   // Coulomb reading B (C12): accumulated g(x), 2 parity blocks of 18 reals per site
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -236,15 +237,21 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T tempera
 // ---------------------------------------------------------------------------------------------------------
 // the half-sweep kernel
 // ---------------------------------------------------------------------------------------------------------
-template <typename T, int R, int TPS, int MODE>
+// CB = Coulomb reading B (C12): the temporal links enter neither K nor F nor theta, they are only multiplied by
+// g(x).  Instead of moving them through every half-sweep, the thread that would own them accumulates
+// G(x) <- g(x) G(x) in a site field (18 reals, one link's worth instead of two) and the temporal links are
+// transformed once at the end of the call, U_t(x) <- G(x) U_t(x) G(x+t)^dagger (coulomb_finish_kernel): 14/16 of the
+// bytes of reading A, same result up to rounding.
+template <typename T, int R, int TPS, int MODE, bool CB = false>
 struct SweepKernel {
     static constexpr int NMU = 4 / TPS;
     using IO = LinkIO<T, R>;
+    using GIO = LinkIO<T, 18>;
 
     template <int I, int J, int SUB>
     static __device__ __forceinline__ void subgroup(const SweepParams& p, cx<T> (&K)[9], cx<T> (&F)[NMU][9],
                                                     cx<T> (&B)[NMU][9], uint32_t site_canon, bool record,
-                                                    const EarlyRandom& early)
+                                                    const EarlyRandom& early, int lane_mu0, cx<T> (&Gt)[9])
     {
         T k[4], h[4];
         su2_project<I, J>(K, k);
@@ -262,8 +269,12 @@ struct SweepKernel {
         const cx<T> a = {h[0], h[3]}, b = {h[2], h[1]}; // C4
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
-            su2_left<I, J>(a, b, F[m]);                 // U_mu(x)     <- G U_mu(x)
-            su2_right_dagger<I, J, 3>(a, b, B[m]);      // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
+            if (CB && lane_mu0 + m == 3) {
+                su2_left<I, J>(a, b, Gt);               // G(x) <- g G(x): the temporal links wait (reading B)
+            } else {
+                su2_left<I, J>(a, b, F[m]);             // U_mu(x)     <- G U_mu(x)
+                su2_right_dagger<I, J, 3>(a, b, B[m]);  // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
+            }
         }
         su2_left<I, J>(a, b, K);                        // K <- G K  (C8)
     }
@@ -303,6 +314,7 @@ struct SweepKernel {
                 for (int m = 0; m < NMU; ++m) {
                     const int mu = lane_mu0 + m;
                     const long long hbd = (long long)hb[m] + d;
+                    if (CB && mu == 3) continue;
                     IO::prefetch(base + (size_t)(p.parity * 4 + mu) * R * H, H, (size_t)hf);
                     if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, (size_t)hbd);
                 }
@@ -312,9 +324,13 @@ struct SweepKernel {
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
             const int mu = lane_mu0 + m;
+            if (CB && mu == 3) continue;
             IO::load(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.ld);
             IO::load(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.ld);
         }
+        cx<T> Gt[9];
+        const bool owns_t = CB && (lane_mu0 + NMU - 1 == 3); // the thread that would hold the temporal links
+        if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)p.parity * 18 * H, H, s.h, Gt, pol.ld);
         // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
         const uint32_t sc = canonical_index(s);
         EarlyRandom early[3];
@@ -331,7 +347,12 @@ struct SweepKernel {
         }
         if (p.reunit) {
 #pragma unroll
-            for (int m = 0; m < NMU; ++m) { reunitarise(F[m]); reunitarise(B[m]); }
+            for (int m = 0; m < NMU; ++m) {
+                if (CB && lane_mu0 + m == 3) continue;
+                reunitarise(F[m]);
+                reunitarise(B[m]);
+            }
+            if (owns_t) reunitarise(Gt);
         }
 
         // K(x) = sum_{mu < nd} [ U_mu(x) + U_mu(x-mu)^dagger ]   (eq. 2.3; C2)
@@ -340,7 +361,7 @@ struct SweepKernel {
         for (int e = 0; e < 9; ++e) K[e] = {T(0), T(0)};
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
-            if (lane_mu0 + m < p.nd) {
+            if (lane_mu0 + m < p.nd && !(CB && lane_mu0 + m == 3)) {
 #pragma unroll
                 for (int r = 0; r < 3; ++r)
 #pragma unroll
@@ -359,25 +380,27 @@ struct SweepKernel {
         }
 
         const bool record = active && (lane_mu0 == 0);
-        subgroup<0, 1, 0>(p, K, F, B, sc, record, early[0]); // Cabibbo-Marinari subgroups in the order of C4
-        subgroup<0, 2, 1>(p, K, F, B, sc, record, early[1]);
-        subgroup<1, 2, 2>(p, K, F, B, sc, record, early[2]);
+        subgroup<0, 1, 0>(p, K, F, B, sc, record, early[0], lane_mu0, Gt); // Cabibbo-Marinari subgroups, order of C4
+        subgroup<0, 2, 1>(p, K, F, B, sc, record, early[1], lane_mu0, Gt);
+        subgroup<1, 2, 2>(p, K, F, B, sc, record, early[2], lane_mu0, Gt);
 
         if (active) {
 #pragma unroll
             for (int m = 0; m < NMU; ++m) {
                 const int mu = lane_mu0 + m;
+                if (CB && mu == 3) continue;
                 IO::store(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.st);
                 IO::store(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.st);
             }
+            if (owns_t) GIO::store(reinterpret_cast<T*>(p.G) + (size_t)p.parity * 18 * H, H, s.h, Gt, pol.st);
         }
     }
 };
 
-template <typename T, int R, int TPS, int MODE>
+template <typename T, int R, int TPS, int MODE, bool CB = false>
 __global__ void __launch_bounds__(MAX_BLOCK) gf_half_sweep_kernel(const SweepParams p)
 {
-    SweepKernel<T, R, TPS, MODE>::run(p);
+    SweepKernel<T, R, TPS, MODE, CB>::run(p);
 }
 
 } // namespace gf

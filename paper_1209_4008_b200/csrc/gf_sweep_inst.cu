@@ -1,6 +1,6 @@
 // gf_sweep_inst.cu -- one translation unit per (precision, reals-per-link): compiled four times by build.py with
 //   -DGF_INST_FP64={0,1} -DGF_INST_R={12,18}
-// so the thirty-six half-sweep kernels build in parallel.  Each unit exports one launcher and one
+// so the sixty half-sweep kernels build in parallel.  Each unit exports one launcher and one
 // attribute query, declared in gf_internal.h.
 #include "gf_internal.h"
 #include "gf_sweep.cuh"
@@ -24,9 +24,21 @@ namespace gf {
 
 typedef void (*sweep_fn)(const SweepParams);
 
-static sweep_fn pick(int tps, int mode)
+static sweep_fn pick(int tps, int mode, bool cb)
 {
     constexpr int R = GF_INST_R;
+    if (cb) { // Coulomb reading B: relaxation sweeps only
+        if (mode == MODE_OVERRELAX) {
+            if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX, true>;
+            if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX, true>;
+            if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_OVERRELAX, true>;
+        } else if (mode == MODE_VARIANT) {
+            if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_VARIANT, true>;
+            if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_VARIANT, true>;
+            if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_VARIANT, true>;
+        }
+        return nullptr;
+    }
     if (mode == MODE_OVERRELAX) {
         if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX>;
         if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX>;
@@ -45,7 +57,7 @@ static sweep_fn pick(int tps, int mode)
 
 cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParams& p, cudaStream_t stream)
 {
-    sweep_fn fn = pick(tps, mode);
+    sweep_fn fn = pick(tps, mode, p.G != nullptr);
     if (fn == nullptr || block <= 0 || block > MAX_BLOCK || (block % 32) != 0) return cudaErrorInvalidValue;
     const unsigned long long threads = (unsigned long long)p.h_count * (unsigned long long)tps;
     if (p.h_count == 0) return cudaSuccess;
@@ -71,7 +83,7 @@ cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParam
 
 cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, cudaFuncAttributes* attr)
 {
-    sweep_fn fn = pick(tps, mode);
+    sweep_fn fn = pick(tps, mode, false);
     if (fn == nullptr) return cudaErrorInvalidValue;
     return cudaFuncGetAttributes(attr, fn);
 }

@@ -242,3 +242,57 @@ def test_r12_stays_unitary_under_hot_updates(gfm, precision, tol):
     uu_off, _ = oracle.unitarity_defect(fx.download(), dims)
     assert uu_off > 1e3 * tol
     fx.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("R", [18, 12])
+@pytest.mark.parametrize("tps", [0, 1, 2, 4])
+def test_coulomb_reading_b_matches_reading_a_and_oracle(gfm, precision, R, tps):
+    """C12 reading B (temporal links transformed once per call from the accumulated g(x)) against the oracle
+    (reading A): one sweep within the per-link tolerance, several sweeps and the other update kinds within its
+    growth; spatial links bit-identical to reading A of the CUDA path (same arithmetic, they never see G)"""
+    dims = (8, 6, 4, 10)
+    U = gf_inputs.smooth_random(dims, 0.4, 57)
+    tol = TOL_LINK[precision]
+    a = gfm.GaugeFixer(dims, precision=precision, gauge="coulomb", reals_per_link=R)
+    b = gfm.GaugeFixer(dims, precision=precision, gauge="coulomb", reals_per_link=R)
+    for fx in (a, b):
+        gfm.gf_set_tuning(fx.ctx, tps, 0 if tps == 0 else 64)
+        fx.load(U)
+    gfm.gf_set_coulomb_reading(a.ctx, False)
+    gfm.gf_set_coulomb_reading(b.ctx, True)
+    ref = U.copy()
+    a.overrelax(1.7, 1); b.overrelax(1.7, 1)
+    oracle.overrelax(ref, dims, 1.7, 1, oracle.COULOMB)
+    ga, gb = a.download(), b.download()
+    # same launch shape: same arithmetic on the spatial links (automatic shape differs between the readings in fp32)
+    same_shape = tps != 0
+    assert np.array_equal(ga[:, :3], gb[:, :3]) if same_shape else np.abs(ga - gb).max() <= 2 * tol
+    assert np.abs(gb - ref).max() <= tol
+    a.overrelax(1.7, 4); b.overrelax(1.7, 4)
+    a.relax(gfm.GF_UPDATE_STOCHASTIC, 0.4, 2, seed=5); b.relax(gfm.GF_UPDATE_STOCHASTIC, 0.4, 2, seed=5)
+    a.relax(gfm.GF_UPDATE_OVERRELAX1, 1.5, 2); b.relax(gfm.GF_UPDATE_OVERRELAX1, 1.5, 2)
+    ga, gb = a.download(), b.download()
+    assert np.abs(ga - gb).max() <= 20 * tol
+    if same_shape:
+        assert np.array_equal(ga[:, :3], gb[:, :3])
+        assert b.functional() == a.functional() and b.theta() == a.theta()  # F, theta do not see the temporal links
+    assert abs(oracle.plaquette(gb, dims) - oracle.plaquette(U, dims)) < (1e-12 if precision == "fp64" else 2e-5)
+    a.close(); b.close()
+
+
+def test_coulomb_reading_b_with_fix_slices_and_errors(gfm):
+    dims = (6, 6, 6, 8)
+    U = gf_inputs.smooth_random(dims, 0.5, 45)
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge="coulomb")
+    gfm.gf_set_coulomb_reading(fx.ctx, True)
+    fx.load(U)
+    n, th, F, per = fx.fix_slices(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=5, max_sweeps=3000)
+    n_ref, th_ref, F_ref, per_ref = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 5, 3000)
+    assert per == per_ref.tolist() and F == pytest.approx(F_ref, rel=1e-10)
+    assert np.abs(fx.download() - U).max() < 1e-9
+    fx.close()
+    lx = gfm.GaugeFixer(dims, precision="fp64", gauge="landau")
+    with pytest.raises(gfm.GFError):
+        gfm.gf_set_coulomb_reading(lx.ctx, True)
+    lx.close()
