@@ -59,9 +59,13 @@ def volume(dims):
     return dims[0] * dims[1] * dims[2] * dims[3]
 
 
-def model_bytes_per_site_update(R: int, precision: str) -> int:
-    """every half-sweep reads and writes every link once (C6): 16 R s bytes per site-update"""
-    return 16 * R * (8 if precision == "fp64" else 4)
+def model_bytes_per_site_update(R: int, precision: str, gauge: str = "landau", anneal: bool = False) -> int:
+    """every half-sweep reads and writes every link once (C6): 16 R s bytes per site-update.  Coulomb relaxation
+    sweeps in fp32 run reading B (C12): 6 of the 8 links plus the 18-real g(x) field, (12 R + 36) s."""
+    s = 8 if precision == "fp64" else 4
+    if gauge == "coulomb" and precision == "fp32" and not anneal:
+        return (12 * R + 36) * s
+    return 16 * R * s
 
 
 def measured_peaks():
@@ -206,7 +210,8 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
 def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None):
     """dominant kernel = the half-sweep kernel: algorithmic bytes per launch = (V/2) * 16 R s"""
     peak, which = measured_peaks()
-    per_launch_bytes = (volume(w["dims"]) // 2) * model_bytes_per_site_update(w["R"], w["precision"])
+    per_launch_bytes = (volume(w["dims"]) // 2) * model_bytes_per_site_update(w["R"], w["precision"], w["gauge"],
+                                                                              bool(w.get("anneal")))
     nlaunch = 2 * sweeps * steps
     avg_s = in_sweeps_s / nlaunch
     achieved = per_launch_bytes / avg_s / 1e9
