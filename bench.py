@@ -61,10 +61,10 @@ def volume(dims):
 
 def model_bytes_per_site_update(R: int, precision: str, gauge: str = "landau", anneal: bool = False) -> int:
     """every half-sweep reads and writes every link once (C6): 16 R s bytes per site-update.  Coulomb relaxation
-    sweeps in fp32 run reading B (C12): 6 of the 8 links plus the 18-real g(x) field, (12 R + 36) s."""
+    and annealing sweeps in fp32 run reading B (C12): 6 of the 8 links plus the 18-real g(x) field, (12 R + 36) s."""
     s = 8 if precision == "fp64" else 4
-    if gauge == "coulomb" and precision == "fp32" and not anneal:
-        return (12 * R + 36) * s
+    if gauge == "coulomb" and precision == "fp32":
+        return (12 * R + 36) * s  # annealing sweeps run reading B too
     return 16 * R * s
 
 

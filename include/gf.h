@@ -186,7 +186,7 @@ int gf_set_prefetch(gf_ctx* ctx, int sites);
  * A when the site field cannot be allocated.  Reading B: the relaxation sweeps (gf_overrelax / gf_relax / gf_fix / gf_fix_slices)
  * leave the temporal links in memory, accumulate g(x) in a site field owned by the context (V * 18 reals) and
  * transform the temporal links once at the end of each call -- 14/16 of the bytes, same result up to rounding.
- * Annealing sweeps always use reading A.  GF_EINVAL for a Landau context. */
+ * gf_anneal / gf_anneal_micro keep one site field over the whole call.  GF_EINVAL for a Landau context. */
 int gf_set_coulomb_reading(gf_ctx* ctx, int reading_b);
 /* Slab fusion of the two half-sweeps of a sweep through L2 (0 = off, default): RED and BLACK are launched as a
  * wavefront over chunks of `chunk_slices` timeslices (BLACK on slice t after RED on t-1, t, t+1), so that BLACK

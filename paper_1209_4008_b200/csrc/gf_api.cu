@@ -205,7 +205,8 @@ extern "C" unsigned long long gf_launch_count(const gf_ctx* c) { return c ? c->l
 // threads per site the thread that drops the temporal links idles (fp64: -2 %), so automatic = fp32 only.
 static bool uses_reading_b(const gf_ctx* c, int mode)
 {
-    if (c->gauge != GF_COULOMB || mode == MODE_HEATBATH) return false;
+    (void)mode;
+    if (c->gauge != GF_COULOMB) return false;
     return c->coulomb_b < 0 ? c->precision == GF_FP32 : c->coulomb_b != 0;
 }
 
@@ -447,27 +448,45 @@ extern "C" int gf_convert(gf_ctx* src, const void* U_src, gf_ctx* dst, void* U_d
 
 // Coulomb reading B (gf_set_coulomb_reading): G = 1, the sweeps leave the temporal links alone and accumulate g(x) in
 // G, then one pass transforms the temporal links.  Reading A otherwise.
-static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
-                      cudaStream_t st, const char* who, const unsigned char* active = nullptr)
+// reading_b_begin: *gfield = the context's g(x) field set to 1, or NULL when this call runs reading A
+static int reading_b_begin(gf_ctx* c, int mode, cudaStream_t st, void** gfield, const char* who)
 {
-    if (!uses_reading_b(c, mode) || nsweeps == 0)
-        return run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, nullptr);
+    *gfield = nullptr;
+    if (!uses_reading_b(c, mode)) return GF_OK;
     cudaError_t e;
     if (c->d_gfield == nullptr && (e = cudaMalloc(&c->d_gfield, (size_t)c->L.H * 2 * 18 * real_size(c))) != cudaSuccess) {
         c->d_gfield = nullptr;
         (void)cudaGetLastError();
         if (c->coulomb_b < 0) { // automatic choice and no room for the g(x) field: reading A needs none
             c->coulomb_b = 0;
-            return run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, nullptr);
+            return GF_OK;
         }
         return cuda_fail(c, e, "Coulomb reading B: allocation of the g(x) field");
     }
     if ((e = launch_coulomb_init(c->precision, c->L, c->d_gfield, st)) != cudaSuccess) return cuda_fail(c, e, who);
-    int rc = run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, c->d_gfield);
-    if (rc != GF_OK) return rc;
-    if ((e = launch_coulomb_finish(c->precision, c->R, c->L, U, c->d_gfield, st)) != cudaSuccess) return cuda_fail(c, e, who);
-    c->launches += 2;
+    c->launches += 1;
+    *gfield = c->d_gfield;
     return GF_OK;
+}
+
+static int reading_b_end(gf_ctx* c, void* U, void* gfield, cudaStream_t st, const char* who)
+{
+    if (gfield == nullptr) return GF_OK;
+    cudaError_t e = launch_coulomb_finish(c->precision, c->R, c->L, U, gfield, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, who);
+    c->launches += 1;
+    return GF_OK;
+}
+
+static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
+                      cudaStream_t st, const char* who, const unsigned char* active = nullptr)
+{
+    if (nsweeps == 0) return GF_OK;
+    void* gfield;
+    int rc = reading_b_begin(c, mode, st, &gfield, who);
+    if (rc == GF_OK) rc = run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, gfield);
+    if (rc == GF_OK) rc = reading_b_end(c, U, gfield, st, who);
+    return rc;
 }
 
 extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void* stream)
@@ -512,6 +531,11 @@ extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end,
     SweepParams p = base_params(c, U);
     p.key0 = (uint32_t)seed;
     p.key1 = (uint32_t)(seed >> 32);
+    if (nsteps == 0) return GF_OK;
+    void* gfield; // Coulomb reading B: one g(x) field over the whole call, heatbath and microcanonical sweeps alike
+    int rc0 = reading_b_begin(c, MODE_HEATBATH, st, &gfield, "gf_anneal");
+    if (rc0 != GF_OK) return rc0;
+    p.G = gfield;
     for (int step = 0; step < nsteps; ++step) {
         // T_i = T_start + (T_end - T_start) i / (nsteps - 1)   (C13)
         p.T = nsteps > 1 ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
@@ -530,11 +554,12 @@ extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end,
         c->sweeps_done += 1;
         // microcanonical sweeps g -> g^2 (C19): stochastic relaxation with p = 2 > u, i.e. always
         if (n_micro > 0) {
-            int rc = run_sweeps(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, seed, st, "gf_anneal_micro: kernel launch");
+            int rc = run_sweeps_core(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, seed, st,
+                                     "gf_anneal_micro: kernel launch", nullptr, gfield);
             if (rc != GF_OK) return rc;
         }
     }
-    return GF_OK;
+    return reading_b_end(c, U, gfield, st, "gf_anneal");
 }
 
 extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, unsigned long long seed, void* stream)

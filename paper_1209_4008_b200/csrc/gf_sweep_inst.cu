@@ -1,6 +1,6 @@
 // gf_sweep_inst.cu -- one translation unit per (precision, reals-per-link): compiled four times by build.py with
 //   -DGF_INST_FP64={0,1} -DGF_INST_R={12,18}
-// so the sixty half-sweep kernels build in parallel.  Each unit exports one launcher and one
+// so the seventy-two half-sweep kernels build in parallel.  Each unit exports one launcher and one
 // attribute query, declared in gf_internal.h.
 #include "gf_internal.h"
 #include "gf_sweep.cuh"
@@ -27,8 +27,12 @@ typedef void (*sweep_fn)(const SweepParams);
 static sweep_fn pick(int tps, int mode, bool cb)
 {
     constexpr int R = GF_INST_R;
-    if (cb) { // Coulomb reading B: relaxation sweeps only
-        if (mode == MODE_OVERRELAX) {
+    if (cb) { // Coulomb reading B
+        if (mode == MODE_HEATBATH) {
+            if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_HEATBATH, true>;
+            if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_HEATBATH, true>;
+            if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_HEATBATH, true>;
+        } else if (mode == MODE_OVERRELAX) {
             if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX, true>;
             if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX, true>;
             if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_OVERRELAX, true>;

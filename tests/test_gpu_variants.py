@@ -296,3 +296,25 @@ def test_coulomb_reading_b_with_fix_slices_and_errors(gfm):
     with pytest.raises(gfm.GFError):
         gfm.gf_set_coulomb_reading(lx.ctx, True)
     lx.close()
+
+
+@pytest.mark.parametrize("R,tps", [(18, 0), (18, 1), (12, 2), (18, 4)])
+def test_coulomb_reading_b_annealing_decisions_fp64(gfm, R, tps):
+    """annealing (heatbath + microcanonical sweeps) under reading B: the draw never sees the temporal links, so the
+    accept decisions are those of the oracle (reading A) and the links agree to rounding"""
+    import torch
+
+    dims = (6, 4, 4, 8)
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.5, 58)
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge="coulomb", reals_per_link=R)
+    gfm.gf_set_tuning(fx.ctx, tps, 0 if tps == 0 else 64)
+    gfm.gf_set_coulomb_reading(fx.ctx, True)
+    trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
+    gfm.gf_set_trial_buffer(fx.ctx, trials)
+    fx.load(U)
+    fx.anneal(1.2, 0.3, 3, 7, n_micro=1)
+    ref_trials = oracle.anneal_micro(U, dims, 1.2, 0.3, 3, 1, 7, oracle.COULOMB, trials=True)
+    assert np.array_equal(trials.cpu().numpy().reshape(V, 3), ref_trials)
+    assert np.abs(fx.download() - U).max() <= 1e-10
+    fx.close()
