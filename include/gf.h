@@ -183,8 +183,8 @@ int gf_set_pdl(gf_ctx* ctx, int on);
 int gf_set_prefetch(gf_ctx* ctx, int sites);
 /* Coulomb gauge, treatment of the temporal links (C12): 0 = reading A: every half-sweep moves and multiplies all 8
  * links of a site; 1 = reading B; -1 = automatic (default): B in fp32 (+14 % at one thread per site), A in fp64, and
- * A when the site field cannot be allocated.  Reading B: the relaxation sweeps (gf_overrelax / gf_relax / gf_fix / gf_fix_slices)
- * leave the temporal links in memory, accumulate g(x) in a site field owned by the context (V * 18 reals) and
+ * A when the site field cannot be allocated.  Reading B: the sweeps (relaxation and annealing alike) leave the
+ * temporal links in memory, accumulate g(x) in a site field owned by the context (V * 18 reals) and
  * transform the temporal links once at the end of each call -- 14/16 of the bytes, same result up to rounding.
  * gf_anneal / gf_anneal_micro keep one site field over the whole call.  GF_EINVAL for a Landau context. */
 int gf_set_coulomb_reading(gf_ctx* ctx, int reading_b);
