@@ -226,7 +226,7 @@ def max_over_ranks(seconds: float, device) -> float:
     import torch
     import torch.distributed as dist
 
-    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+    if not (dist.is_available() and dist.is_initialized()):
         return seconds
     tt = torch.tensor([seconds], dtype=torch.float64, device=device)
     dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -350,9 +350,11 @@ def main():
     gfm.load_library()
     torch.cuda.set_device(local_rank)
     barrier = None
-    if world > 1:
+    under_torchrun = "RANK" in os.environ and "MASTER_ADDR" in os.environ
+    if world > 1 or under_torchrun:  # one rank per GPU over NCCL; a 1-rank torchrun launch takes the same path
         import torch.distributed as dist
 
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")  # NCCL logs to stdout by default: keep it to the JSON line
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         barrier = dist.barrier
     stream = torch.cuda.Stream()
@@ -390,7 +392,7 @@ def main():
     V = volume(w["dims"])
     value = whole_job_value(world, V, sweeps, steps, total)
 
-    if world > 1:
+    if world > 1 or under_torchrun:
         dist.barrier()
         dist.destroy_process_group()
     if rank != 0:
