@@ -310,10 +310,33 @@ def main_reference(args, w, rank):
         "e2e": {"value": value, "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
-    print(json.dumps(line), flush=True)
+    _print_json(line)
+
+
+_JSON_FD = None
+
+
+def _reserve_stdout():
+    """Libraries (NCCL prints its version banner) write to stdout: keep fd 1 for the ONE JSON line by pointing it at
+    stderr for the rest of the run and writing the line to the saved descriptor."""
+    global _JSON_FD
+    if _JSON_FD is None:
+        sys.stdout.flush()
+        _JSON_FD = os.dup(1)
+        os.dup2(2, 1)
+
+
+def _print_json(line: dict) -> None:
+    data = (json.dumps(line) + "\n").encode()
+    if _JSON_FD is None:
+        sys.stdout.write(data.decode())
+        sys.stdout.flush()
+    else:
+        os.write(_JSON_FD, data)
 
 
 def main():
+    _reserve_stdout()
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
@@ -469,7 +492,7 @@ def main():
         "roofline": m["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
         "clocks": m["clocks"], "also": also,
     }
-    print(json.dumps(line), flush=True)
+    _print_json(line)
 
 
 if __name__ == "__main__":
