@@ -201,7 +201,7 @@ int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);
 /* Number of kernels this ctx has launched so far. */
 unsigned long long gf_launch_count(const gf_ctx* ctx);
 /* Registers per thread and local-memory (spill) bytes per thread of the sweep kernel that the current
- * (precision, storage, tuning) selects; mode 0 = overrelaxation, 1 = heatbath. */
+ * (precision, storage, gauge reading, tuning) selects; mode 0 = overrelaxation, 1 = heatbath, 2 = gf_relax variants. */
 int gf_kernel_info(gf_ctx* ctx, int mode, int* regs_per_thread, int* local_bytes_per_thread);
 
 #ifdef __cplusplus

@@ -241,12 +241,13 @@ static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p_in, cu
 extern "C" int gf_kernel_info(gf_ctx* c, int mode, int* regs, int* local_bytes)
 {
     if (c == nullptr) return GF_EINVAL;
-    if (mode != 0 && mode != 1) return fail(c, GF_EINVAL, "gf_kernel_info: mode must be 0 or 1");
+    if (mode < 0 || mode > 2) return fail(c, GF_EINVAL, "gf_kernel_info: mode must be 0 (overrelaxation), 1 (heatbath) or 2 (variants)");
     cudaFuncAttributes a;
     cudaError_t e;
     const int tps = auto_tps(c, mode);
-    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(tps, mode, &a) : sweep_attributes_f32_r12(tps, mode, &a);
-    else e = c->R == 18 ? sweep_attributes_f64_r18(tps, mode, &a) : sweep_attributes_f64_r12(tps, mode, &a);
+    const bool rb = uses_reading_b(c, mode);
+    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(tps, mode, rb, &a) : sweep_attributes_f32_r12(tps, mode, rb, &a);
+    else e = c->R == 18 ? sweep_attributes_f64_r18(tps, mode, rb, &a) : sweep_attributes_f64_r12(tps, mode, rb, &a);
     if (e != cudaSuccess) return cuda_fail(c, e, "gf_kernel_info");
     if (regs) *regs = a.numRegs;
     if (local_bytes) *local_bytes = (int)a.localSizeBytes;

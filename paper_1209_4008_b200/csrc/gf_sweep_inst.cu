@@ -85,9 +85,9 @@ cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParam
     return cudaLaunchKernelEx(&cfg, fn, p);
 }
 
-cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, cudaFuncAttributes* attr)
+cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, bool reading_b, cudaFuncAttributes* attr)
 {
-    sweep_fn fn = pick(tps, mode, false);
+    sweep_fn fn = pick(tps, mode, reading_b);
     if (fn == nullptr) return cudaErrorInvalidValue;
     return cudaFuncGetAttributes(attr, fn);
 }
