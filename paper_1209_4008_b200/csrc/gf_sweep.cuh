@@ -49,8 +49,8 @@ struct SweepParams {
 // Guards (C9) on the squared norms: |k|^2 below TinySq<T> takes G = 1 (the CPU oracle tests |k| < 1e-300; the
 // two differ only for |k| in [1e-300, 1e-150), fp32 [.., 1e-18) -- DESIGN.md "Differences").
 template <typename T> struct Tiny;
-template <> struct Tiny<float> { static constexpr float n = 1e-30f; static constexpr float sq = 1e-36f; };
-template <> struct Tiny<double> { static constexpr double n = 1e-300; static constexpr double sq = 1e-300; };
+template <> struct Tiny<float> { static constexpr float sq = 1e-36f; };
+template <> struct Tiny<double> { static constexpr double sq = 1e-300; };
 
 template <typename T>
 __device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[4])
