@@ -318,3 +318,52 @@ def test_coulomb_reading_b_annealing_decisions_fp64(gfm, R, tps):
     assert np.array_equal(trials.cpu().numpy().reshape(V, 3), ref_trials)
     assert np.abs(fx.download() - U).max() <= 1e-10
     fx.close()
+
+
+def _degenerate_field(dims):
+    """U_mu(y) = 1 on even sites, diag(-1,-1,1) on odd sites: K(x) = 4 (1 + D) = diag(0,0,8) at every site, so the
+    (0,1) block of K vanishes identically (the |k| = 0 guard of C9) while (0,2) and (1,2) give g = 1"""
+    V = int(np.prod(dims))
+    s = np.arange(V)
+    x = s % dims[0] + (s // dims[0]) % dims[1] + (s // (dims[0] * dims[1])) % dims[2] + s // (dims[0] * dims[1] * dims[2])
+    U = np.zeros((V, 4, 3, 3), dtype=np.complex128)
+    U[:, :, 0, 0] = U[:, :, 1, 1] = np.where(x % 2 == 0, 1.0, -1.0)[:, None]
+    U[:, :, 2, 2] = 1.0
+    return U
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_degenerate_block_and_empty_calls(gfm, precision):
+    import torch
+
+    dims = (4, 4, 2, 6)
+    V = int(np.prod(dims))
+    U = _degenerate_field(dims)
+    ref = U.copy()
+    oracle.overrelax(ref, dims, 1.7, 2)
+    assert np.array_equal(ref, U)  # the oracle takes G = 1 in the vanishing block and g = 1 in the others
+    fx = gfm.GaugeFixer(dims, precision=precision)
+    gfm.gf_set_reunit(fx.ctx, 0)
+    fx.load(U)
+    fx.overrelax(1.7, 2)
+    fx.relax(gfm.GF_UPDATE_OVERRELAX1, 1.5, 1)
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 0.5, 1, seed=3)
+    assert np.array_equal(fx.download(), U)
+    assert fx.theta() == 0.0 and fx.functional() == pytest.approx(1.0 / 3.0, abs=1e-15)
+    # heatbath: the vanishing block takes no trial (count 0) on both sides
+    trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
+    gfm.gf_set_trial_buffer(fx.ctx, trials)
+    fx.anneal(0.7, 0.7, 1, 7)
+    got = trials.cpu().numpy().reshape(V, 3)
+    work = U.copy()
+    ref_tr = oracle.anneal(work, dims, 0.7, 0.7, 1, 7, trials=True)
+    red = np.array([(s % 4 + (s // 4) % 4 + (s // 16) % 2 + s // 32) % 2 == 0 for s in range(V)])
+    assert (got[red, 0] == 0).all() and (ref_tr[red, 0] == 0).all()  # RED sites see the untouched degenerate K
+    # empty calls leave every bit alone
+    fx.load(U)
+    fx.overrelax(1.7, 0)
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 0.5, 0)
+    fx.anneal(1.0, 0.5, 0, 1)
+    assert fx.fix(1e-30, max_sweeps=0)[0] == 0
+    assert np.array_equal(fx.download(), U)
+    fx.close()
