@@ -367,3 +367,49 @@ def test_degenerate_block_and_empty_calls(gfm, precision):
     assert fx.fix(1e-30, max_sweeps=0)[0] == 0
     assert np.array_equal(fx.download(), U)
     fx.close()
+
+
+@pytest.mark.parametrize("precision,R,gauge", [("fp32", 18, "landau"), ("fp32", 12, "coulomb"), ("fp64", 18, "coulomb"),
+                                               ("fp64", 12, "landau")])
+def test_no_write_outside_the_field(gfm, precision, R, gauge):
+    """compute-sanitizer is closed on this pool: guard bands of a sentinel pattern before and after the native field
+    (and around the canonical buffer) must survive every kernel -- pack, all sweep kinds with every launch shape on a
+    lattice with a ragged last warp, reductions, convert, unpack"""
+    import torch
+
+    dims = (6, 2, 6, 10)  # V/2 = 360: ragged for 32-thread blocks at 1, 2 and 4 threads per site
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.4, 59)
+    prec = gfm.GF_FP64 if precision == "fp64" else gfm.GF_FP32
+    ctx = gfm.gf_create(*dims, prec, gfm.GF_COULOMB if gauge == "coulomb" else gfm.GF_LANDAU)
+    gfm.gf_set_storage(ctx, R)
+    nbytes = gfm.gf_field_bytes(ctx)
+    band = 1 << 16
+    buf = torch.full((nbytes + 2 * band,), 0xA5, dtype=torch.uint8, device="cuda")
+    field = buf[band:band + nbytes]
+    assert field.data_ptr() % 256 == 0
+    cbuf = torch.full((V * 72 + 2 * 8192,), float("nan"), dtype=torch.float64, device="cuda")
+    canon = cbuf[8192:8192 + V * 72]
+    canon.copy_(torch.from_numpy(U.view("float64").reshape(-1)))
+    gfm.gf_pack(ctx, canon, field)
+    for tps in (0, 1, 2, 4):
+        for block in ((0,) if tps == 0 else (32, 96)):
+            gfm.gf_set_tuning(ctx, tps, block)
+            gfm.gf_set_prefetch(ctx, 100)
+            gfm.gf_overrelax(ctx, field, 1.7, 2)
+            gfm.gf_relax(ctx, field, gfm.GF_UPDATE_STOCHASTIC, 0.5, 1, 3)
+            gfm.gf_relax(ctx, field, gfm.GF_UPDATE_OVERRELAX1, 1.4, 1, 0)
+            gfm.gf_anneal_micro(ctx, field, 1.0, 0.5, 2, 1, 7)
+            gfm.gf_set_fusion(ctx, 2)
+            gfm.gf_overrelax(ctx, field, 1.7, 1)
+            gfm.gf_set_fusion(ctx, 0)
+    gfm.gf_functional(ctx, field)
+    gfm.gf_theta(ctx, field)
+    if gauge == "coulomb":
+        gfm.gf_fix_slices(ctx, field, dims[3], gfm.GF_UPDATE_OVERRELAX2, 1.5, 1e-3, 2, 6)
+    gfm.gf_unpack(ctx, field, canon)
+    torch.cuda.synchronize()
+    assert bool((buf[:band] == 0xA5).all()) and bool((buf[band + nbytes:] == 0xA5).all())
+    assert bool(torch.isnan(cbuf[:8192]).all()) and bool(torch.isnan(cbuf[8192 + V * 72:]).all())
+    assert not bool(torch.isnan(canon).any())
+    gfm.gf_destroy(ctx)
