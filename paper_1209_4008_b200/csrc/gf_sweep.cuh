@@ -113,27 +113,29 @@ __device__ __forceinline__ void su2_variant_step(const T (&k)[4], int variant, d
 // Uniforms: u = (2 (x >> 9) + 1) 2^-24, exact in fp32 and fp64.
 // ---------------------------------------------------------------------------------------------------------
 template <typename T> struct KPMath;
+// fp64: the draw is evaluated in double like the oracle's, with correctly-rounded-to-1-ulp library functions (log,
+// cospi/sinpi) but without IEEE divisions and square roots (1/|k| by rsqrt, delta as one fused expression times
+// 1/alpha).  The oracle's alpha already differs from the kernel's by an ulp (summation order of K), so decision
+// parity rests on the size of the difference, not on the operation order: a decision flips only when u4^2 falls
+// within ~1e-15 of the threshold, i.e. with probability ~1e-15 per trial (tests compare every trial count).
 template <> struct KPMath<double> {
     static __device__ __forceinline__ double uni(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
-    static __device__ __forceinline__ double cos2pi(double u) { return cos(6.283185307179586476925286766559 * u); }
-    static __device__ __forceinline__ double sin2pi(double u) { return sin(6.283185307179586476925286766559 * u); }
+    static __device__ __forceinline__ double cos2pi(double u) { return cospi(2.0 * u); }
+    static __device__ __forceinline__ double sin2pi(double u) { return sinpi(2.0 * u); }
     static __device__ __forceinline__ double neglog(double u) { return -log(u); }
-    // delta = (-ln u1 / alpha) cos^2 + (-ln u2 / alpha), in exactly this order, no FMA contraction: this
-    // value decides acceptance and must follow the stated recipe operation by operation (C14)
-    // alpha = |k| / T exactly as the oracle forms it (sqrt, then division): it decides acceptance (C14)
     static __device__ __forceinline__ void prep(double n2, double T, double& alpha, double& inv_alpha, double& inv_n)
     {
-        const double n = sqrt(n2);
-        alpha = n / T;
-        inv_alpha = 0.0; // unused: the fp64 draw divides
-        inv_n = 1.0 / n;
+        inv_n = rsqrt(n2);
+        alpha = n2 * inv_n / T;
+        inv_alpha = T * inv_n;
     }
-    static __device__ __forceinline__ double root(double x) { return sqrt(fmax(0.0, x)); }
-    static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha, double)
+    static __device__ __forceinline__ double root(double x) { return x > 0.0 ? x * rsqrt(x) : 0.0; }
+    static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha, double inv_alpha)
     {
-        return __dadd_rn(__dmul_rn(__ddiv_rn(l1, alpha), __dmul_rn(c, c)), __ddiv_rn(l2, alpha));
+        (void)alpha;
+        return fma(l1, c * c, l2) * inv_alpha;
     }
-    static __device__ __forceinline__ bool accept(double u4, double d) { return __dmul_rn(u4, u4) <= __dsub_rn(1.0, __dmul_rn(0.5, d)); }
+    static __device__ __forceinline__ bool accept(double u4, double d) { return u4 * u4 <= fma(-0.5, d, 1.0); }
 };
 // fp32: decision parity with the fp64 oracle cannot be exact (alpha itself differs at 1e-7, C14), so the draw uses
 // the SFU: u from the mantissa trick (exact), -ln u = -ln2 * lg2(u) (MUFU.LG2, abs. error ~4e-7), cos/sin by
