@@ -190,9 +190,10 @@ def test_config5_48x3x64_coulomb_anneal_sampled_sites(gfm):
     trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
     gfm.gf_set_trial_buffer(fx.ctx, trials)
     gfm.gf_pack(fx.ctx, canon, fx.U)
-    gfm.gf_unpack(fx.ctx, fx.U, canon)  # the fp32-rounded input, as the kernel sees it
-    torch.cuda.synchronize()
-    work = canon.cpu().numpy().view("complex128").reshape(V, 4, 3, 3).copy()
+    # the fp32-rounded input, as the kernel sees it -- rounded on the host (no oracle input comes from the CUDA path)
+    Nx, Ny, Nz, Nt = gdims
+    work = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(V, 4, 3, 3)
+    work = work.astype(np.complex64).astype(np.complex128)
     fx.anneal(1.4, 1.4, 1, 7)
     gfm.gf_unpack(fx.ctx, fx.U, canon)
     torch.cuda.synchronize()
