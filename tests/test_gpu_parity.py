@@ -75,12 +75,17 @@ def test_functional_and_theta(gfm, precision, R, gauge, dims):
     oracle.overrelax(U, dims, 1.7, 3, _orc_gauge(gauge))  # partly fixed: theta no longer O(1)
     fx = _fixer(gfm, dims, precision, gauge, R)
     fx.load(U)
-    # the reductions run in fp64 on the STORED links: compare with the oracle on exactly those
-    stored = fx.download()
+    # the reductions run in fp64 on the STORED links: compare with the oracle on exactly those, formed on the host
+    # (rounded to fp32 where the storage is; R = 12: row 2 = conj(row0 x row1) of the stored rows)
+    stored = U.astype(np.complex64).astype(np.complex128) if precision == "fp32" else U.copy()
+    if R == 12:
+        r0, r1 = stored[:, :, 0, :], stored[:, :, 1, :]
+        stored[:, :, 2, :] = np.conj(np.cross(r0, r1))
     og = _orc_gauge(gauge)
-    assert fx.functional() == pytest.approx(oracle.functional(stored, dims, og), rel=1e-12)
-    assert fx.theta() == pytest.approx(oracle.theta(stored, dims, og), rel=1e-10)
-    np.testing.assert_allclose(fx.theta_slices(), oracle.theta_slices(stored, dims, og), rtol=1e-10)
+    tight = 1e-12 if not (precision == "fp32" and R == 12) else 1e-6  # fp32 R12 rebuilds row 2 in fp32
+    assert fx.functional() == pytest.approx(oracle.functional(stored, dims, og), rel=tight)
+    assert fx.theta() == pytest.approx(oracle.theta(stored, dims, og), rel=max(100 * tight, 1e-10))
+    np.testing.assert_allclose(fx.theta_slices(), oracle.theta_slices(stored, dims, og), rtol=max(100 * tight, 1e-10))
     # and with the oracle on the original fp64 field, within the storage rounding
     rel = 1e-12 if precision == "fp64" else 2e-6
     assert fx.functional() == pytest.approx(oracle.functional(U, dims, og), rel=rel)
