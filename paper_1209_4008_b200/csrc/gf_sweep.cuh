@@ -281,6 +281,29 @@ struct SweepKernel {
         su2_left<I, J>(a, b, K);                        // K <- G K  (C8)
     }
 
+    // L2 prefetch for the block that runs `prefetch` sites further along the traversal: the few fat warps of
+    // an SM cannot keep enough bytes in flight while they compute, prefetches hold no register and no
+    // scoreboard entry, and the 126 MB L2 is the staging buffer.  Addresses are those of this thread shifted
+    // by the distance (exact for forward links, exact up to the periodic wrap for backward links: a hint).
+    static __device__ __forceinline__ void issue_prefetch(const SweepParams& p, const Site& s, const unsigned (&hb)[NMU],
+                                                          int lane_mu0, T* base, size_t H)
+    {
+        if (p.prefetch) {
+            const long long d = p.reverse ? -(long long)p.prefetch : (long long)p.prefetch;
+            const long long hf = (long long)s.h + d;
+            if (hf >= 0 && hf < (long long)H) {
+#pragma unroll
+                for (int m = 0; m < NMU; ++m) {
+                    const int mu = lane_mu0 + m;
+                    const long long hbd = (long long)hb[m] + d;
+                    if (CB && mu == 3) continue;
+                    IO::prefetch(base + (size_t)(p.parity * 4 + mu) * R * H, H, (size_t)hf);
+                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, (size_t)hbd);
+                }
+            }
+        }
+    }
+
     static __device__ __forceinline__ void run(const SweepParams& p)
     {
         const unsigned blk = p.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
@@ -304,24 +327,9 @@ struct SweepKernel {
             cudaTriggerProgrammaticLaunchCompletion();
             cudaGridDependencySynchronize();
         }
-        // L2 prefetch for the block that runs `prefetch` sites further along the traversal: the few fat warps of
-        // an SM cannot keep enough bytes in flight while they compute, prefetches hold no register and no
-        // scoreboard entry, and the 126 MB L2 is the staging buffer.  Addresses are those of this thread shifted
-        // by the distance (exact for forward links, exact up to the periodic wrap for backward links: a hint).
-        if (p.prefetch) {
-            const long long d = p.reverse ? -(long long)p.prefetch : (long long)p.prefetch;
-            const long long hf = (long long)s.h + d;
-            if (hf >= 0 && hf < (long long)H) {
-#pragma unroll
-                for (int m = 0; m < NMU; ++m) {
-                    const int mu = lane_mu0 + m;
-                    const long long hbd = (long long)hb[m] + d;
-                    if (CB && mu == 3) continue;
-                    IO::prefetch(base + (size_t)(p.parity * 4 + mu) * R * H, H, (size_t)hf);
-                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, (size_t)hbd);
-                }
-            }
-        }
+        // the relaxation kernels prefetch before their loads (placed after them the fp64 kernel spills twice as
+        // much); the heatbath kernel issues its loads first and hides the prefetch and the generator behind them
+        if (MODE != MODE_HEATBATH) issue_prefetch(p, s, hb, lane_mu0, base, H);
         // issue every load before the first use
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
@@ -333,6 +341,7 @@ struct SweepKernel {
         cx<T> Gt[9];
         const bool owns_t = CB && (lane_mu0 + NMU - 1 == 3); // the thread that would hold the temporal links
         if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)p.parity * 18 * H, H, s.h, Gt, pol.ld);
+        if (MODE == MODE_HEATBATH) issue_prefetch(p, s, hb, lane_mu0, base, H);
         // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
         const uint32_t sc = canonical_index(s);
         EarlyRandom early[3];
