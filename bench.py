@@ -207,7 +207,7 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
     return total, in_sweeps, gfm.gf_launch_count(fx.ctx) - launches0, F, th, clocks
 
 
-def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None):
+def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None, total_s=None):
     """dominant kernel = the half-sweep kernel: algorithmic bytes per launch = (V/2) * 16 R s"""
     peak, which = measured_peaks()
     per_launch_bytes = (volume(w["dims"]) // 2) * model_bytes_per_site_update(w["R"], w["precision"], w["gauge"],
@@ -218,7 +218,8 @@ def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None):
     return {"bound": "hbm", "kernel": "gf_half_sweep_kernel", "achieved": round(achieved, 1), "peak": peak,
             "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": traffic,
             "bytes_per_launch": per_launch_bytes, "avg_launch_us": round(avg_s * 1e6, 3), "peak_source": which,
-            "frac_of_nominal_8TBs": round(achieved / 8000.0, 4)}
+            "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
+            "share_of_step": round(in_sweeps_s / total_s, 4) if total_s else None}
 
 
 def max_over_ranks(seconds: float, device) -> float:
@@ -407,7 +408,7 @@ def main():
         torch.cuda.empty_cache()
         return dict(U=U if not tiled else None, total=total, in_sweeps=in_sw, launches=launches, F=F, theta=th,
                     clocks=clocks, regs=regs, spill=spill, tiled=tiled, gdims=gdims,
-                    roofline=roofline_entry(wl, sweeps, steps, in_sw, traffic.get(name)))
+                    roofline=roofline_entry(wl, sweeps, steps, in_sw, traffic.get(name), total))
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
     m = measure(args.workload, w, sampler, barrier)
