@@ -52,7 +52,7 @@ WORKLOADS = {
 }
 # further workloads timed after the main one in the default run (lattices above 32^4: at most 3 steps each)
 ALSO_DEFAULT = ["32^4-f32-r12", "32^4-f64-r18", "32^4-f64-r12", "64^4-f32-r18", "64^4-f64-r18",
-                "48^3x64-f32-r18-coulomb", "48^3x64-f32-r18-coulomb-anneal"]
+                "48^3x64-f32-r18-coulomb", "48^3x64-f32-r18-coulomb-anneal", "16^3x32-f32-r18", "16^3x32-f64-r18"]
 
 
 def volume(dims):
@@ -453,7 +453,8 @@ def main():
         a = measure(name, wl, steps=a_steps)
         va = Va * sweeps * a_steps / a["total"]
         also.append({"workload": name, "value": va, "unit": "site-updates/s", "gflops_paper_model": va * FLOP_PER_SITE / 1e9,
-                     "steps": a_steps, "ms_per_step": a["total"] / a_steps * 1e3, "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
+                     "steps": a_steps, "ms_per_step": a["total"] / a_steps * 1e3,
+                     "fits_l2": 4 * Va * wl["R"] * (8 if wl["precision"] == "fp64" else 4) <= L2_BYTES, "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
                      "regs_per_thread": a["regs"], "spill_bytes": a["spill"]})
 
     cpu = None
