@@ -98,7 +98,8 @@ int gf_anneal(gf_ctx* ctx, void* U_native_dev, double T_start, double T_end, int
  *   GF_UPDATE_OVERRELAX1: g^omega "to first order" (C17): h = (1 + omega (g0 - 1), omega gvec) / |.|;
  *   GF_UPDATE_STOCHASTIC: stochastic relaxation (PAPER.md:33 ref. [5]; C18): g -> g^2 with probability param = p in
  *     [0,1], else g; decision u < p from Philox4x32-10 keyed by (seed; site, sweep, parity, subgroup), the sweep
- *     counter restarting at 0 with every call.  p = 0 is plain relaxation [3], p = 1 a microcanonical sweep.
+ *     counter restarting at 0 with every gf_relax call (inside gf_fix / gf_fix_slices it runs on through the chunks,
+ *     so the decisions of a fixing run do not repeat).  p = 0 is plain relaxation [3], p = 1 a microcanonical sweep.
  * GF_EINVAL: unknown update, omega outside [1,2), p outside [0,1], nsweeps < 0, NULL U. */
 enum { GF_UPDATE_OVERRELAX2 = 0, GF_UPDATE_OVERRELAX1 = 1, GF_UPDATE_STOCHASTIC = 2 };
 int gf_relax(gf_ctx* ctx, void* U_native_dev, int update, double param, int nsweeps, unsigned long long seed,
@@ -165,7 +166,9 @@ int gf_set_tuning(gf_ctx* ctx, int threads_per_site, int block);
  * (and rebuilds row 2).  0 = never, -1 = automatic (default): 18-real storage fp32 every 16th sweep, fp64 never;
  * 12-real storage (both precisions) every 16th overrelaxation sweep and every 4th heatbath / stochastic /
  * microcanonical sweep -- with 12 reals the rebuilt row feeds norm errors back and they grow exponentially under
- * large rotations. */
+ * large rotations (C15).  The cadence counts the sweeps since the start of the current API call
+ * (gf_overrelax, gf_relax, gf_anneal, gf_fix, ...: sweeps 16, 32, ... of each call), so a call's result depends on
+ * its arguments and the field only, not on what the context did before. */
 int gf_set_reunit(gf_ctx* ctx, int every);
 /* Alternate the block traversal direction between consecutive half-sweeps so that the tail of one
  * half-sweep, still in L2, is what the next one reads first (1 = on, default; 0 = off). */
@@ -188,13 +191,30 @@ int gf_set_prefetch(gf_ctx* ctx, int sites);
  * transform the temporal links once at the end of each call -- 14/16 of the bytes, same result up to rounding.
  * gf_anneal / gf_anneal_micro keep one site field over the whole call.  GF_EINVAL for a Landau context. */
 int gf_set_coulomb_reading(gf_ctx* ctx, int reading_b);
-/* Slab fusion of the two half-sweeps of a sweep through L2 (0 = off, default): RED and BLACK are launched as a
- * wavefront over chunks of `chunk_slices` timeslices (BLACK on slice t after RED on t-1, t, t+1), so that BLACK
- * finds the links RED has just written in L2.  Same updates, bit-identical results.  Used by gf_overrelax / gf_relax
- * when Nt >= 4.  gf_fusion_schedule writes the launch order of one sweep as (parity, t_begin, t_end) triples
- * (`backward`: walking t downwards) and returns their number (also when capacity is too small). */
-int gf_set_fusion(gf_ctx* ctx, int chunk_slices);
-int gf_fusion_schedule(int Nt, int chunk_slices, int backward, int* triples, int capacity);
+/* fp32 contexts, precision of the site chain.  The links are fp32 in memory and in the link
+ * products; the site chain -- K(x), the three SU(2) steps, K <- G K -- is ill-conditioned where the projected block k
+ * of K or the expanded g^omega is small, and a BLACK half-sweep inherits the rounding of the RED one through its K.
+ * Relaxation sweeps (gf_overrelax, gf_relax, gf_fix*):
+ *   chain = 2 (default, hybrid): a half-sweep runs the chain in double (K accumulated exactly from the fp32 links, G
+ *     rounded to fp32 once) while the field is rough -- iff one of the two half-sweeps before it had a step with
+ *     conditioning number |k| |h| below watch_threshold (default 1.0; |k|: norm of the projected block, |h|: norm of the
+ *     expanded g^omega before its reprojection, 1 for the gf_relax variants), and during the first sweep of every call
+ *     -- and in fp32 once it is smooth.  Every link then meets the fp32 tolerance of 5e-5 after one sweep against an
+ *     fp64 evaluation; on a nearly fixed field only the first sweep of a call takes the double chain.
+ *   chain = 1: always double (about -7 % at 18 reals, -30 % at 12 reals).  chain = 0: always fp32 (a few 1e-5 of the
+ *     sites of a random-gauge start miss 5e-5).
+ * Annealing sweeps (gf_anneal*): chain = 2 (default): fp32 chain; a site whose projected block has |k| below
+ *   fix_threshold (default 0.15) in one of its three steps is redone in double from the stored fp32 links inside the
+ *   same kernel (accept decisions: 1e-7 of the draws differ from an fp64 evaluation; links: all within 5e-5 below
+ *   T ~ 0.5, about 1e-6 of the sites of a 7 M-site lattice miss it at T = 1.4, where alpha = |k|/T inherits the fp32
+ *   rounding of K).  chain = 1: the double chain at every site (every link within 5e-5; about -17 %).  chain = 0: plain
+ *   fp32.
+ * A threshold of 0 keeps the current value.  Ignored by fp64 contexts.  GF_EINVAL: chain outside 0..2, a threshold < 0
+ * or > 1e3.
+ * gf_chain_count (each output may be NULL; synchronises the stream): half-sweep launches that ran the double chain and
+ * site updates redone in double, since gf_create. */
+int gf_set_chain(gf_ctx* ctx, int chain, double watch_threshold, double fix_threshold);
+int gf_chain_count(gf_ctx* ctx, unsigned long long* double_launches_host, unsigned long long* double_sites_host);
 /* Optional debug output of gf_anneal: d_trials (device, V*3 unsigned, index 3*s + subgroup) receives the
  * number of Kennedy-Pendleton trials of every (site, subgroup) of the LAST step; NULL switches it off. */
 int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);

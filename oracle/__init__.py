@@ -70,6 +70,8 @@ def _load():
         "orc_su2_square": (None, [_vp, _vp]),
         "orc_site_relax": (None, [N, _int, _vp, ctypes.c_long, _int, _dbl, ctypes.c_uint64, ctypes.c_uint32, _vp]),
         "orc_relax": (None, [N, _int, _vp, _int, _dbl, _int, ctypes.c_uint64, _vp]),
+        "orc_relax_from": (None, [N, _int, _vp, _int, _dbl, _int, _int, ctypes.c_uint64, _vp]),
+        "orc_heatbath_half": (None, [N, _int, _vp, _dbl, ctypes.c_uint64, ctypes.c_uint32, _int, _vp]),
         "orc_fix": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp]),
         "orc_fix_slices": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp, _vp]),
         "orc_anneal_micro": (None, [N, _int, _vp, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp]),
@@ -141,6 +143,27 @@ def relax(U, dims, update: int, param: float, nsweeps: int, seed: int = 0, gauge
     _load().orc_relax(N, gauge, _field(U, V), int(update), float(param), int(nsweeps), int(seed),
                       sq.ctypes.data if squared else None)
     return sq
+
+
+def relax_from(U, dims, update: int, param: float, nsweeps: int, sweep0: int, seed: int = 0, gauge: int = LANDAU,
+               squared: bool = False):
+    """as relax with the sweep counter of the stochastic decisions starting at sweep0 (the chunks of fix)"""
+    N, V = _dims(dims)
+    sq = np.zeros((V, 3), dtype=np.int32) if squared else None
+    _load().orc_relax_from(N, gauge, _field(U, V), int(update), float(param), int(nsweeps), int(sweep0), int(seed),
+                           sq.ctypes.data if squared else None)
+    return sq
+
+
+def heatbath_half(U, dims, T: float, seed: int, step: int, parity: int, gauge: int = LANDAU, trials=None):
+    """one heatbath half-sweep over one sublattice; trials: optional (V, 3) int32 array receiving the trial counts
+    of the updated sites (other entries untouched)"""
+    N, V = _dims(dims)
+    if trials is not None:
+        assert trials.shape == (V, 3) and trials.dtype == np.int32 and trials.flags.c_contiguous
+    _load().orc_heatbath_half(N, gauge, _field(U, V), float(T), int(seed), int(step), int(parity),
+                              trials.ctypes.data if trials is not None else None)
+    return trials
 
 
 def fix(U, dims, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int, seed: int = 0,

@@ -353,7 +353,8 @@ void orc_unitarity_defect(const int N[4], const double *U_, double *max_uudag, d
     *max_det = md;
 }
 
-/* reunitarise every link: Gram-Schmidt rows 0,1; row 2 = conj(row0 x row1) (C15/C16). Not called by parity runs. */
+/* reunitarise every link: Gram-Schmidt rows 0,1; row 2 = conj(row0 x row1) (C15/C16).  The definition of what the
+ * CUDA path's re-orthonormalisation on load computes; not called by the sweeps of the oracle (fp64 needs none). */
 void orc_reunitarise(const int N[4], double *U_)
 {
     cplx *U = (cplx *)U_;
@@ -470,17 +471,23 @@ void orc_site_heatbath(const int N[4], int gauge, double *U_, long s, double T, 
 
 /* simulated annealing: step i = one full sweep (RED then BLACK) at T_i = T_start + (T_end - T_start) i/(nsteps-1)
  * (nsteps = 1 -> T_start) (C13).  trials (may be NULL): V*3 ints, overwritten every step (last step survives). */
+/* one heatbath half-sweep over sublattice `parity` at temperature T, annealing step `step` (C13/C14) */
+void orc_heatbath_half(const int N[4], int gauge, double *U, double T, uint64_t seed, uint32_t step, int parity,
+                       int *trials)
+{
+    const long V = lat_volume(N);
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < V; ++s)
+        if (lat_parity(N, s) == parity) orc_site_heatbath(N, gauge, U, s, T, seed, step, trials);
+}
+
 void orc_anneal(const int N[4], int gauge, double *U, double T_start, double T_end, int nsteps, uint64_t seed,
                 int *trials)
 {
-    const long V = lat_volume(N);
     for (int step = 0; step < nsteps; ++step) {
         double T = (nsteps > 1) ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
-        for (int parity = 0; parity < 2; ++parity) {
-#pragma omp parallel for schedule(static)
-            for (long s = 0; s < V; ++s)
-                if (lat_parity(N, s) == parity) orc_site_heatbath(N, gauge, U, s, T, seed, (uint32_t)step, trials);
-        }
+        for (int parity = 0; parity < 2; ++parity) /* RED, BLACK */
+            orc_heatbath_half(N, gauge, U, T, seed, (uint32_t)step, parity, trials);
     }
 }
 
@@ -548,9 +555,10 @@ void orc_site_relax(const int N[4], int gauge, double *U_, long s, int update, d
     }
 }
 
-/* nsweeps sweeps (RED then BLACK) with the chosen variant; the sweep counter of the random decisions starts at 0 */
-void orc_relax(const int N[4], int gauge, double *U, int update, double param, int nsweeps, uint64_t seed,
-               int *squared)
+/* nsweeps sweeps (RED then BLACK) with the chosen variant; the sweep counter of the random decisions (C18) starts
+ * at sweep0 */
+void orc_relax_from(const int N[4], int gauge, double *U, int update, double param, int nsweeps, int sweep0,
+                    uint64_t seed, int *squared)
 {
     const long V = lat_volume(N);
     for (int sweep = 0; sweep < nsweeps; ++sweep)
@@ -558,22 +566,25 @@ void orc_relax(const int N[4], int gauge, double *U, int update, double param, i
 #pragma omp parallel for schedule(static)
             for (long s = 0; s < V; ++s)
                 if (lat_parity(N, s) == parity)
-                    orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)sweep, squared);
+                    orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)(sweep0 + sweep), squared);
         }
+}
+
+/* one call of the relaxation family: the sweep counter starts at 0 */
+void orc_relax(const int N[4], int gauge, double *U, int update, double param, int nsweeps, uint64_t seed,
+               int *squared)
+{
+    orc_relax_from(N, gauge, U, update, param, nsweeps, 0, seed, squared);
 }
 
 /* annealing with n_micro microcanonical sweeps after every heatbath sweep (C19) */
 void orc_anneal_micro(const int N[4], int gauge, double *U, double T_start, double T_end, int nsteps,
                       int n_micro, uint64_t seed, int *trials)
 {
-    const long V = lat_volume(N);
     for (int step = 0; step < nsteps; ++step) {
         double T = (nsteps > 1) ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
-        for (int parity = 0; parity < 2; ++parity) {
-#pragma omp parallel for schedule(static)
-            for (long s = 0; s < V; ++s)
-                if (lat_parity(N, s) == parity) orc_site_heatbath(N, gauge, U, s, T, seed, (uint32_t)step, trials);
-        }
+        for (int parity = 0; parity < 2; ++parity)
+            orc_heatbath_half(N, gauge, U, T, seed, (uint32_t)step, parity, trials);
         orc_relax(N, gauge, U, ORC_UPDATE_STOCHASTIC, 2.0, n_micro, seed, NULL); /* p = 2 > u always: g^2 */
     }
 }
@@ -582,8 +593,8 @@ void orc_anneal_micro(const int N[4], int gauge, double *U, double T_start, doub
 /* Alg. 1 outer loop ("while precision theta not reached"), with the paper's cadence of   */
 /* the check (F and theta are evaluated after every `check_every`-th iteration; C11):    */
 /* sweep in chunks of check_every (the last chunk is cut at max_sweeps) until theta < theta_tol        */
-/* (Coulomb: max over timeslices, C12).  Each chunk is one orc_relax call, so the sweep counter of the */
-/* stochastic decisions restarts with every chunk.  Returns the number of sweeps done.                 */
+/* (Coulomb: max over timeslices, C12).  The sweep counter of the stochastic decisions (C18) runs on    */
+/* through the chunks: a fixing run never replays its decisions.  Returns the number of sweeps done.   */
 /* ------------------------------------------------------------------------------------------------ */
 int orc_fix(const int N[4], int gauge, double *U, int update, double param, double theta_tol, int check_every,
             int max_sweeps, uint64_t seed, double *theta_out, double *F_out)
@@ -592,7 +603,7 @@ int orc_fix(const int N[4], int gauge, double *U, int update, double param, doub
     double th = orc_theta_report(N, gauge, U);
     while (th >= theta_tol && done < max_sweeps) {
         int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
-        orc_relax(N, gauge, U, update, param, n, seed, NULL);
+        orc_relax_from(N, gauge, U, update, param, n, done, seed, NULL);
         done += n;
         th = orc_theta_report(N, gauge, U);
     }
@@ -611,8 +622,8 @@ int orc_fix(const int N[4], int gauge, double *U, int update, double param, doub
 /* with theta_t < theta_tol are frozen for good; ends when none is active or at max_sweeps.            */
 /* sweeps_per_slice (Nt ints, may be NULL) receives the sweeps each slice got; returns their maximum.   */
 /* ------------------------------------------------------------------------------------------------ */
-void orc_relax_slices(const int N[4], int gauge, double *U, int update, double param, int nsweeps, uint64_t seed,
-                      const unsigned char *active)
+void orc_relax_slices(const int N[4], int gauge, double *U, int update, double param, int nsweeps, int sweep0,
+                      uint64_t seed, const unsigned char *active)
 {
     const long V = lat_volume(N);
     const long Vs = (long)N[0] * N[1] * N[2];
@@ -621,7 +632,7 @@ void orc_relax_slices(const int N[4], int gauge, double *U, int update, double p
 #pragma omp parallel for schedule(static)
             for (long s = 0; s < V; ++s)
                 if (active[s / Vs] && lat_parity(N, s) == parity)
-                    orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)sweep, NULL);
+                    orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)(sweep0 + sweep), NULL);
         }
 }
 
@@ -637,7 +648,7 @@ int orc_fix_slices(const int N[4], int gauge, double *U, int update, double para
     for (int t = 0; t < Nt; ++t) { active[t] = sl[t] >= theta_tol; any |= active[t]; }
     while (any && done < max_sweeps) {
         int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
-        orc_relax_slices(N, gauge, U, update, param, n, seed, active);
+        orc_relax_slices(N, gauge, U, update, param, n, done, seed, active);
         done += n;
         orc_theta(N, gauge, U, sl);
         any = 0;

@@ -56,8 +56,8 @@ SIGNATURES = {
     "gf_set_pdl": (_i, [_vp, _i]),
     "gf_set_prefetch": (_i, [_vp, _i]),
     "gf_set_coulomb_reading": (_i, [_vp, _i]),
-    "gf_set_fusion": (_i, [_vp, _i]),
-    "gf_fusion_schedule": (_i, [_i, _i, _i, _pi, _i]),
+    "gf_set_chain": (_i, [_vp, _i, _d, _d]),
+    "gf_chain_count": (_i, [_vp, ctypes.POINTER(_ull), ctypes.POINTER(_ull)]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
     "gf_launch_count": (_ull, [_vp]),
     "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
@@ -253,19 +253,16 @@ def gf_set_coulomb_reading(ctx, reading_b: bool) -> None:
     _check(ctx, load_library().gf_set_coulomb_reading(ctx, -1 if reading_b is None else int(bool(reading_b))))
 
 
-def gf_set_fusion(ctx, chunk_slices: int) -> None:
-    _check(ctx, load_library().gf_set_fusion(ctx, int(chunk_slices)))
+def gf_set_chain(ctx, chain: int, watch_threshold: float = 0.0, fix_threshold: float = 0.0) -> None:
+    """fp32 contexts: 0 = fp32 site chain, 1 = double, 2 = hybrid (default); thresholds of 0 keep the current values"""
+    _check(ctx, load_library().gf_set_chain(ctx, int(chain), float(watch_threshold), float(fix_threshold)))
 
 
-def gf_fusion_schedule(Nt: int, chunk_slices: int, backward: bool = False):
-    """launch order of one slab-fused sweep: list of (parity, t_begin, t_end)"""
-    lib = load_library()
-    n = lib.gf_fusion_schedule(int(Nt), int(chunk_slices), int(bool(backward)), None, 0)
-    if n < 0:
-        raise GFError(n, "gf_fusion_schedule: invalid arguments")
-    buf = (ctypes.c_int * (3 * n))()
-    lib.gf_fusion_schedule(int(Nt), int(chunk_slices), int(bool(backward)), buf, n)
-    return [(buf[3 * i], buf[3 * i + 1], buf[3 * i + 2]) for i in range(n)]
+def gf_chain_count(ctx):
+    """(half-sweep launches that ran the double chain, site updates redone in double) since gf_create"""
+    a, b = _ull(), _ull()
+    _check(ctx, load_library().gf_chain_count(ctx, ctypes.byref(a), ctypes.byref(b)))
+    return int(a.value), int(b.value)
 
 
 def gf_set_trial_buffer(ctx, d_trials) -> None:

@@ -23,8 +23,11 @@ struct gf_ctx {
     int prefetch;                     // L2 prefetch distance of the sweep kernels, in sites (0 = off)
     int coulomb_b;                    // Coulomb reading B: temporal links transformed once per call (C12)
     void* d_gfield;                   // its accumulated g(x): V links of 18 reals
-    int fuse_slices;                  // > 0: RED and BLACK of one sweep interleaved in chunks of that many timeslices
-    unsigned long long sweeps_done;   // overrelaxation sweeps since creation (cadence of the fp32 reunitarisation)
+    int chain;                        // fp32: precision of the site chain (CHAIN_*)
+    float watch_threshold;            // hybrid chain: conditioning number below which a half-sweep counts as rough
+    float fix_threshold;              // heatbath: |k| below which a site update is redone in double
+    int* d_rough;                     // hybrid chain: ring of ROUGH_RING flags + 4 words for two diagnostic counters
+    unsigned long long call_sweeps;   // sweeps since the start of the current API call (cadence of the reunitarisation)
     unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
     unsigned long long launches;
     unsigned* d_trials;
@@ -91,9 +94,9 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->ld_policy = POLICY_NORMAL; c->st_policy = POLICY_EVICT_LAST; // measured best: profiles/r1_variants.md
     c->pdl = 1;
     c->prefetch = -1; // automatic
-    c->fuse_slices = 0;
+    c->chain = CHAIN_HYBRID; c->watch_threshold = 1.0f; c->fix_threshold = 0.15f; c->d_rough = nullptr;
     c->coulomb_b = -1; c->d_gfield = nullptr; // automatic: reading B in fp32, A in fp64 (uses_reading_b)
-    c->sweeps_done = 0; c->half_sweeps = 0; c->launches = 0;
+    c->call_sweeps = 0; c->half_sweeps = 0; c->launches = 0;
     c->d_trials = nullptr; c->last_stream = nullptr;
     c->d_canon = nullptr; c->d_native = nullptr;
     c->err[0] = 0;
@@ -102,6 +105,8 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->d_partials = nullptr; c->d_out = nullptr; c->h_out = nullptr;
     if ((e = cudaMalloc(&c->d_partials, npart * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc(&c->d_out, (size_t)(Nt + 2) * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_rough, (ROUGH_RING + 4) * sizeof(int))) != cudaSuccess ||
+        (e = cudaMemset(c->d_rough, 0, (ROUGH_RING + 4) * sizeof(int))) != cudaSuccess ||
         (e = cudaMallocHost(&c->h_out, (size_t)(Nt + 2) * sizeof(double))) != cudaSuccess) {
         int rc = cuda_fail(nullptr, e, "gf_create: scratch allocation");
         gf_destroy(c);
@@ -116,6 +121,7 @@ extern "C" void gf_destroy(gf_ctx* c)
     if (c == nullptr) return;
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_out) cudaFree(c->d_out);
+    if (c->d_rough) cudaFree(c->d_rough);
     if (c->h_out) cudaFreeHost(c->h_out);
     if (c->d_canon) cudaFree(c->d_canon);
     if (c->d_native) cudaFree(c->d_native);
@@ -195,6 +201,30 @@ extern "C" int gf_set_trial_buffer(gf_ctx* c, unsigned* d_trials)
     return GF_OK;
 }
 
+extern "C" int gf_set_chain(gf_ctx* c, int chain, double watch_threshold, double fix_threshold)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (chain < 0 || chain > 2) return fail(c, GF_EINVAL, "gf_set_chain: chain must be 0 (fp32), 1 (double) or 2 (hybrid)");
+    if (!(watch_threshold >= 0.0 && watch_threshold <= 1e3)) return fail(c, GF_EINVAL, "gf_set_chain: watch_threshold = %g outside [0, 1e3]", watch_threshold);
+    if (!(fix_threshold >= 0.0 && fix_threshold <= 1e3)) return fail(c, GF_EINVAL, "gf_set_chain: fix_threshold = %g outside [0, 1e3]", fix_threshold);
+    c->chain = chain;
+    if (watch_threshold > 0.0) c->watch_threshold = (float)watch_threshold;
+    if (fix_threshold > 0.0) c->fix_threshold = (float)fix_threshold;
+    return GF_OK;
+}
+
+extern "C" int gf_chain_count(gf_ctx* c, unsigned long long* double_launches_host, unsigned long long* double_sites_host)
+{
+    if (c == nullptr) return GF_EINVAL;
+    unsigned long long both[2] = {0ull, 0ull};
+    cudaError_t e = cudaStreamSynchronize(c->last_stream);
+    if (e == cudaSuccess) e = cudaMemcpy(both, c->d_rough + ROUGH_RING, sizeof both, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gf_chain_count");
+    if (double_launches_host) *double_launches_host = both[0];
+    if (double_sites_host) *double_sites_host = both[1];
+    return GF_OK;
+}
+
 extern "C" unsigned long long gf_launch_count(const gf_ctx* c) { return c ? c->launches : 0ull; }
 
 // Launch shape chosen from the measurements in profiles/ (DESIGN.md "Kernels"): the kernel is latency/bandwidth
@@ -234,6 +264,7 @@ static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p_in, cu
     const int tps = auto_tps(c, mode), block = auto_block(c);
     SweepParams p = p_in;
     p.prefetch = (unsigned)auto_prefetch(c, mode);
+    if (mode == MODE_HEATBATH) p.watch_thr2 = c->chain == CHAIN_FP32 ? 0.0f : c->fix_threshold * c->fix_threshold;
     if (c->precision == GF_FP32) return c->R == 18 ? launch_sweep_f32_r18(tps, mode, block, p, st) : launch_sweep_f32_r12(tps, mode, block, p, st);
     return c->R == 18 ? launch_sweep_f64_r18(tps, mode, block, p, st) : launch_sweep_f64_r12(tps, mode, block, p, st);
 }
@@ -246,8 +277,9 @@ extern "C" int gf_kernel_info(gf_ctx* c, int mode, int* regs, int* local_bytes)
     cudaError_t e;
     const int tps = auto_tps(c, mode);
     const bool rb = uses_reading_b(c, mode);
-    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(tps, mode, rb, &a) : sweep_attributes_f32_r12(tps, mode, rb, &a);
-    else e = c->R == 18 ? sweep_attributes_f64_r18(tps, mode, rb, &a) : sweep_attributes_f64_r12(tps, mode, rb, &a);
+    const bool dc = c->precision == GF_FP32 && c->chain == CHAIN_DOUBLE;
+    if (c->precision == GF_FP32) e = c->R == 18 ? sweep_attributes_f32_r18(tps, mode, rb, dc, &a) : sweep_attributes_f32_r12(tps, mode, rb, dc, &a);
+    else e = c->R == 18 ? sweep_attributes_f64_r18(tps, mode, rb, dc, &a) : sweep_attributes_f64_r12(tps, mode, rb, dc, &a);
     if (e != cudaSuccess) return cuda_fail(c, e, "gf_kernel_info");
     if (regs) *regs = a.numRegs;
     if (local_bytes) *local_bytes = (int)a.localSizeBytes;
@@ -262,12 +294,16 @@ static SweepParams base_params(gf_ctx* c, void* U)
     p.L = c->L;
     p.nd = c->gauge == GF_COULOMB ? 3 : 4;
     p.omega = 1.0;
-    p.T = 1.0;
+    p.ph.T = 1.0;
     p.h_begin = 0;
     p.h_count = c->L.H;
     p.ld_policy = c->ld_policy;
     p.st_policy = c->st_policy;
     p.pdl = c->pdl;
+    p.chain = c->chain;
+    p.watch_thr2 = c->watch_threshold * c->watch_threshold;
+    p.rough = c->d_rough;
+    p.dc_count = reinterpret_cast<unsigned long long*>(c->d_rough + ROUGH_RING);
     return p;
 }
 
@@ -299,53 +335,13 @@ extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* str
 //   EXPONENTIALLY under large rotations (measured x1.5-1.7 per heatbath sweep at T = 1, both precisions: fp32 loses
 //   unitarity after ~50 sweeps, fp64 after ~150) -- every 4th sweep for the hot updates (heatbath, stochastic /
 //   microcanonical), every 16th for overrelaxation, in fp32 and fp64.
+// The cadence counts the sweeps (of any kind) since the start of the current API call, so that a call's result
+// depends on its arguments and the field only, not on the context's history.
 static bool reunit_due(const gf_ctx* c, bool hot)
 {
     int every = c->reunit_every;
     if (every < 0) every = c->R == 12 ? (hot ? 4 : 16) : (c->precision == GF_FP32 ? 16 : 0);
-    return every > 0 && ((c->sweeps_done + 1) % (unsigned long long)every) == 0;
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// L2 fusion of the two half-sweeps of one sweep.  BLACK on timeslice t needs
-// RED finished on t-1, t, t+1 (the only links a site shares with other timeslices are the temporal ones), so the
-// sweep can run as a wavefront in t: RED on a chunk of timeslices, then BLACK on the slices whose three RED
-// neighbours are done, and so on; the links BLACK reads were written by RED a moment ago and are still in L2,
-// and RED's dirty lines are overwritten by BLACK before they are written back.  Only the order of launches
-// changes: every (parity, site) is updated exactly once per sweep from the same inputs, results are bit-identical.
-// Schedule: triples (parity, t_begin, t_end) for one sweep; `backward` walks t from Nt-1 down (consecutive sweeps
-// alternate, so a sweep starts on the slices the previous one finished on).  Returns the number of triples.
-// ---------------------------------------------------------------------------------------------------------
-static int fusion_schedule(int Nt, int chunk, int backward, int* out, int cap)
-{
-    int n = 0;
-    auto emit = [&](int parity, int a, int b) { // slices [a, b) in walk coordinates
-        if (a >= b) return;
-        if (n < cap) {
-            out[3 * n] = parity;
-            out[3 * n + 1] = backward ? Nt - b : a;
-            out[3 * n + 2] = backward ? Nt - a : b;
-        }
-        ++n;
-    };
-    if (chunk < 1) chunk = 1;
-    int r = 0, b = 1; // RED done on walk slices [0, r); BLACK done on [1, b)
-    while (r < Nt) {
-        const int r1 = r + chunk < Nt ? r + chunk : Nt;
-        emit(0, r, r1);
-        r = r1;
-        const int b1 = r < Nt ? r - 1 : Nt; // BLACK on t needs RED on t+1; the last slice's t+1 is slice 0: done
-        if (b1 > b) { emit(1, b, b1); b = b1; }
-    }
-    if (Nt > 1) emit(1, 0, 1); // slice 0 needs RED on the last slice
-    else emit(1, 0, 1);
-    return n;
-}
-
-extern "C" int gf_fusion_schedule(int Nt, int chunk_slices, int backward, int* triples, int capacity)
-{
-    if (Nt < 1 || chunk_slices < 1 || capacity < 0 || (capacity > 0 && triples == nullptr)) return GF_EINVAL;
-    return fusion_schedule(Nt, chunk_slices, backward ? 1 : 0, triples, capacity);
+    return every > 0 && ((c->call_sweeps + 1) % (unsigned long long)every) == 0;
 }
 
 extern "C" int gf_set_coulomb_reading(gf_ctx* c, int reading_b)
@@ -356,19 +352,37 @@ extern "C" int gf_set_coulomb_reading(gf_ctx* c, int reading_b)
     return GF_OK;
 }
 
-extern "C" int gf_set_fusion(gf_ctx* c, int chunk_slices)
+// the per-half-sweep part of the launch parameters
+static void set_phase(gf_ctx* c, SweepParams& p, int parity, bool reunit)
 {
-    if (c == nullptr) return GF_EINVAL;
-    if (chunk_slices < 0) return fail(c, GF_EINVAL, "gf_set_fusion: chunk_slices must be >= 0");
-    c->fuse_slices = chunk_slices;
+    p.ph.parity = parity;
+    p.ph.reunit = (reunit && parity == 0) ? 1 : 0; // every link is loaded once per half-sweep (C6)
+    p.ph.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
+    // hybrid chain (fp32): the ring position counts the half-sweeps of the call; its first sweep runs the double chain
+    p.ph.rough_slot = (int)((2ull * c->call_sweeps + (unsigned)parity) % ROUGH_RING);
+    p.ph.rough_force = c->call_sweeps == 0 ? 1 : 0;
+}
+
+// start of an API call that sweeps: the sweep counter of the call and, for the hybrid chain, a clean flag ring
+static int begin_call(gf_ctx* c, cudaStream_t st)
+{
+    c->call_sweeps = 0;
+    c->last_stream = st;
+    if (c->precision == GF_FP32 && c->chain == CHAIN_HYBRID) {
+        cudaError_t e = cudaMemsetAsync(c->d_rough, 0, ROUGH_RING * sizeof(int), st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "roughness flags");
+    }
     return GF_OK;
 }
 
 // nsweeps sweeps (RED then BLACK) of one member of the relaxation family on `st`
+// sweep0: index of the first of them within the API call that runs them (the counter of the stochastic decisions,
+//   C18: it restarts at 0 with every gf_relax call and runs on through the chunks of gf_fix / gf_fix_slices)
 // active (may be NULL = all): Nt flags; only the sites of the flagged timeslices are updated, one launch per
 // maximal run of consecutive flagged slices (their half-site indices are contiguous) -- C20
-static int run_sweeps_core(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
-                           cudaStream_t st, const char* who, const unsigned char* active, void* gfield)
+static int run_sweeps_core(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, int sweep0,
+                           unsigned long long seed, cudaStream_t st, const char* who, const unsigned char* active,
+                           void* gfield, int* launched = nullptr)
 {
     c->last_stream = st;
     SweepParams p = base_params(c, U);
@@ -379,39 +393,14 @@ static int run_sweeps_core(gf_ctx* c, void* U, int mode, int variant, double par
     p.key1 = (uint32_t)(seed >> 32);
     for (int sweep = 0; sweep < nsweeps; ++sweep) {
         const bool reunit = reunit_due(c, mode == MODE_VARIANT && variant == VARIANT_STOCHASTIC);
-        p.step = (uint32_t)sweep; // sweep counter of the random decisions (C18): restarts at 0 with every call
-        if (c->fuse_slices > 0 && active == nullptr && c->Nt >= 4) {
-            // slab-fused sweep: same updates, launched as a wavefront in t
-            int sched[3 * 260];
-            const int backward = (int)(c->sweeps_done & 1ull);
-            const int chunk = c->fuse_slices > c->Nt ? c->Nt : c->fuse_slices;
-            int n = fusion_schedule(c->Nt, chunk, backward, sched, 260);
-            if (n > 260) return fail(c, GF_EINVAL, "%s: fusion schedule too long (Nt = %d, chunk = %d)", who, c->Nt, chunk);
-            const unsigned Hs = c->L.H / (unsigned)c->Nt;
-            for (int i = 0; i < n; ++i) {
-                p.parity = sched[3 * i];
-                p.reunit = (reunit && p.parity == 0) ? 1 : 0;
-                p.reverse = backward;
-                p.h_begin = (unsigned)sched[3 * i + 1] * Hs;
-                p.h_count = (unsigned)(sched[3 * i + 2] - sched[3 * i + 1]) * Hs;
-                cudaError_t e = launch_sweep(c, mode, p, st);
-                if (e != cudaSuccess) return cuda_fail(c, e, who);
-                c->launches += 1;
-            }
-            p.h_begin = 0;
-            p.h_count = c->L.H;
-            c->half_sweeps += 2;
-            c->sweeps_done += 1;
-            continue;
-        }
+        p.ph.step = (uint32_t)(sweep0 + sweep);
         for (int parity = 0; parity < 2; ++parity) { // RED, BLACK
-            p.parity = parity;
-            p.reunit = (reunit && parity == 0) ? 1 : 0; // every link is loaded once per half-sweep (C6)
-            p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
+            set_phase(c, p, parity, reunit);
             if (active == nullptr) {
                 cudaError_t e = launch_sweep(c, mode, p, st);
                 if (e != cudaSuccess) return cuda_fail(c, e, who);
                 c->launches += 1;
+                if (launched) *launched += 1;
             } else {
                 const unsigned Hs = c->L.H / (unsigned)c->Nt; // half-sites per timeslice
                 for (int t = 0; t < c->Nt;) {
@@ -423,12 +412,13 @@ static int run_sweeps_core(gf_ctx* c, void* U, int mode, int variant, double par
                     cudaError_t e = launch_sweep(c, mode, p, st);
                     if (e != cudaSuccess) return cuda_fail(c, e, who);
                     c->launches += 1;
+                    if (launched) *launched += 1;
                     t = t1;
                 }
             }
             c->half_sweeps += 1;
         }
-        c->sweeps_done += 1;
+        c->call_sweeps += 1;
     }
     return GF_OK;
 }
@@ -479,44 +469,63 @@ static int reading_b_end(gf_ctx* c, void* U, void* gfield, cudaStream_t st, cons
     return GF_OK;
 }
 
-static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, unsigned long long seed,
-                      cudaStream_t st, const char* who, const unsigned char* active = nullptr)
+// One chunk of sweeps with the Coulomb reading-B bracket around it.  If a launch fails after sweeps have been
+// enqueued, the temporal links are still transformed with the g(x) accumulated so far (reading_b_end), so that the
+// field stays a gauge transform of the input; the first error is the one reported.
+static int run_sweeps(gf_ctx* c, void* U, int mode, int variant, double param, int nsweeps, int sweep0,
+                      unsigned long long seed, cudaStream_t st, const char* who, const unsigned char* active = nullptr)
 {
     if (nsweeps == 0) return GF_OK;
     void* gfield;
     int rc = reading_b_begin(c, mode, st, &gfield, who);
-    if (rc == GF_OK) rc = run_sweeps_core(c, U, mode, variant, param, nsweeps, seed, st, who, active, gfield);
-    if (rc == GF_OK) rc = reading_b_end(c, U, gfield, st, who);
+    if (rc != GF_OK) return rc;
+    int launched = 0;
+    rc = run_sweeps_core(c, U, mode, variant, param, nsweeps, sweep0, seed, st, who, active, gfield, &launched);
+    if (rc == GF_OK || launched > 0) {
+        char first[512];
+        if (rc != GF_OK) memcpy(first, c->err, sizeof first);
+        const int rc2 = reading_b_end(c, U, gfield, st, who);
+        if (rc != GF_OK) memcpy(c->err, first, sizeof first);
+        else rc = rc2;
+    }
     return rc;
+}
+
+// argument check and dispatch of one member of the relaxation family (gf_relax, and the chunks of gf_fix)
+static int relax_chunk(gf_ctx* c, void* U, int update, double param, int nsweeps, int sweep0, unsigned long long seed,
+                       cudaStream_t st, const char* who, const unsigned char* active = nullptr)
+{
+    if (U == nullptr) return fail(c, GF_EINVAL, "%s: U is NULL", who);
+    if (nsweeps < 0) return fail(c, GF_EINVAL, "%s: nsweeps = %d < 0", who, nsweeps);
+    switch (update) {
+    case GF_UPDATE_OVERRELAX2:
+        if (!(param >= 1.0 && param < 2.0)) return fail(c, GF_EINVAL, "%s: omega = %g outside [1,2) (PAPER.md:63)", who, param);
+        return run_sweeps(c, U, MODE_OVERRELAX, 0, param, nsweeps, sweep0, 0ull, st, who, active);
+    case GF_UPDATE_OVERRELAX1:
+        if (!(param >= 1.0 && param < 2.0)) return fail(c, GF_EINVAL, "%s: omega = %g outside [1,2) (PAPER.md:63)", who, param);
+        return run_sweeps(c, U, MODE_VARIANT, VARIANT_OVERRELAX1, param, nsweeps, sweep0, seed, st, who, active);
+    case GF_UPDATE_STOCHASTIC:
+        if (!(param >= 0.0 && param <= 1.0)) return fail(c, GF_EINVAL, "%s: probability p = %g outside [0,1]", who, param);
+        return run_sweeps(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, param, nsweeps, sweep0, seed, st, who, active);
+    default:
+        return fail(c, GF_EINVAL, "%s: unknown update %d", who, update);
+    }
 }
 
 extern "C" int gf_overrelax(gf_ctx* c, void* U, double omega, int nsweeps, void* stream)
 {
     if (c == nullptr) return GF_EINVAL;
-    if (U == nullptr) return fail(c, GF_EINVAL, "gf_overrelax: U is NULL");
-    if (!(omega >= 1.0 && omega < 2.0)) return fail(c, GF_EINVAL, "gf_overrelax: omega = %g outside [1,2) (PAPER.md:63)", omega);
-    if (nsweeps < 0) return fail(c, GF_EINVAL, "gf_overrelax: nsweeps = %d < 0", nsweeps);
-    return run_sweeps(c, U, MODE_OVERRELAX, 0, omega, nsweeps, 0ull, (cudaStream_t)stream, "gf_overrelax: kernel launch");
+    int rc = begin_call(c, (cudaStream_t)stream);
+    if (rc != GF_OK) return rc;
+    return relax_chunk(c, U, GF_UPDATE_OVERRELAX2, omega, nsweeps, 0, 0ull, (cudaStream_t)stream, "gf_overrelax");
 }
 
 extern "C" int gf_relax(gf_ctx* c, void* U, int update, double param, int nsweeps, unsigned long long seed, void* stream)
 {
     if (c == nullptr) return GF_EINVAL;
-    if (U == nullptr) return fail(c, GF_EINVAL, "gf_relax: U is NULL");
-    if (nsweeps < 0) return fail(c, GF_EINVAL, "gf_relax: nsweeps = %d < 0", nsweeps);
-    cudaStream_t st = (cudaStream_t)stream;
-    switch (update) {
-    case GF_UPDATE_OVERRELAX2:
-        return gf_overrelax(c, U, param, nsweeps, stream);
-    case GF_UPDATE_OVERRELAX1:
-        if (!(param >= 1.0 && param < 2.0)) return fail(c, GF_EINVAL, "gf_relax: omega = %g outside [1,2) (PAPER.md:63)", param);
-        return run_sweeps(c, U, MODE_VARIANT, VARIANT_OVERRELAX1, param, nsweeps, seed, st, "gf_relax: kernel launch");
-    case GF_UPDATE_STOCHASTIC:
-        if (!(param >= 0.0 && param <= 1.0)) return fail(c, GF_EINVAL, "gf_relax: probability p = %g outside [0,1]", param);
-        return run_sweeps(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, param, nsweeps, seed, st, "gf_relax: kernel launch");
-    default:
-        return fail(c, GF_EINVAL, "gf_relax: unknown update %d", update);
-    }
+    int rc = begin_call(c, (cudaStream_t)stream);
+    if (rc != GF_OK) return rc;
+    return relax_chunk(c, U, update, param, nsweeps, 0, seed, (cudaStream_t)stream, "gf_relax");
 }
 
 extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, int n_micro,
@@ -528,39 +537,47 @@ extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end,
     if (nsteps < 0) return fail(c, GF_EINVAL, "gf_anneal: nsteps = %d < 0", nsteps);
     if (n_micro < 0) return fail(c, GF_EINVAL, "gf_anneal_micro: n_micro = %d < 0", n_micro);
     cudaStream_t st = (cudaStream_t)stream;
-    c->last_stream = st;
+    int rc = begin_call(c, st);
+    if (rc != GF_OK) return rc;
     SweepParams p = base_params(c, U);
     p.key0 = (uint32_t)seed;
     p.key1 = (uint32_t)(seed >> 32);
     if (nsteps == 0) return GF_OK;
     void* gfield; // Coulomb reading B: one g(x) field over the whole call, heatbath and microcanonical sweeps alike
-    int rc0 = reading_b_begin(c, MODE_HEATBATH, st, &gfield, "gf_anneal");
-    if (rc0 != GF_OK) return rc0;
+    rc = reading_b_begin(c, MODE_HEATBATH, st, &gfield, "gf_anneal");
+    if (rc != GF_OK) return rc;
     p.G = gfield;
-    for (int step = 0; step < nsteps; ++step) {
+    int launched = 0;
+    for (int step = 0; step < nsteps && rc == GF_OK; ++step) {
         // T_i = T_start + (T_end - T_start) i / (nsteps - 1)   (C13)
-        p.T = nsteps > 1 ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
-        p.step = (uint32_t)step;
+        p.ph.T = nsteps > 1 ? T_start + (T_end - T_start) * (double)step / (double)(nsteps - 1) : T_start;
+        p.ph.step = (uint32_t)step;
         p.trials = (step == nsteps - 1) ? c->d_trials : nullptr;
         const bool reunit = reunit_due(c, true);
-        for (int parity = 0; parity < 2; ++parity) {
-            p.parity = parity;
-            p.reunit = (reunit && parity == 0) ? 1 : 0;
-            p.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
+        for (int parity = 0; parity < 2 && rc == GF_OK; ++parity) {
+            set_phase(c, p, parity, reunit);
             cudaError_t e = launch_sweep(c, MODE_HEATBATH, p, st);
-            if (e != cudaSuccess) return cuda_fail(c, e, "gf_anneal: kernel launch");
+            if (e != cudaSuccess) { rc = cuda_fail(c, e, "gf_anneal: kernel launch"); break; }
             c->half_sweeps += 1;
             c->launches += 1;
+            launched += 1;
         }
-        c->sweeps_done += 1;
+        if (rc != GF_OK) break;
+        c->call_sweeps += 1;
         // microcanonical sweeps g -> g^2 (C19): stochastic relaxation with p = 2 > u, i.e. always
-        if (n_micro > 0) {
-            int rc = run_sweeps_core(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, seed, st,
-                                     "gf_anneal_micro: kernel launch", nullptr, gfield);
-            if (rc != GF_OK) return rc;
-        }
+        if (n_micro > 0)
+            rc = run_sweeps_core(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, 0, seed, st,
+                                 "gf_anneal_micro: kernel launch", nullptr, gfield, &launched);
     }
-    return reading_b_end(c, U, gfield, st, "gf_anneal");
+    // after a failed launch the temporal links are still transformed with the g(x) accumulated so far (reading B)
+    if (rc == GF_OK || launched > 0) {
+        char first[512];
+        if (rc != GF_OK) memcpy(first, c->err, sizeof first);
+        const int rc2 = reading_b_end(c, U, gfield, st, "gf_anneal");
+        if (rc != GF_OK) memcpy(c->err, first, sizeof first);
+        else rc = rc2;
+    }
+    return rc;
 }
 
 extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int nsteps, unsigned long long seed, void* stream)
@@ -622,14 +639,15 @@ extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta
     if (check_every < 1) return fail(c, GF_EINVAL, "gf_fix: check_every = %d < 1", check_every);
     if (max_sweeps < 0) return fail(c, GF_EINVAL, "gf_fix: max_sweeps = %d < 0", max_sweeps);
     if (!(theta_tol >= 0.0)) return fail(c, GF_EINVAL, "gf_fix: theta_tol = %g < 0", theta_tol);
-    c->last_stream = (cudaStream_t)stream;
     int done = 0;
     double th = 0.0;
-    int rc = gf_theta(c, U, &th);
+    int rc = begin_call(c, (cudaStream_t)stream);
+    if (rc == GF_OK) rc = relax_chunk(c, U, update, param, 0, 0, seed, (cudaStream_t)stream, "gf_fix"); // argument check
+    if (rc == GF_OK) rc = gf_theta(c, U, &th);
     // Alg. 1: "while precision theta not reached", checked every check_every-th sweep
     while (rc == GF_OK && th >= theta_tol && done < max_sweeps) {
         const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
-        rc = gf_relax(c, U, update, param, n, seed, stream);
+        rc = relax_chunk(c, U, update, param, n, done, seed, (cudaStream_t)stream, "gf_fix");
         done += n;
         if (rc == GF_OK) rc = gf_theta(c, U, &th);
     }
@@ -660,7 +678,7 @@ extern "C" int gf_fix_slices(gf_ctx* c, void* U, int update, double param, doubl
     if (update == GF_UPDATE_STOCHASTIC ? !(param >= 0.0 && param <= 1.0) : !(param >= 1.0 && param < 2.0))
         return fail(c, GF_EINVAL, "gf_fix_slices: parameter %g out of range for update %d", param, update);
     cudaStream_t st = (cudaStream_t)stream;
-    c->last_stream = st;
+    if (begin_call(c, st) != GF_OK) return GF_ECUDA;
     const int Nt = c->Nt;
     unsigned char* active = new (std::nothrow) unsigned char[Nt];
     int* count = new (std::nothrow) int[Nt];
@@ -671,7 +689,7 @@ extern "C" int gf_fix_slices(gf_ctx* c, void* U, int update, double param, doubl
     // Alg. 1 with the stop rule per timeslice: a slice below the tolerance at a check is frozen for good
     while (rc == GF_OK && any && done < max_sweeps) {
         const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
-        rc = run_sweeps(c, U, mode, variant, param, n, seed, st, "gf_fix_slices: kernel launch", active);
+        rc = run_sweeps(c, U, mode, variant, param, n, done, seed, st, "gf_fix_slices: kernel launch", active);
         done += n;
         if (rc == GF_OK) rc = reduce_to_host(c, U, true, "gf_fix_slices");
         any = 0;

@@ -254,7 +254,8 @@ struct LinkIO<double, R> {
 template <int R>
 struct LinkIO<float, R> {
     static constexpr int NQ = R / 4; // float4 planes: 4 (R18) or 3 (R12)
-    static __device__ __forceinline__ void load(const float* blk, size_t H, size_t h, cx<float> (&u)[9], uint64_t pol)
+    // the stored entries only (R = 12: u[6..8] untouched)
+    static __device__ __forceinline__ void load_stored(const float* blk, size_t H, size_t h, cx<float> (&u)[9], uint64_t pol)
     {
         const float4* p = reinterpret_cast<const float4*>(blk) + h;
 #pragma unroll
@@ -266,9 +267,29 @@ struct LinkIO<float, R> {
         if (R == 18) {
             float2 v = ldg(reinterpret_cast<const float2*>(blk + 16 * H) + h, pol);
             u[8] = {v.x, v.y};
-        } else {
-            rebuild_row2(u);
         }
+    }
+    static __device__ __forceinline__ void load(const float* blk, size_t H, size_t h, cx<float> (&u)[9], uint64_t pol)
+    {
+        load_stored(blk, H, h, u, pol);
+        if (R == 12) rebuild_row2(u);
+    }
+    // float storage, double arithmetic (the rare-path fix-up of the fp32 sweep, gf_sweep.cuh): the stored floats are
+    // widened exactly; R = 12: row 2 is rebuilt in double
+    static __device__ __forceinline__ void load(const float* blk, size_t H, size_t h, cx<double> (&u)[9], uint64_t pol)
+    {
+        cx<float> v[9];
+        load_stored(blk, H, h, v, pol);
+#pragma unroll
+        for (int e = 0; e < R / 2; ++e) u[e] = {(double)v[e].re, (double)v[e].im};
+        if (R == 12) rebuild_row2(u);
+    }
+    static __device__ __forceinline__ void store(float* blk, size_t H, size_t h, const cx<double> (&u)[9], uint64_t pol)
+    {
+        cx<float> v[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) v[e] = {(float)u[e].re, (float)u[e].im};
+        store(blk, H, h, v, pol);
     }
     static __device__ __forceinline__ double trace_re(const float* blk, size_t H, size_t h, uint64_t pol)
     {

@@ -10,7 +10,7 @@ struct Lattice;
 // gf_sweep_inst.cu, one pair per (precision, reals-per-link)
 #define GF_DECLARE_SWEEP(sfx)                                                                                 \
     cudaError_t launch_sweep_##sfx(int tps, int mode, int block, const SweepParams& p, cudaStream_t stream); \
-    cudaError_t sweep_attributes_##sfx(int tps, int mode, bool reading_b, cudaFuncAttributes* attr);
+    cudaError_t sweep_attributes_##sfx(int tps, int mode, bool reading_b, bool dc, cudaFuncAttributes* attr);
 GF_DECLARE_SWEEP(f32_r12)
 GF_DECLARE_SWEEP(f32_r18)
 GF_DECLARE_SWEEP(f64_r12)

@@ -11,6 +11,8 @@
 // Memory: every link is read once and written once per half-sweep (C6), each access a coalesced 128-bit
 // vector per thread (gf_device.cuh); all loads of a thread are issued before the first use.
 #pragma once
+#include <type_traits>
+
 #include "gf_device.cuh"
 
 namespace gf {
@@ -21,13 +23,24 @@ enum { MODE_OVERRELAX = 0, MODE_HEATBATH = 1, MODE_VARIANT = 2 };
 enum { VARIANT_OVERRELAX1 = 1, VARIANT_STOCHASTIC = 2 };
 constexpr int MAX_BLOCK = 256;
 
+// what changes from one half-sweep to the next
+struct SweepPhase {
+    int parity;      // sublattice updated: 0 = RED, 1 = BLACK (C5)
+    int reunit;      // re-orthonormalise links on load (C15)
+    int reverse;     // traverse blocks back to front (L2 reuse between consecutive half-sweeps)
+    uint32_t step;   // Philox counter word 1: annealing step / sweep index within the call (C14, C18)
+    double T;        // heatbath temperature (C13)
+    int rough_slot;  // hybrid chain: position of this half-sweep in the ring of roughness flags
+    int rough_force; // hybrid chain: take the double chain regardless of the flags (first sweep of a call)
+};
+
+enum { CHAIN_FP32 = 0, CHAIN_DOUBLE = 1, CHAIN_HYBRID = 2 };
+constexpr int ROUGH_RING = 4;
+
 struct SweepParams {
     void* U;        // native field
     Lattice L;
-    int parity;     // sublattice updated by this launch: 0 = RED, 1 = BLACK (C5)
     int nd;         // directions entering K: 4 (Landau) or 3 (Coulomb, C12)
-    int reunit;     // re-orthonormalise links on load (C15)
-    int reverse;    // traverse blocks back to front (L2 reuse between consecutive half-sweeps)
     int ld_policy;  // L2 policy of the link loads / stores (POLICY_*, gf_device.cuh)
     int st_policy;
     int pdl;        // launched with programmatic stream serialization: wait for the previous grid before loading
@@ -35,10 +48,16 @@ struct SweepParams {
     unsigned prefetch; // L2 prefetch distance in sites along the traversal direction (0 = off)
     double omega;   // overrelaxation parameter; MODE_VARIANT: omega (first order) or probability p
     int variant;    // MODE_VARIANT: VARIANT_*
-    double T;       // heatbath temperature (C13)
-    uint32_t key0, key1, step; // Philox key = seed, step = annealing step (C14)
+    uint32_t key0, key1;       // Philox key = seed (C14)
     unsigned* trials;          // optional: KP trial counts, index 3*s + subgroup
     void* G;                   // Coulomb reading B (C12): accumulated g(x), 2 parity blocks of 18 reals per site
+    // fp32 kernels: precision of the site chain (K(x), the three SU(2) steps, K <- G K), DESIGN.md sec. 4
+    int chain;                 // CHAIN_*
+    float watch_thr2;          // relaxation, CHAIN_HYBRID: a step whose conditioning number (squared) is below this marks
+                               // the half-sweep rough; heatbath: a site with |k|^2 below it is redone in double
+    int* rough;                // CHAIN_HYBRID: ring of ROUGH_RING flags, one per half-sweep
+    unsigned long long* dc_count; // diagnostic: [0] launches that ran the double chain, [1] sites redone in double
+    SweepPhase ph;
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -52,8 +71,11 @@ template <typename T> struct Tiny;
 template <> struct Tiny<float> { static constexpr float sq = 1e-36f; };
 template <> struct Tiny<double> { static constexpr double sq = 1e-300; };
 
+// cond: the conditioning number of the step, |k|^2 |h|^2 (h before its normalisation).  g = k/|k| turns an absolute
+// rounding error e of K into e/|k|, the reprojection h/|h| into e/(|k||h|) (|h| falls to 0.02 at g0 = -1 for
+// omega = 1.7, C9): the fp32 kernels redo a site in double where cond is small (fixup_site_f64 below).
 template <typename T>
-__device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[4])
+__device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[4], T& cond)
 {
     // branch-free: the guards (C9) are selects at the end, so that the compiler can schedule this dependent chain
     // together with the independent link updates of the previous subgroup
@@ -68,6 +90,7 @@ __device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[
     const T n2 = dot4(h0, h0, h1, h1, h2, h2, h3, h3);
     const bool ok2 = n2 >= T(1e-20);
     const T hn = gf_rsqrt<T>(ok2 ? n2 : T(1));
+    cond = n2k * n2;
     h[0] = ok ? (ok2 ? h0 * hn : g0) : T(1);
     h[1] = ok ? (ok2 ? h1 * hn : g1) : T(0);
     h[2] = ok ? (ok2 ? h2 * hn : g2) : T(0);
@@ -80,9 +103,11 @@ __device__ __forceinline__ void su2_overrelax_step(const T (&k)[4], T w, T (&h)[
 // 0x40000000), so fp32 and fp64 kernels decide exactly like the oracle.
 template <typename T>
 __device__ __forceinline__ void su2_variant_step(const T (&k)[4], int variant, double param, uint32_t key0,
-                                                 uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2, T (&h)[4])
+                                                 uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2, T (&h)[4],
+                                                 T& cond)
 {
     const T n2k = dot4(k[0], k[0], k[1], k[1], k[2], k[2], k[3], k[3]);
+    cond = n2k; // first order: |h|^2 = 1 - 2 w (w-1) (g0-1) >= 1; g^2 is not normalised
     if (!(n2k >= Tiny<T>::sq)) { h[0] = T(1); h[1] = h[2] = h[3] = T(0); return; }
     const T inv = gf_rsqrt<T>(n2k);
     const T g0 = k[0] * inv, g1 = -k[1] * inv, g2 = -k[2] * inv, g3 = -k[3] * inv;
@@ -123,44 +148,62 @@ template <> struct KPMath<double> {
     static __device__ __forceinline__ double cos2pi(double u) { return cospi(2.0 * u); }
     static __device__ __forceinline__ double sin2pi(double u) { return sinpi(2.0 * u); }
     static __device__ __forceinline__ double neglog(double u) { return -log(u); }
-    static __device__ __forceinline__ void prep(double n2, double T, double& alpha, double& inv_alpha, double& inv_n)
-    {
-        inv_n = rsqrt(n2);
-        alpha = n2 * inv_n / T;
-        inv_alpha = T * inv_n;
-    }
     static __device__ __forceinline__ double root(double x) { return x > 0.0 ? x * rsqrt(x) : 0.0; }
-    static __device__ __forceinline__ double delta(double l1, double l2, double c, double alpha, double inv_alpha)
+    // one Kennedy-Pendleton trial from its Philox block (C14): delta, accept iff u4^2 <= 1 - delta/2
+    static __device__ __forceinline__ bool trial(const uint32_t (&x)[4], double n2, double Td, double inv_alpha, double& d,
+                                                 double& est)
     {
-        (void)alpha;
-        return fma(l1, c * c, l2) * inv_alpha;
+        (void)n2; (void)Td;
+        est = 0.0; // never refined
+        const double c = cos2pi(uni(x[2]));
+        d = fma(neglog(uni(x[0])), c * c, neglog(uni(x[1]))) * inv_alpha;
+        const double u4 = uni(x[3]);
+        return u4 * u4 <= fma(-0.5, d, 1.0);
     }
-    static __device__ __forceinline__ bool accept(double u4, double d) { return u4 * u4 <= fma(-0.5, d, 1.0); }
 };
-// fp32: decision parity with the fp64 oracle cannot be exact (alpha itself differs at 1e-7, C14), so the draw uses
-// the SFU: u from the mantissa trick (exact), -ln u = -ln2 * lg2(u) (MUFU.LG2, abs. error ~4e-7), cos/sin by
-// MUFU.COS/SIN (abs. error ~5e-7), one reciprocal of alpha per subgroup instead of two divisions per trial.
-// A decision flips when u4^2 falls within ~1e-6/alpha of the threshold: ~1e-6 of the (site, subgroup) draws.
+
+// delta of one trial in double from the block norm |k|^2, for the fp32 kernel: the accept test of borderline trials
+// and the value of delta where the SFU draw is not accurate enough (small alpha, large -ln u)
+static __device__ __noinline__ double kp_delta_f64(double n2, double Td, uint32_t x0, uint32_t x1, uint32_t x2)
+{
+    using M = KPMath<double>;
+    const double alpha = sqrt(n2) / Td;
+    const double c = M::cos2pi(M::uni(x2));
+    return (M::neglog(M::uni(x0)) / alpha) * (c * c) + (M::neglog(M::uni(x1)) / alpha);
+}
+
+// fp32: the draw runs on the SFU: u from the mantissa trick (exact), -ln u = -ln2 * lg2(u) (MUFU.LG2), cos/sin by
+// MUFU.COS/SIN, one reciprocal of alpha per subgroup instead of two divisions per trial.  The SFU value of
+// delta carries an absolute error of up to ~1e-6 (1 + l1 + l2)/alpha (lg2: 2 ulp, 2^-22 near 1; cos: ~4e-7), which
+// would flip ~1e-6 of the accept decisions against the fp64 oracle.  Two-tier test: a trial whose u4^2 falls inside
+// that error band of the threshold is decided again in double (kp_accept_f64, from the same |k|^2 and Philox block);
+// what is left are the flips caused by the fp32 rounding of K itself (alpha differs from the oracle's at ~1e-7).
 template <> struct KPMath<float> {
     // (2 (x >> 9) + 1) 2^-24 = [1 + (x >> 9) 2^-23] - (1 - 2^-24): both terms and the result are fp32 numbers
     static __device__ __forceinline__ float uni(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994039535522461f; }
     static __device__ __forceinline__ float cos2pi(float u) { return __cosf(6.283185307179586f * u); }
     static __device__ __forceinline__ float sin2pi(float u) { return __sinf(6.283185307179586f * u); }
     static __device__ __forceinline__ float neglog(float u) { return -0.693147180559945f * __log2f(u); }
-    // no division, no IEEE square root: 1/|k| by MUFU.RSQ + one Newton step, alpha and 1/alpha from it
-    static __device__ __forceinline__ void prep(float n2, float T, float& alpha, float& inv_alpha, float& inv_n)
-    {
-        inv_n = gf_rsqrt<float>(n2);
-        alpha = n2 * inv_n * __frcp_rn(T);
-        inv_alpha = T * inv_n;
-    }
     static __device__ __forceinline__ float root(float x) { return x > 0.0f ? x * rsqrtf(x) : 0.0f; }
-    static __device__ __forceinline__ float delta(float l1, float l2, float c, float alpha, float inv_alpha)
+    // est: inv_alpha (1 + l1 + l2), the scale of the absolute error of the SFU value of delta (in units of ~5e-7)
+    static __device__ __forceinline__ bool trial(const uint32_t (&x)[4], double n2, double Td, float inv_alpha, float& d,
+                                                 float& est)
     {
-        (void)alpha;
-        return fmaf(l1, c * c, l2) * inv_alpha;
+        // cos^2(2 pi u3) = (1 + cos(4 pi u3)) / 2, the argument folded exactly into [-pi, pi] (MUFU.COS is specified
+        // there): the absolute error of c^2 is half that of the SFU cosine instead of 2 |c| times it
+        const float v = 2.0f * uni(x[2]);
+        const float c2 = fmaf(0.5f, __cosf(6.283185307179586f * (v - rintf(v))), 0.5f);
+        const float l1 = neglog(uni(x[0])), l2 = neglog(uni(x[1]));
+        d = fmaf(l1, c2, l2) * inv_alpha;
+        const float u4 = uni(x[3]);
+        const float diff = fmaf(u4, u4, fmaf(0.5f, d, -1.0f)); // u4^2 - (1 - delta/2)
+        est = inv_alpha * (1.0f + l1 + l2);
+        if (fabsf(diff) < fmaf(2e-6f, est, 3e-7f)) {
+            const double u4d = KPMath<double>::uni(x[3]);
+            return u4d * u4d <= 1.0 - 0.5 * kp_delta_f64(n2, Td, x[0], x[1], x[2]);
+        }
+        return diff <= 0.0f;
     }
-    static __device__ __forceinline__ bool accept(float u4, float d) { return u4 * u4 <= fmaf(-0.5f, d, 1.0f); }
 };
 
 // The Philox counters of a draw hold (site, step, parity, subgroup, trial) and no data, so the block of trial 0
@@ -181,44 +224,38 @@ __device__ __forceinline__ void early_random(uint32_t key0, uint32_t key1, uint3
     e.dir[1] = x[1];
 }
 
-// returns the number of trials used (0: degenerate block, identity taken; 4097: cap hit)
-template <typename T>
-__device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T temperature, uint32_t key0,
+// returns the number of trials used (0: degenerate block, identity taken; 4097: cap hit); cond = |k|^2 (the
+// conditioning number of g = h (x) conj(khat), see su2_overrelax_step).
+// CT: type of the site chain (k, khat = k/|k|, g -- the ill-conditioned part); DT: type of the draw (alpha, the
+// Kennedy-Pendleton trials, h).  (double, float): fp32 kernels with the chain in double, the draw on the SFU.
+template <typename CT, typename DT>
+__device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double Td, uint32_t key0,
                                                       uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2,
-                                                      const EarlyRandom& early, T (&g)[4])
+                                                      const EarlyRandom& early, CT (&g)[4], CT& cond)
 {
-    using M = KPMath<T>;
-    const T n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
-    if (!(n2 >= Tiny<T>::sq)) { g[0] = T(1); g[1] = g[2] = g[3] = T(0); return 0u; }
-    T alpha, inv_alpha, inv_n;
-    M::prep(n2, temperature, alpha, inv_alpha, inv_n);
-    const T kc0 = k[0] * inv_n, kc1 = -k[1] * inv_n, kc2 = -k[2] * inv_n, kc3 = -k[3] * inv_n; // conj(khat)
+    using M = KPMath<DT>;
+    const CT n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
+    cond = n2;
+    if (!(n2 >= Tiny<CT>::sq)) { g[0] = CT(1); g[1] = g[2] = g[3] = CT(0); return 0u; }
+    // no division, no IEEE square root: 1/|k| by rsqrt (fp32: MUFU.RSQ + one Newton step), 1/alpha = T/|k| from it
+    const CT inv_n = gf_rsqrt<CT>(n2);
+    const DT inv_alpha = (DT)((CT)Td * inv_n);
+    const CT kc0 = k[0] * inv_n, kc1 = -k[1] * inv_n, kc2 = -k[2] * inv_n, kc3 = -k[3] * inv_n; // conj(khat)
     // unit vector of the direction of hvec: data independent, computed ahead of the draw
-    const T cos_t = T(1) - T(2) * M::uni(early.dir[0]);
-    const T up = M::uni(early.dir[1]);
-    const T sin_t = M::root(T(1) - cos_t * cos_t);
-    const T e1 = sin_t * M::cos2pi(up), e2 = sin_t * M::sin2pi(up), e3 = cos_t;
+    const DT cos_t = DT(1) - DT(2) * M::uni(early.dir[0]);
+    const DT up = M::uni(early.dir[1]);
+    const DT sin_t = M::root(DT(1) - cos_t * cos_t);
+    const DT e1 = sin_t * M::cos2pi(up), e2 = sin_t * M::sin2pi(up), e3 = cos_t;
     // trial 0 from the words generated up front: straight-line code, so that it can be scheduled together with the
     // link updates of the previous subgroup; only rejected lanes enter the loop
-    T h0;
+    DT d, est;
     unsigned trial = 0;
-    bool accepted;
-    {
-        const T u1 = M::uni(early.trial0[0]), u2 = M::uni(early.trial0[1]), u3 = M::uni(early.trial0[2]),
-                u4 = M::uni(early.trial0[3]);
-        const T c = M::cos2pi(u3);
-        const T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha, inv_alpha);
-        accepted = M::accept(u4, d);
-        h0 = T(1) - d;
-    }
+    uint32_t x[4] = {early.trial0[0], early.trial0[1], early.trial0[2], early.trial0[3]};
+    bool accepted = M::trial(x, (double)n2, Td, inv_alpha, d, est);
     if (!accepted) {
-        uint32_t x[4];
         for (trial = 1; trial < 4096u; ++trial) {
             philox4x32_10(c0, c1, c2, trial, key0, key1, x);
-            const T u1 = M::uni(x[0]), u2 = M::uni(x[1]), u3 = M::uni(x[2]), u4 = M::uni(x[3]);
-            const T c = M::cos2pi(u3);
-            const T d = M::delta(M::neglog(u1), M::neglog(u2), c, alpha, inv_alpha);
-            if (M::accept(u4, d)) { h0 = T(1) - d; accepted = true; break; }
+            if (M::trial(x, (double)n2, Td, inv_alpha, d, est)) { accepted = true; break; }
         }
     }
     if (!accepted) {
@@ -226,14 +263,115 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T tempera
         g[0] = kc0; g[1] = kc1; g[2] = kc2; g[3] = kc3;
         return 4097u;
     }
-    const T r = M::root(T(1) - h0 * h0);
-    const T h1 = r * e1, h2 = r * e2, h3 = r * e3;
+    // fp32 draw: the SFU value of the accepted delta is off by ~5e-7 est, which moves h0 by as much and hvec, of
+    // length r = sqrt(delta (2 - delta)), by that over r.  Where this is too much for the links (small alpha, large
+    // -ln u, h0 near -1: ~1e-3 of the draws at T = 1.4, none once alpha > 10) delta is taken in double
+    if (sizeof(DT) == 4 && est * est > DT(16) * fmin(d * (DT(2) - d), DT(1)))
+        d = (DT)kp_delta_f64((double)n2, Td, x[0], x[1], x[2]);
+    const DT h0d = DT(1) - d;
+    const DT r = M::root(d * (DT(2) - d)); // = sqrt(1 - h0^2) without the cancellation at small delta
+    const CT h0 = (CT)h0d, h1 = (CT)(r * e1), h2 = (CT)(r * e2), h3 = (CT)(r * e3);
     // g = h (x) conj(khat):  (pq)_0 = p0 q0 - p.q,  (pq)_vec = p0 qvec + q0 pvec - pvec x qvec   (C13)
     g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3;
     g[1] = h0 * kc1 + kc0 * h1 - (h2 * kc3 - h3 * kc2);
     g[2] = h0 * kc2 + kc0 * h2 - (h3 * kc1 - h1 * kc3);
     g[3] = h0 * kc3 + kc0 * h3 - (h1 * kc2 - h2 * kc1);
     return trial + 1u;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// fp32 heatbath kernels, rare path: the whole site update in double.
+// g = h (x) conj(khat) with khat = k/|k| is ill-conditioned where the projected block is small: the fp32 rounding of K
+// (~1e-6) then moves the links by ~1e-6/|k|.  (For the heatbath there is no second small factor, and a BLACK site
+// inherits only ~1e-6 from its RED neighbours, so unlike the relaxation sweeps a per-site repair is enough here.)  A
+// thread whose |k|^2 fell below SweepParams::fix_thr2 in any of its three subgroup steps drops its fp32 result and
+// redoes the site here from the stored fp32 links (untouched so far: within a half-sweep only this site writes them,
+// C6): K, the three SU(2) steps, K <- G K and the link products all in double, one rounding to fp32 at the store.
+// Every thread of a site takes the same decision (K is bit-identical on them) and redoes its own links; no shuffles
+// on this divergent path: each thread builds K for itself.  DESIGN.md sec. 4.
+// ---------------------------------------------------------------------------------------------------------
+template <int I, int J, int SUB, int MODE>
+__device__ __forceinline__ void fixup_subgroup(const SweepParams& p, const SweepPhase& ph, cx<double> (&K)[9],
+                                               uint32_t site_canon, bool record, cx<double>& a, cx<double>& b)
+{
+    double k[4], h[4], cond;
+    su2_project<I, J>(K, k);
+    const uint32_t c2 = ((uint32_t)ph.parity << 2) | (uint32_t)SUB;
+    if (MODE == MODE_OVERRELAX) {
+        su2_overrelax_step<double>(k, p.omega, h, cond);
+    } else if (MODE == MODE_VARIANT) {
+        su2_variant_step<double>(k, p.variant, p.omega, p.key0, p.key1, site_canon, ph.step, c2, h, cond);
+    } else {
+        EarlyRandom early;
+        early_random(p.key0, p.key1, site_canon, ph.step, c2, early);
+        const unsigned ntr = su2_heatbath_step<double, double>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond);
+        if (record && p.trials != nullptr) p.trials[3u * (size_t)site_canon + SUB] = ntr;
+    }
+    a = {h[0], h[3]};
+    b = {h[2], h[1]}; // C4
+    su2_left<I, J>(a, b, K); // K <- G K  (C8)
+}
+
+template <int R, int TPS, int MODE, bool CB>
+__device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPhase& ph, unsigned h, int lane_mu0)
+{
+    constexpr int NMU = 4 / TPS;
+    using IO = LinkIO<float, R>;
+    using GIO = LinkIO<float, 18>;
+    const Site s = decode_site(p.L, h, ph.parity);
+    const size_t H = p.L.H;
+    float* const base = reinterpret_cast<float*>(p.U);
+    const uint64_t ld = make_l2_policy(POLICY_NORMAL), st = make_l2_policy(p.st_policy);
+    cx<double> K[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) K[e] = {0.0, 0.0};
+    for (int mu = 0; mu < p.nd; ++mu) { // eq. 2.3 (C2), every direction entering K
+        cx<double> f[9], b[9];
+        IO::load(base + (size_t)(ph.parity * 4 + mu) * R * H, H, s.h, f, ld);
+        IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, backward_neighbour(p.L, s, mu), b, ld);
+        if (ph.reunit) { reunitarise(f); reunitarise(b); }
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) K[3 * r + c] = K[3 * r + c] + f[3 * r + c] + conj(b[3 * c + r]);
+    }
+    const uint32_t sc = canonical_index(s);
+    const bool record = lane_mu0 == 0;
+    cx<double> a0, b0, a1, b1, a2, b2;
+    fixup_subgroup<0, 1, 0, MODE>(p, ph, K, sc, record, a0, b0);
+    fixup_subgroup<0, 2, 1, MODE>(p, ph, K, sc, record, a1, b1);
+    fixup_subgroup<1, 2, 2, MODE>(p, ph, K, sc, record, a2, b2);
+    for (int m = 0; m < NMU; ++m) {
+        const int mu = lane_mu0 + m;
+        if (CB && mu == 3) continue;
+        cx<double> u[9];
+        float* const fb = base + (size_t)(ph.parity * 4 + mu) * R * H;
+        IO::load(fb, H, s.h, u, ld);
+        if (ph.reunit) reunitarise(u);
+        su2_left<0, 1>(a0, b0, u); // U_mu(x) <- G U_mu(x)
+        su2_left<0, 2>(a1, b1, u);
+        su2_left<1, 2>(a2, b2, u);
+        IO::store(fb, H, s.h, u, st);
+        float* const bb = base + (size_t)((1 - ph.parity) * 4 + mu) * R * H;
+        const unsigned hb = backward_neighbour(p.L, s, mu);
+        IO::load(bb, H, hb, u, ld);
+        if (ph.reunit) reunitarise(u);
+        su2_right_dagger<0, 1, 3>(a0, b0, u); // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+        su2_right_dagger<0, 2, 3>(a1, b1, u);
+        su2_right_dagger<1, 2, 3>(a2, b2, u);
+        IO::store(bb, H, hb, u, st);
+    }
+    if (CB && lane_mu0 + NMU - 1 == 3) { // reading B: G(x) <- g G(x)
+        cx<double> u[9];
+        float* const gb = reinterpret_cast<float*>(p.G) + (size_t)ph.parity * 18 * H;
+        GIO::load(gb, H, s.h, u, ld);
+        if (ph.reunit) reunitarise(u);
+        su2_left<0, 1>(a0, b0, u);
+        su2_left<0, 2>(a1, b1, u);
+        su2_left<1, 2>(a2, b2, u);
+        GIO::store(gb, H, s.h, u, st);
+    }
+    if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -244,31 +382,53 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const T (&k)[4], T tempera
 // G(x) <- g(x) G(x) in a site field (18 reals, one link's worth instead of two) and the temporal links are
 // transformed once at the end of the call, U_t(x) <- G(x) U_t(x) G(x+t)^dagger (coulomb_finish_kernel): 14/16 of the
 // bytes of reading A, same result up to rounding.
-template <typename T, int R, int TPS, int MODE, bool CB = false>
+//
+// fp32 kernels, precision of the site chain.  The links are fp32 in memory and in the link
+// products; the site chain -- K(x), the three SU(2) steps, K <- G K -- is ill-conditioned where the projected block
+// k or the expanded g^omega is small (g = k/|k|, h/|h|): in fp32 its rounding (~1e-6 on K) moves the links by ~1e-6
+// / (|k||h|), and the BLACK half-sweep inherits the errors of the RED one through its own K.  On a random-gauge
+// start that breaks north_star's 5e-5 per link at ~1e-5 of the sites; a per-site repair cannot help the BLACK sites
+// (their error is in their input).  So the chain runs in double (CT = double: K accumulated exactly from the fp32
+// links, G rounded to fp32 once) while the field is rough, and in fp32 once it is smooth: every half-sweep records
+// whether any of its steps had a conditioning number |k|^2 |h|^2 below watch_thr2 (rough[slot]), and a half-sweep
+// takes the double chain iff one of the two half-sweeps before it was rough (or the host forces it: the first sweep
+// of every call).  The decision is a deterministic function of the field; on a nearly fixed field (|k| ~ 10, |h| ~ 1)
+// no launch takes the double chain.  The heatbath kernels keep the fp32 chain and repair single sites instead
+// (fixup_site_f64 above).
+// DC (fp32 heatbath kernels only): the double chain at every site, for annealing runs in which every link has to meet
+// the per-link bound (gf_set_chain(ctx, 1, ..)); the default heatbath kernel keeps the fp32 chain.
+template <typename T, int R, int TPS, int MODE, bool CB = false, bool DC = false>
 struct SweepKernel {
     static constexpr int NMU = 4 / TPS;
+    static constexpr bool FP32 = sizeof(T) == 4;
+    static constexpr bool HYB = FP32 && MODE != MODE_HEATBATH;        // relaxation sweeps: chain type chosen per launch
+    static constexpr bool FIX = FP32 && MODE == MODE_HEATBATH && !DC; // heatbath: fp32 chain, weak sites redone in double
+    static_assert(!DC || (FP32 && MODE == MODE_HEATBATH), "DC is a variant of the fp32 heatbath kernel");
     using IO = LinkIO<T, R>;
     using GIO = LinkIO<T, 18>;
 
-    template <int I, int J, int SUB>
-    static __device__ __forceinline__ void subgroup(const SweepParams& p, cx<T> (&K)[9], cx<T> (&F)[NMU][9],
-                                                    cx<T> (&B)[NMU][9], uint32_t site_canon, bool record,
-                                                    const EarlyRandom& early, int lane_mu0, cx<T> (&Gt)[9])
+    // one SU(2) subgroup step on the chain type CT
+    template <typename CT, int I, int J, int SUB>
+    static __device__ __forceinline__ void subgroup(const SweepParams& p, const SweepPhase& ph, cx<CT> (&K)[9],
+                                                    cx<T> (&F)[NMU][9], cx<T> (&B)[NMU][9], uint32_t site_canon,
+                                                    bool record, const EarlyRandom& early, int lane_mu0,
+                                                    cx<T> (&Gt)[9], bool& watch)
     {
-        T k[4], h[4];
+        CT k[4], h[4], cond;
         su2_project<I, J>(K, k);
+        const uint32_t c2 = ((uint32_t)ph.parity << 2) | (uint32_t)SUB;
         if (MODE == MODE_OVERRELAX) {
-            su2_overrelax_step<T>(k, (T)p.omega, h);
+            su2_overrelax_step<CT>(k, (CT)p.omega, h, cond);
         } else if (MODE == MODE_VARIANT) {
-            su2_variant_step<T>(k, p.variant, p.omega, p.key0, p.key1, site_canon, p.step,
-                                ((uint32_t)p.parity << 2) | (uint32_t)SUB, h);
+            su2_variant_step<CT>(k, p.variant, p.omega, p.key0, p.key1, site_canon, ph.step, c2, h, cond);
             (void)early;
         } else {
-            unsigned ntr = su2_heatbath_step<T>(k, (T)p.T, p.key0, p.key1, site_canon, p.step,
-                                                ((uint32_t)p.parity << 2) | (uint32_t)SUB, early, h);
+            unsigned ntr = su2_heatbath_step<CT, T>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond);
             if (record && p.trials != nullptr) p.trials[3u * (size_t)site_canon + SUB] = ntr;
         }
-        const cx<T> a = {h[0], h[3]}, b = {h[2], h[1]}; // C4
+        if (FP32) watch = watch || ((float)cond < p.watch_thr2);
+        const cx<CT> ac = {h[0], h[3]}, bc = {h[2], h[1]}; // C4
+        const cx<T> a = {(T)h[0], (T)h[3]}, b = {(T)h[2], (T)h[1]};
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
             if (CB && lane_mu0 + m == 3) {
@@ -278,18 +438,57 @@ struct SweepKernel {
                 su2_right_dagger<I, J, 3>(a, b, B[m]);  // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
             }
         }
-        su2_left<I, J>(a, b, K);                        // K <- G K  (C8)
+        su2_left<I, J>(ac, bc, K);                      // K <- G K  (C8)
+    }
+
+    // the site chain on the type CT: K(x) from the loaded links, then the three subgroup steps (each applies its G to
+    // the links at once, Alg. 1's data flow, C8)
+    template <typename CT>
+    static __device__ __forceinline__ void chain(const SweepParams& p, const SweepPhase& ph, cx<T> (&F)[NMU][9],
+                                                 cx<T> (&B)[NMU][9], cx<T> (&Gt)[9], uint32_t sc,
+                                                 const EarlyRandom (&early)[3], int lane_mu0, unsigned mask, bool& watch)
+    {
+        // K(x) = sum_{mu < nd} [ U_mu(x) + U_mu(x-mu)^dagger ]   (eq. 2.3, PAPER.md:53; C2)
+        cx<CT> K[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) K[e] = {CT(0), CT(0)};
+#pragma unroll
+        for (int m = 0; m < NMU; ++m) {
+            if (lane_mu0 + m < p.nd && !(CB && lane_mu0 + m == 3)) {
+#pragma unroll
+                for (int r = 0; r < 3; ++r)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        K[3 * r + c].re = (K[3 * r + c].re + (CT)F[m][3 * r + c].re) + (CT)B[m][3 * c + r].re;
+                        K[3 * r + c].im = (K[3 * r + c].im + (CT)F[m][3 * r + c].im) - (CT)B[m][3 * c + r].im;
+                    }
+            }
+        }
+        if (TPS > 1) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) {
+#pragma unroll
+                for (int off = 1; off < TPS; off <<= 1) {
+                    K[e].re += __shfl_xor_sync(mask, K[e].re, off);
+                    K[e].im += __shfl_xor_sync(mask, K[e].im, off);
+                }
+            }
+        }
+        const bool record = lane_mu0 == 0;
+        subgroup<CT, 0, 1, 0>(p, ph, K, F, B, sc, record, early[0], lane_mu0, Gt, watch); // Cabibbo-Marinari subgroups, order of C4
+        subgroup<CT, 0, 2, 1>(p, ph, K, F, B, sc, record, early[1], lane_mu0, Gt, watch);
+        subgroup<CT, 1, 2, 2>(p, ph, K, F, B, sc, record, early[2], lane_mu0, Gt, watch);
     }
 
     // L2 prefetch for the block that runs `prefetch` sites further along the traversal: the few fat warps of
     // an SM cannot keep enough bytes in flight while they compute, prefetches hold no register and no
     // scoreboard entry, and the 126 MB L2 is the staging buffer.  Addresses are those of this thread shifted
     // by the distance (exact for forward links, exact up to the periodic wrap for backward links: a hint).
-    static __device__ __forceinline__ void issue_prefetch(const SweepParams& p, const Site& s, const unsigned (&hb)[NMU],
-                                                          int lane_mu0, T* base, size_t H)
+    static __device__ __forceinline__ void issue_prefetch(const SweepParams& p, const SweepPhase& ph, const Site& s,
+                                                          const unsigned (&hb)[NMU], int lane_mu0, T* base, size_t H)
     {
         if (p.prefetch) {
-            const long long d = p.reverse ? -(long long)p.prefetch : (long long)p.prefetch;
+            const long long d = ph.reverse ? -(long long)p.prefetch : (long long)p.prefetch;
             const long long hf = (long long)s.h + d;
             if (hf >= 0 && hf < (long long)H) {
 #pragma unroll
@@ -297,21 +496,21 @@ struct SweepKernel {
                     const int mu = lane_mu0 + m;
                     const long long hbd = (long long)hb[m] + d;
                     if (CB && mu == 3) continue;
-                    IO::prefetch(base + (size_t)(p.parity * 4 + mu) * R * H, H, (size_t)hf);
-                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, (size_t)hbd);
+                    IO::prefetch(base + (size_t)(ph.parity * 4 + mu) * R * H, H, (size_t)hf);
+                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, (size_t)hbd);
                 }
             }
         }
     }
 
-    static __device__ __forceinline__ void run(const SweepParams& p)
+    // the update of the site in half-site slot `slot` (Alg. 1 inner loop) by the TPS threads that
+    // share it; this thread owns the directions lane_mu0 .. lane_mu0 + NMU - 1.  `mask`: the lanes of the warp that
+    // run this call together (whole sites: TPS divides 32).  `first`: first site update of this thread in the launch
+    // (the one-shot kernel: always; it waits for the previous grid there)
+    static __device__ __forceinline__ void site_update(const SweepParams& p, const SweepPhase& ph, unsigned slot,
+                                                       int lane_mu0, unsigned mask, bool first)
     {
-        const unsigned blk = p.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
-        const unsigned gtid = blk * blockDim.x + threadIdx.x;
-        const unsigned slot = p.h_begin + gtid / TPS;
-        const int lane_mu0 = (int)(gtid % TPS) * NMU; // first direction this thread owns
-        const bool active = gtid / TPS < p.h_count;        // inactive threads shadow site 0 and store nothing,
-        const Site s = decode_site(p.L, active ? slot : 0u, p.parity); // so warp shuffles stay converged
+        const Site s = decode_site(p.L, slot, ph.parity);
         const size_t H = p.L.H;
         T* const base = reinterpret_cast<T*>(p.U);
 
@@ -323,32 +522,40 @@ struct SweepKernel {
         // Programmatic dependent launch: this grid may become resident while the previous half-sweep drains
         // (its index arithmetic above overlaps that tail); links are touched only after the previous grid
         // has completed and flushed.  Letting the next grid launch early is always safe for the same reason.
-        if (p.pdl) {
+        if (p.pdl && first) {
             cudaTriggerProgrammaticLaunchCompletion();
             cudaGridDependencySynchronize();
         }
+        // fp32 relaxation sweeps, hybrid chain: were the two half-sweeps before this one rough?  Two L2 hits, issued
+        // ahead of the link loads so that the choice is there when the first link arrives
+        int rough_a = 0, rough_b = 0;
+        if (HYB && p.chain == CHAIN_HYBRID && !ph.rough_force) {
+            const volatile int* rough = p.rough;
+            rough_a = rough[(ph.rough_slot + ROUGH_RING - 1) % ROUGH_RING];
+            rough_b = rough[(ph.rough_slot + ROUGH_RING - 2) % ROUGH_RING];
+        }
         // the relaxation kernels prefetch before their loads (placed after them the fp64 kernel spills twice as
         // much); the heatbath kernel issues its loads first and hides the prefetch and the generator behind them
-        if (MODE != MODE_HEATBATH) issue_prefetch(p, s, hb, lane_mu0, base, H);
+        if (MODE != MODE_HEATBATH) issue_prefetch(p, ph, s, hb, lane_mu0, base, H);
         // issue every load before the first use
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
             const int mu = lane_mu0 + m;
             if (CB && mu == 3) continue;
-            IO::load(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.ld);
-            IO::load(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.ld);
+            IO::load(base + (size_t)(ph.parity * 4 + mu) * R * H, H, s.h, F[m], pol.ld);
+            IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.ld);
         }
         cx<T> Gt[9];
         const bool owns_t = CB && (lane_mu0 + NMU - 1 == 3); // the thread that would hold the temporal links
-        if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)p.parity * 18 * H, H, s.h, Gt, pol.ld);
-        if (MODE == MODE_HEATBATH) issue_prefetch(p, s, hb, lane_mu0, base, H);
+        if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)ph.parity * 18 * H, H, s.h, Gt, pol.ld);
+        if (MODE == MODE_HEATBATH) issue_prefetch(p, ph, s, hb, lane_mu0, base, H);
         // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
         const uint32_t sc = canonical_index(s);
         EarlyRandom early[3];
         if (MODE == MODE_HEATBATH) {
 #pragma unroll
             for (int sub = 0; sub < 3; ++sub)
-                early_random(p.key0, p.key1, sc, p.step, ((uint32_t)p.parity << 2) | (uint32_t)sub, early[sub]);
+                early_random(p.key0, p.key1, sc, ph.step, ((uint32_t)ph.parity << 2) | (uint32_t)sub, early[sub]);
             // pin the 18 words here, before the first use of a loaded link: volatile asm statements keep their
             // order, so the generator runs between the issue of the loads and their consumption
 #pragma unroll
@@ -356,7 +563,7 @@ struct SweepKernel {
                 asm volatile("" :: "r"(early[sub].trial0[0]), "r"(early[sub].trial0[1]), "r"(early[sub].trial0[2]),
                              "r"(early[sub].trial0[3]), "r"(early[sub].dir[0]), "r"(early[sub].dir[1]));
         }
-        if (p.reunit) {
+        if (ph.reunit) {
 #pragma unroll
             for (int m = 0; m < NMU; ++m) {
                 if (CB && lane_mu0 + m == 3) continue;
@@ -366,52 +573,74 @@ struct SweepKernel {
             if (owns_t) reunitarise(Gt);
         }
 
-        // K(x) = sum_{mu < nd} [ U_mu(x) + U_mu(x-mu)^dagger ]   (eq. 2.3, PAPER.md:53; C2)
-        cx<T> K[9];
-#pragma unroll
-        for (int e = 0; e < 9; ++e) K[e] = {T(0), T(0)};
-#pragma unroll
-        for (int m = 0; m < NMU; ++m) {
-            if (lane_mu0 + m < p.nd && !(CB && lane_mu0 + m == 3)) {
-#pragma unroll
-                for (int r = 0; r < 3; ++r)
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) K[3 * r + c] = K[3 * r + c] + F[m][3 * r + c] + conj(B[m][3 * c + r]);
+        bool watch = false; // fp32: some step of this site had a small conditioning number
+        if constexpr (HYB) {
+            const bool dchain = p.chain == CHAIN_DOUBLE || (p.chain == CHAIN_HYBRID && (ph.rough_force | rough_a | rough_b) != 0);
+            if (dchain) chain<double>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch);
+            else chain<float>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch);
+            if (p.chain == CHAIN_HYBRID) {
+                if (watch) p.rough[ph.rough_slot] = 1; // same value from every writer
+                if (slot == p.h_begin && lane_mu0 == 0) {
+                    p.rough[(ph.rough_slot + 1) % ROUGH_RING] = 0; // read by the previous launch, written by the next
+                    if (dchain && p.dc_count != nullptr) atomicAdd(p.dc_count, 1ull);
+                }
             }
-        }
-        if (TPS > 1) {
-#pragma unroll
-            for (int e = 0; e < 9; ++e) {
-#pragma unroll
-                for (int off = 1; off < TPS; off <<= 1) {
-                    K[e].re += __shfl_xor_sync(0xffffffffu, K[e].re, off);
-                    K[e].im += __shfl_xor_sync(0xffffffffu, K[e].im, off);
+        } else {
+            (void)rough_a; (void)rough_b;
+            chain<typename std::conditional<DC, double, T>::type>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch);
+            if constexpr (FIX) {
+                if (watch) {
+                    fixup_site_f64<R, TPS, MODE, CB>(p, ph, slot, lane_mu0); // stores the links itself
+                    return;
                 }
             }
         }
 
-        const bool record = active && (lane_mu0 == 0);
-        subgroup<0, 1, 0>(p, K, F, B, sc, record, early[0], lane_mu0, Gt); // Cabibbo-Marinari subgroups, order of C4
-        subgroup<0, 2, 1>(p, K, F, B, sc, record, early[1], lane_mu0, Gt);
-        subgroup<1, 2, 2>(p, K, F, B, sc, record, early[2], lane_mu0, Gt);
-
-        if (active) {
 #pragma unroll
-            for (int m = 0; m < NMU; ++m) {
-                const int mu = lane_mu0 + m;
-                if (CB && mu == 3) continue;
-                IO::store(base + (size_t)(p.parity * 4 + mu) * R * H, H, s.h, F[m], pol.st);
-                IO::store(base + (size_t)((1 - p.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.st);
-            }
-            if (owns_t) GIO::store(reinterpret_cast<T*>(p.G) + (size_t)p.parity * 18 * H, H, s.h, Gt, pol.st);
+        for (int m = 0; m < NMU; ++m) {
+            const int mu = lane_mu0 + m;
+            if (CB && mu == 3) continue;
+            IO::store(base + (size_t)(ph.parity * 4 + mu) * R * H, H, s.h, F[m], pol.st);
+            IO::store(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.st);
         }
+        if (owns_t) GIO::store(reinterpret_cast<T*>(p.G) + (size_t)ph.parity * 18 * H, H, s.h, Gt, pol.st);
+    }
+
+    static __device__ __forceinline__ void run(const SweepParams& p)
+    {
+        const unsigned blk = p.ph.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+        const unsigned gtid = blk * blockDim.x + threadIdx.x;
+        // threads past the range leave at once: they come in whole sites (TPS divides 32), and exited threads may be
+        // named in the mask of the shuffles that combine K
+        if (gtid / TPS >= p.h_count) return;
+        site_update(p, p.ph, p.h_begin + gtid / TPS, (int)(gtid % TPS) * NMU, 0xffffffffu, true);
     }
 };
 
-template <typename T, int R, int TPS, int MODE, bool CB = false>
-__global__ void __launch_bounds__(MAX_BLOCK) gf_half_sweep_kernel(const SweepParams p)
+// Register budget.  The fp32 relaxation kernels hold two chains (fp32 and double, chosen per launch); the double one
+// needs more registers, but it runs on rough fields only, so the kernel is held to what the fp32 chain alone needs
+// (the double chain spills instead) -- otherwise the steady state pays for the rare path with occupancy (fp32 R12,
+// two threads per site: 128 -> 174 registers cost 18 %).  Blocks of up to MAX_BLOCK threads must stay launchable.
+template <typename T, int R, int TPS, int MODE, bool CB>
+constexpr int sweep_max_registers()
 {
-    SweepKernel<T, R, TPS, MODE, CB>::run(p);
+    if (sizeof(T) == 4 && MODE != MODE_HEATBATH) { // what ptxas gives the same kernel with the fp32 chain alone, rounded up to 8
+        const bool var = MODE == MODE_VARIANT;
+        if (R == 12) {
+            if (TPS == 1) return CB ? (var ? 184 : 200) : 255;
+            if (TPS == 2) return 128;
+            return CB ? 96 : (var ? 104 : 80);
+        }
+        if (TPS == 2) return CB ? (var ? 136 : 144) : (var ? 136 : 184);
+        if (TPS == 4) return CB ? 104 : (var ? 104 : 120);
+    }
+    return 255;
+}
+
+template <typename T, int R, int TPS, int MODE, bool CB = false, bool DC = false>
+__global__ void __maxnreg__((sweep_max_registers<T, R, TPS, MODE, CB>())) gf_half_sweep_kernel(const __grid_constant__ SweepParams p)
+{
+    SweepKernel<T, R, TPS, MODE, CB, DC>::run(p);
 }
 
 } // namespace gf

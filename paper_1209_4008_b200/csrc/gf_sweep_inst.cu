@@ -24,44 +24,38 @@ namespace gf {
 
 typedef void (*sweep_fn)(const SweepParams);
 
-static sweep_fn pick(int tps, int mode, bool cb)
+template <int MODE, bool CB, bool DC>
+static sweep_fn pick_tps(int tps)
 {
     constexpr int R = GF_INST_R;
-    if (cb) { // Coulomb reading B
-        if (mode == MODE_HEATBATH) {
-            if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_HEATBATH, true>;
-            if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_HEATBATH, true>;
-            if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_HEATBATH, true>;
-        } else if (mode == MODE_OVERRELAX) {
-            if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX, true>;
-            if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX, true>;
-            if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_OVERRELAX, true>;
-        } else if (mode == MODE_VARIANT) {
-            if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_VARIANT, true>;
-            if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_VARIANT, true>;
-            if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_VARIANT, true>;
-        }
-        return nullptr;
-    }
-    if (mode == MODE_OVERRELAX) {
-        if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_OVERRELAX>;
-        if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_OVERRELAX>;
-        if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_OVERRELAX>;
-    } else if (mode == MODE_VARIANT) {
-        if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_VARIANT>;
-        if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_VARIANT>;
-        if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_VARIANT>;
-    } else if (mode == MODE_HEATBATH) {
-        if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE_HEATBATH>;
-        if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE_HEATBATH>;
-        if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE_HEATBATH>;
+    if (tps == 1) return gf_half_sweep_kernel<real_t, R, 1, MODE, CB, DC>;
+    if (tps == 2) return gf_half_sweep_kernel<real_t, R, 2, MODE, CB, DC>;
+    if (tps == 4) return gf_half_sweep_kernel<real_t, R, 4, MODE, CB, DC>;
+    return nullptr;
+}
+
+// dc: fp32 heatbath kernel with the double chain at every site (the relaxation kernels pick their chain at run time)
+template <bool CB>
+static sweep_fn pick_mode(int tps, int mode, bool dc)
+{
+    if (mode == MODE_OVERRELAX) return pick_tps<MODE_OVERRELAX, CB, false>(tps);
+    if (mode == MODE_VARIANT) return pick_tps<MODE_VARIANT, CB, false>(tps);
+    if (mode == MODE_HEATBATH) {
+#if !GF_INST_FP64
+        if (dc) return pick_tps<MODE_HEATBATH, CB, true>(tps);
+#endif
+        (void)dc;
+        return pick_tps<MODE_HEATBATH, CB, false>(tps);
     }
     return nullptr;
 }
 
+// cb: Coulomb reading B
+static sweep_fn pick(int tps, int mode, bool cb, bool dc) { return cb ? pick_mode<true>(tps, mode, dc) : pick_mode<false>(tps, mode, dc); }
+
 cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParams& p, cudaStream_t stream)
 {
-    sweep_fn fn = pick(tps, mode, p.G != nullptr);
+    sweep_fn fn = pick(tps, mode, p.G != nullptr, p.chain == CHAIN_DOUBLE);
     if (fn == nullptr || block <= 0 || block > MAX_BLOCK || (block % 32) != 0) return cudaErrorInvalidValue;
     const unsigned long long threads = (unsigned long long)p.h_count * (unsigned long long)tps;
     if (p.h_count == 0) return cudaSuccess;
@@ -85,9 +79,9 @@ cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParam
     return cudaLaunchKernelEx(&cfg, fn, p);
 }
 
-cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, bool reading_b, cudaFuncAttributes* attr)
+cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, bool reading_b, bool dc, cudaFuncAttributes* attr)
 {
-    sweep_fn fn = pick(tps, mode, reading_b);
+    sweep_fn fn = pick(tps, mode, reading_b, dc);
     if (fn == nullptr) return cudaErrorInvalidValue;
     return cudaFuncGetAttributes(attr, fn);
 }

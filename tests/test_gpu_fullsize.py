@@ -66,6 +66,24 @@ def test_config3_32x4_every_link_and_F_theta(gfm, field32, oracle32, precision, 
     fx.close()
 
 
+@pytest.mark.parametrize("seed", [11, 12, 13])
+@pytest.mark.parametrize("omega", [1.7, 1.8])
+def test_32x4_fp32_every_link_more_seeds(gfm, seed, omega):
+    """the fp32 per-link bound on every link of further random-gauge starts, both storage formats (the tail of the
+    error distribution is what the bound is about: 3 seeds x 2 omega x 1 048 576 sites x 2 formats)"""
+    dims = (32, 32, 32, 32)
+    U = gf_inputs.smooth_random(dims, 0.4, seed)
+    ref = U.copy()
+    oracle.overrelax(ref, dims, omega, 1)
+    for R in (18, 12):
+        fx = gfm.GaugeFixer(dims, precision="fp32", reals_per_link=R)
+        fx.load(U)
+        fx.overrelax(omega, 1)
+        err = np.abs(fx.download() - ref).max()
+        fx.close()
+        assert err <= TOL_LINK["fp32"], (R, err)
+
+
 @pytest.fixture(scope="module")
 def oracle32_500(field32):
     """the headline config run to its end by the oracle: 500 sweeps at omega = 1.7 (about 40 s on 16 cores)"""
@@ -96,9 +114,9 @@ def _tiled_device(U, gdims):
     return t.view(Nt, Nz, Ny, Nx, 72).repeat(2, 2, 2, 2, 1).contiguous().view(-1)
 
 
-def _check_tiles(canon_dev, gdims, ref, tol, tail=0.0, tail_tol=None):
-    """canon_dev: device float64 canonical field of the doubled lattice; every tile equal, tile 0 close to ref.
-    tail > 0: that fraction of the sites may exceed tol (but not tail_tol) -- fp32 only, see the caller."""
+def _check_tiles(canon_dev, gdims, ref, tol):
+    """canon_dev: device float64 canonical field of the doubled lattice; every tile equal, every link of tile 0 within
+    tol of ref"""
     import torch
 
     Nx, Ny, Nz, Nt = gdims
@@ -110,11 +128,8 @@ def _check_tiles(canon_dev, gdims, ref, tol, tail=0.0, tail_tol=None):
                 for d in range(2):
                     assert torch.equal(v[a, :, b, :, c, :, d, :, :], first), (a, b, c, d)
     got = first.contiguous().cpu().numpy().view("complex128").reshape(-1, 4, 3, 3)
-    err = np.abs(got - ref).reshape(len(ref), -1).max(axis=1)
-    if tail == 0.0:
-        assert err.max() <= tol
-    else:
-        assert (err > tol).mean() <= tail and err.max() <= tail_tol, ((err > tol).sum(), err.max())
+    err = np.abs(got - ref)
+    assert err.max() <= tol, (err.max(), int((err.reshape(len(ref), -1).max(axis=1) > tol).sum()))
 
 
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
@@ -130,21 +145,17 @@ def test_config4_64x4_tiles_and_oracle(gfm, precision):
     gfm.gf_unpack(fx.ctx, fx.U, canon)
     torch.cuda.synchronize()
     oracle.overrelax(U, gdims, 1.8, 1)
-    # The stated per-link tolerance is for ONE sweep.  fp64: every link.  fp32: the maximiser g = k/|k| is
-    # ill-conditioned where the projected block is small (error ~ 1e-6/|k|), and on a random-gauge start |k| < 0.1
-    # happens at a handful of the 3.1e6 (site, subgroup) steps of this lattice: every link of
-    # config 3 (omega 1.7, seed 3) is inside 5e-5 (test above); here (omega 1.8, seed 4) 7 sites of 1 048 576 reach
-    # 6.3e-5, so the bar is: at most 2e-5 of the sites above 5e-5, none above 2e-4.
-    if precision == "fp64":
-        _check_tiles(canon, gdims, U, TOL_LINK[precision])
-    else:
-        _check_tiles(canon, gdims, U, TOL_LINK[precision], tail=2e-5, tail_tol=2e-4)
+    # The stated per-link tolerance is for ONE sweep, on EVERY link: 1e-12 (fp64), 5e-5 (fp32).  In fp32 the site chain
+    # runs in double on this random-gauge start (hybrid chain); with an fp32 chain 7 sites of
+    # 1 048 576 reached 6.3e-5 here (omega 1.8, seed 4).
+    _check_tiles(canon, gdims, U, TOL_LINK[precision])
     fx.overrelax(1.8, 1)
     gfm.gf_unpack(fx.ctx, fx.U, canon)
     torch.cuda.synchronize()
     oracle.overrelax(U, gdims, 1.8, 1)
-    # second sweep: tiles still bit-identical; errors of the first sweep are amplified by the second
-    _check_tiles(canon, gdims, U, 10 * TOL_LINK[precision], tail=2e-5 if precision == "fp32" else 0.0, tail_tol=2e-3)
+    # second sweep: tiles still bit-identical; north_star states no bound after two sweeps -- the errors of the first
+    # are carried through the second (measured 3.4e-5 fp32, 2e-13 fp64): twice / ten times the one-sweep bound
+    _check_tiles(canon, gdims, U, (2 if precision == "fp32" else 10) * TOL_LINK[precision])
     # F and theta of a tiled field equal those of the tile
     assert fx.functional() == pytest.approx(oracle.functional(U, gdims), rel=TOL_F[precision])
     assert fx.theta() == pytest.approx(oracle.theta(U, gdims), rel=1e-6 if precision == "fp64" else 1e-2)
@@ -175,11 +186,19 @@ def test_config5_48x3x64_coulomb_overrelax_tiles(gfm):
     torch.cuda.empty_cache()
 
 
-def test_config5_48x3x64_coulomb_anneal_sampled_sites(gfm):
-    """One annealing step at T = 1.4 (the schedule's first) on the full lattice.  For sampled BLACK sites b the
-    oracle redoes, one by one from the same (fp32-rounded) input, the RED heatbath updates of the 8 neighbours of
-    b and then the BLACK update of b: after that the 8 links at b are final (every link is touched once per
-    half-sweep, C6) and are compared with the CUDA result, as are the trial counts of all 9 site updates."""
+@pytest.mark.parametrize("T,chain", [(1.4, 2), (0.05, 2), (1.4, 1)])  # chain: gf_set_chain
+def test_config5_48x3x64_coulomb_anneal_census(gfm, T, chain):
+    """One annealing step on the full 48^3x64 lattice at the two ends of the schedule, EVERY Kennedy-Pendleton trial
+    count against the oracle's on the same fp32-rounded input.  RED half-sweep: the inputs are identical, so every
+    mismatch is a genuine flip of an accept decision: at most 1e-5 of the 10.6 M draws (C14; measured 1e-7: 0 or 1).
+    Whole step (the BLACK sites see RED links that differ by fp32 rounding): the same bound.
+    Links, at every site further than Manhattan distance 2 from a flipped decision: at the cold end of the schedule
+    every link is within 5e-5 (measured max 7.7e-6).  At T = 1.4 the fp32 draw leaves a tail: delta and alpha = |k|/T
+    carry ~1e-6 from the SFU draw and the fp32 rounding of K, a BLACK site with a small block |k| amplifies what its RED
+    neighbours left by 1/|k|, and 7 M sites reach |k| ~ 0.05.  Bar: at most 1e-5 of the sites above 5e-5, none above
+    5e-4.  Measured: default chain 46 of 7 077 806 sites above 5e-5, max 1.2e-4; double chain (chain = 1) 15, max
+    7.6e-5.  Stated in gf.h (gf_set_chain) and DESIGN.md sec. 4; at 8^4 every link is inside 5e-5
+    (tests/test_gpu_parity.py::test_anneal_fp32_one_step)."""
     import torch
 
     gdims, dims = (24, 24, 24, 32), (48, 48, 48, 64)
@@ -187,56 +206,51 @@ def test_config5_48x3x64_coulomb_anneal_sampled_sites(gfm):
     U = gf_inputs.smooth_random(gdims, 0.5, 5)
     canon = _tiled_device(U, gdims)
     fx = gfm.GaugeFixer(dims, precision="fp32", gauge="coulomb")
+    gfm.gf_set_chain(fx.ctx, chain)
     trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
     gfm.gf_set_trial_buffer(fx.ctx, trials)
     gfm.gf_pack(fx.ctx, canon, fx.U)
+    fx.anneal(T, T, 1, 7)
+    gfm.gf_unpack(fx.ctx, fx.U, canon)
+    torch.cuda.synchronize()
+    got_trials = trials.cpu().numpy().reshape(V, 3)
+    del trials
     # the fp32-rounded input, as the kernel sees it -- rounded on the host (no oracle input comes from the CUDA path)
     Nx, Ny, Nz, Nt = gdims
     work = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(V, 4, 3, 3)
     work = work.astype(np.complex64).astype(np.complex128)
-    fx.anneal(1.4, 1.4, 1, 7)
-    gfm.gf_unpack(fx.ctx, fx.U, canon)
-    torch.cuda.synchronize()
+    ref_trials = np.zeros((V, 3), dtype=np.int32)
+    oracle.heatbath_half(work, dims, T, 7, 0, 0, oracle.COULOMB, trials=ref_trials)
+    s = np.arange(V)
+    red = ((s % 48 + (s // 48) % 48 + (s // 48**2) % 48 + s // 48**3) & 1) == 0
+    assert got_trials.min() >= 1 and got_trials.max() < 4096
+    if T > 1:
+        assert got_trials.max() > 1
+    flips_red = int((got_trials[red] != ref_trials[red]).sum())
+    assert flips_red <= 1e-5 * 3 * red.sum(), flips_red
+    oracle.heatbath_half(work, dims, T, 7, 0, 1, oracle.COULOMB, trials=ref_trials)
+    flipped = (got_trials != ref_trials).any(axis=1)
+    assert flipped.sum() <= 1e-5 * 3 * V, int(flipped.sum())
     after = canon.cpu().numpy().view("complex128").reshape(V, 4, 3, 3)
-    got_trials = trials.cpu().numpy().reshape(V, 3)
     del canon
-    assert got_trials.min() >= 1 and got_trials.max() < 4096 and got_trials.max() > 1
-
+    err = np.abs(after - work).reshape(V, -1).max(axis=1)
+    del after
+    # a flipped site changes its 8 links, through them K and the draws of its BLACK neighbours and their links
     N = np.array(dims)
-    stride = np.array([1, 48, 48 * 48, 48 * 48 * 48])
-
-    def site(c):
-        return int(((c % N) * stride).sum())
-
-    rng = np.random.default_rng(11)
-    buf = np.zeros((V, 3), dtype=np.int32)
-    done_red, n_sites, n_links_ok, n_trials_ok, n_updates = set(), 0, 0, 0, 0
-    while n_sites < 150:
-        c = rng.integers(0, 64, size=4) % N
-        if c.sum() % 2 == 0:
-            c[0] = (c[0] + 1) % 48  # make it BLACK
-        nbrs = [site(c + d * np.eye(4, dtype=int)[mu]) for mu in range(4) for d in (+1, -1)]
-        if any(r in done_red for r in nbrs):
-            continue  # a RED neighbour already updated in `work` for another sample
-        ok = True
-        for r in nbrs:
-            ref_tr = oracle.site_heatbath(work, dims, r, 1.4, 7, 0, oracle.COULOMB, buf)
-            done_red.add(r)
-            ok &= bool(np.array_equal(ref_tr, got_trials[r]))
-            n_updates += 1
-        b = site(c)
-        ref_tr = oracle.site_heatbath(work, dims, b, 1.4, 7, 0, oracle.COULOMB, buf)
-        ok &= bool(np.array_equal(ref_tr, got_trials[b]))
-        n_updates += 1
-        err = max(np.abs(after[b] - work[b]).max(),
-                  max(np.abs(after[site(c - np.eye(4, dtype=int)[mu]), mu] - work[site(c - np.eye(4, dtype=int)[mu]), mu]).max()
-                      for mu in range(4)))
-        n_sites += 1
-        n_trials_ok += int(ok)
-        n_links_ok += int(err <= TOL_LINK["fp32"])
-    # fp32 vs fp64 alpha: a flipped accept decision is possible but rare (C14)
-    assert n_trials_ok >= n_sites - 2, (n_trials_ok, n_sites)
-    assert n_links_ok >= n_sites - 3, (n_links_ok, n_sites)
+    far = np.ones(V, dtype=bool)
+    offs = [np.array(o) - 2 for o in np.ndindex(5, 5, 5, 5) if sum(abs(np.array(o) - 2)) <= 2]
+    for f in np.nonzero(flipped)[0]:
+        c = np.array([f % 48, (f // 48) % 48, (f // 48**2) % 48, f // 48**3])
+        for o in offs:
+            e = (c + o) % N
+            far[int(e[0] + 48 * (e[1] + 48 * (e[2] + 48 * e[3])))] = False
+    err = err[far]
+    print(f"census T={T} chain={chain}: flips RED {flips_red}, whole step {int(flipped.sum())} sites; links max {err.max():.3e}, "
+          f"above 5e-5: {int((err > 5e-5).sum())}, above 2e-5: {int((err > 2e-5).sum())} of {err.size}")
+    if T < 0.5:
+        assert err.max() <= TOL_LINK["fp32"], (err.max(), int((err > TOL_LINK["fp32"]).sum()))
+    else:
+        assert (err > TOL_LINK["fp32"]).mean() <= 1e-5 and err.max() <= 5e-4, (err.max(), int((err > TOL_LINK["fp32"]).sum()))
     fx.close()
     torch.cuda.empty_cache()
 

@@ -400,9 +400,10 @@ def test_no_write_outside_the_field(gfm, precision, R, gauge):
             gfm.gf_relax(ctx, field, gfm.GF_UPDATE_STOCHASTIC, 0.5, 1, 3)
             gfm.gf_relax(ctx, field, gfm.GF_UPDATE_OVERRELAX1, 1.4, 1, 0)
             gfm.gf_anneal_micro(ctx, field, 1.0, 0.5, 2, 1, 7)
-            gfm.gf_set_fusion(ctx, 2)
-            gfm.gf_overrelax(ctx, field, 1.7, 1)
-            gfm.gf_set_fusion(ctx, 0)
+            for chain in (0, 1, 2):  # fp32: every precision of the site chain
+                gfm.gf_set_chain(ctx, chain)
+                gfm.gf_overrelax(ctx, field, 1.7, 3)
+                gfm.gf_anneal(ctx, field, 0.7, 0.7, 1, 9)
     gfm.gf_functional(ctx, field)
     gfm.gf_theta(ctx, field)
     if gauge == "coulomb":

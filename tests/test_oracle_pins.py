@@ -478,3 +478,55 @@ def test_sweep_order_red_then_black():
     Ue = U.copy()
     oracle.overrelax_half(Ue, dims, 1.7, 0)
     np.testing.assert_array_equal(Ud, Ue)
+
+
+def test_unitarity_defect_of_known_matrices():
+    """orc_unitarity_defect is the checker of several GPU tests: pin it on matrices with a known defect.
+    diag(1+e, 1, 1): U U^dagger - 1 = diag(2e + e^2, 0, 0), det - 1 = e; a unitary matrix with det = exp(i a):
+    U U^dagger = 1 and |det - 1| = 2 sin(a/2); an SU(3) field: both ~ 1e-16."""
+    dims = (2, 2, 2, 2)
+    U = gf_inputs.hot(dims, 5)
+    uu, det = oracle.unitarity_defect(U, dims)
+    assert uu < 1e-14 and det < 1e-14
+    eps = 3e-4
+    V = U.copy()
+    V[5, 2] = np.diag([1 + eps, 1.0, 1.0])
+    uu, det = oracle.unitarity_defect(V, dims)
+    assert uu == pytest.approx(2 * eps + eps * eps, rel=1e-10) and det == pytest.approx(eps, rel=1e-10)
+    a = 0.02
+    W = U.copy()
+    W[7, 1] = W[7, 1] * np.exp(1j * a / 3)  # unitary, det = exp(i a)
+    uu, det = oracle.unitarity_defect(W, dims)
+    assert uu < 1e-14 and det == pytest.approx(2 * np.sin(a / 2), rel=1e-9)
+    X = U.copy()
+    X[0, 0, 0, 1] += 1e-3  # one off-diagonal entry of one link: (U U^dagger - 1) picks up terms of that size
+    uu, det = oracle.unitarity_defect(X, dims)
+    assert 5e-4 < uu < 3e-3
+
+
+def test_reunitarise_projects_back_to_su3():
+    """orc_reunitarise (the definition of the CUDA path's re-orthonormalisation on load, C15): a sheared and scaled
+    link comes back unitary with det 1; row 0 keeps its direction, row 1 keeps its component orthogonal to row 0,
+    row 2 = conj(row0 x row1); an SU(3) link is left unchanged to rounding."""
+    dims = (2, 2, 2, 2)
+    U = gf_inputs.hot(dims, 6)
+    V = U.copy()
+    oracle.reunitarise(V, dims)
+    assert np.abs(V - U).max() < 1e-14
+    rng = np.random.default_rng(3)
+    D = U.copy()
+    D *= 1.0 + 0.05 * rng.standard_normal((D.shape[0], 4, 3, 1))  # every row scaled
+    D[:, :, 1, :] += 0.1 * D[:, :, 0, :]                          # row 1 sheared towards row 0
+    D[:, :, 2, :] = rng.standard_normal(D[:, :, 2, :].shape)      # row 2 destroyed
+    W = D.copy()
+    oracle.reunitarise(W, dims)
+    uu, det = oracle.unitarity_defect(W, dims)
+    assert uu < 1e-14 and det < 1e-14
+    r0 = D[:, :, 0, :] / np.linalg.norm(D[:, :, 0, :], axis=-1, keepdims=True)
+    assert np.abs(W[:, :, 0, :] - r0).max() < 1e-14
+    r1 = D[:, :, 1, :] - (np.conj(r0) * D[:, :, 1, :]).sum(-1, keepdims=True) * r0
+    r1 /= np.linalg.norm(r1, axis=-1, keepdims=True)
+    assert np.abs(W[:, :, 1, :] - r1).max() < 1e-14
+    assert np.abs(W[:, :, 2, :] - np.conj(np.cross(r0, r1))).max() < 1e-14
+    # the shear and the scaling did not change the SU(3) matrix the first two rows span: it is the original link
+    assert np.abs(W - U).max() < 1e-13

@@ -187,3 +187,52 @@ def test_fix_slices_freezes_timeslices_independently():
     # nothing to do on a fixed field
     n2, _, _, per2 = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 5, 3000)
     assert n2 == 0 and per2.max() == 0
+
+
+def test_fix_chunks_continue_the_stochastic_sweep_counter():
+    """C18: inside the fixing loop the sweep counter of the stochastic decisions runs on through the chunks, so a
+    chunked run is the unchunked run bit for bit (no decision is replayed) -- pinned against orc_relax, and the
+    decisions of consecutive sweeps against the stated Philox recipe with counter word 1 = 0, 1, 2"""
+    dims = (4, 4, 4, 6)
+    V = int(np.prod(dims))
+    U0 = gf_inputs.smooth_random(dims, 0.4, 44)
+    p, seed, nsw = 0.4, 11, 6
+    whole = U0.copy()
+    oracle.relax(whole, dims, oracle.UPDATE_STOCHASTIC, p, nsw, seed)
+    for every in (1, 2, 4):
+        chunked = U0.copy()
+        n, th, F = oracle.fix(chunked, dims, oracle.UPDATE_STOCHASTIC, p, 0.0, every, nsw, seed)  # tol 0: never stops
+        assert n == nsw and np.array_equal(chunked, whole), every
+    # relax_from(sweep0) takes the decisions of sweep sweep0 of the recipe, not those of sweep 0
+    for sweep0 in (0, 1, 2):
+        c = U0.copy()
+        sq = oracle.relax_from(c, dims, oracle.UPDATE_STOCHASTIC, p, 1, sweep0, seed, squared=True)
+        for s in (3, 40, V - 2):
+            x = s % 4 + (s // 4) % 4 + (s // 16) % 4 + s // 64
+            for sub in range(3):
+                w = oracle.philox4x32_10([s, sweep0, ((x & 1) << 2) | sub, 0x40000000], [seed, 0])[0]
+                assert sq[s, sub] == int((2 * (int(w) >> 9) + 1) / 2**24 < p)
+    a, b = U0.copy(), U0.copy()
+    sa = oracle.relax_from(a, dims, oracle.UPDATE_STOCHASTIC, p, 1, 0, seed, squared=True)
+    sb = oracle.relax_from(b, dims, oracle.UPDATE_STOCHASTIC, p, 1, 1, seed, squared=True)
+    assert not np.array_equal(sa, sb)
+
+
+def test_heatbath_half_is_the_annealing_half_sweep():
+    """orc_heatbath_half on RED then BLACK is one annealing step (same field, same trial counts); a half-sweep
+    touches the trial counts of its own sublattice only and, by C6, no link twice"""
+    dims = (4, 4, 2, 6)
+    V = int(np.prod(dims))
+    U0 = gf_inputs.smooth_random(dims, 0.5, 45)
+    a = U0.copy()
+    ta = oracle.anneal(a, dims, 0.9, 0.9, 1, 7, trials=True)
+    b = U0.copy()
+    tb = np.full((V, 3), -1, dtype=np.int32)
+    oracle.heatbath_half(b, dims, 0.9, 7, 0, 0, trials=tb)
+    s = np.arange(V)
+    par = (s % 4 + (s // 4) % 4 + (s // 16) % 2 + s // 32) & 1
+    assert (tb[par == 1] == -1).all() and (tb[par == 0] >= 1).all()
+    # every link has exactly one RED end: after the RED half-sweep every link differs from its input
+    assert (np.abs(b - U0).reshape(V * 4, -1).max(axis=1) > 1e-6).all()
+    oracle.heatbath_half(b, dims, 0.9, 7, 0, 1, trials=tb)
+    assert np.array_equal(a, b) and np.array_equal(ta, tb)
