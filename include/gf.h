@@ -125,10 +125,24 @@ int gf_theta_slices(gf_ctx* ctx, const void* U_native_dev, double* theta_host_Nt
 /* ---- Alg. 1 with its stop rule -------------------------------------------------------------------------------- */
 
 /* "while precision theta not reached do" with the check after every `check_every`-th sweep
- * (C11): gf_theta; while theta >= theta_tol and fewer than max_sweeps sweeps done: gf_relax(update,
- * param, min(check_every, max_sweeps - done), seed); gf_theta.  Coulomb: theta = max over timeslices (C12).
- * sweeps_done / theta_host / F_host (each may be NULL) receive the number of sweeps, the last theta and F.
- * Synchronises at every check.  Errors as gf_relax; GF_EINVAL also for check_every < 1, max_sweeps < 0. */
+ * (C11).  Coulomb: theta = max over timeslices (C12).  sweeps_done / theta_host / F_host (each may be
+ * NULL) receive the number of sweeps and theta and F of the field as returned.  Two forms of the loop:
+ *   fused monitor (default where it applies and check_every <= 10, see gf_set_monitor; C21): theta and F of the state
+ *     after sweep n are accumulated by the
+ *     sweep kernels themselves -- the BLACK half-sweep of sweep n leaves K(x) of its sites in registers, the RED
+ *     half-sweep of sweep n+1 builds K(x) of the other half from that state before updating it -- and reduced on the
+ *     device in a fixed order while sweep n+1 runs.  The loop ends ONE SWEEP AFTER the first checked sweep n with
+ *     theta < theta_tol (sweeps_done = n + 1; a check needs the sweep after it, so none takes place at
+ *     n = max_sweeps).  No pass over the field per check, no host synchronisation per check: sweeps are enqueued in
+ *     batches of 32 and launches past the stop return at once.  theta before the first sweep and theta / F of the
+ *     returned field come from the separate reductions.  Oracle: orc_fix_lag(lag = 1).
+ *   separate check (gf_set_monitor(ctx, 0); the paper's second kernel): gf_theta; while theta >=
+ *     theta_tol and fewer than max_sweeps sweeps done: min(check_every, max_sweeps - done) sweeps; gf_theta.
+ *     Synchronises at every check.  Oracle: orc_fix_lag(lag = 0).
+ * The fused form applies when every thread block of the sweep lies inside one timeslice ((Nx Ny Nz / 2) * threads per
+ * site divisible by the block size; true for every lattice of BASELINE.json but 4^4 in fp64) and, for fp32 contexts,
+ * when theta_tol >= 1e-10 (theta formed from the fp32 K of the sweep resolves ~1e-12); otherwise the call falls back
+ * to the separate check.  Errors as gf_relax; GF_EINVAL also for check_every < 1, max_sweeps < 0. */
 int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double theta_tol, int check_every,
            int max_sweeps, unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host,
            void* stream);
@@ -136,7 +150,10 @@ int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double the
 /* Coulomb gauge, "each timeslice fixed independently" (C12, C20): as gf_fix, but a timeslice whose theta_t is below
  * theta_tol at a check is frozen for good (its sites are no longer updated; K, F and theta_t of a slice depend on
  * the spatial links of that slice alone), and the loop ends when no slice is active.  sweeps_done = sweeps of the
- * slowest slice; sweeps_per_slice (Nt ints, may be NULL) the sweeps every slice got.  GF_EINVAL for a Landau ctx. */
+ * slowest slice; sweeps_per_slice (Nt ints, may be NULL) the sweeps every slice got.  Fused monitor: the freeze of a
+ * slice found below the tolerance after sweep n takes effect from sweep n + 2 (it gets n + 1 sweeps; oracle:
+ * orc_fix_slices_lag(lag = 1)); with check_every = 1 every slice stops within one sweep of meeting the tolerance.
+ * GF_EINVAL for a Landau ctx. */
 int gf_fix_slices(gf_ctx* ctx, void* U_native_dev, int update, double param, double theta_tol, int check_every,
                   int max_sweeps, unsigned long long seed, int* sweeps_done, int* sweeps_per_slice,
                   double* theta_host, double* F_host, void* stream);
@@ -191,6 +208,14 @@ int gf_set_prefetch(gf_ctx* ctx, int sites);
  * transform the temporal links once at the end of each call -- 14/16 of the bytes, same result up to rounding.
  * gf_anneal / gf_anneal_micro keep one site field over the whole call.  GF_EINVAL for a Landau context. */
 int gf_set_coulomb_reading(gf_ctx* ctx, int reading_b);
+/* Form of the fixing loops gf_fix / gf_fix_slices: 0 = separate check; 1 (default) = fused monitor where it applies and
+ * check_every <= 10 (a monitored sweep costs ~4 % more than a plain one, a checked one ~20 %, a separate check about
+ * 0.6 sweeps: the fused form wins while checks are frequent); 2 = fused wherever it applies.  GF_EINVAL otherwise. */
+int gf_set_monitor(gf_ctx* ctx, int fused);
+/* The last check completed by a fused fixing loop on this context: the sweep n it belongs to (0: none yet), theta
+ * (Coulomb: max over timeslices) and F of the state after that sweep, the per-timeslice theta_t (Nt doubles).  Each
+ * output may be NULL.  Synchronises.  GF_EINVAL if no fused loop has run. */
+int gf_monitor_last(gf_ctx* ctx, int* check_sweep, double* theta_host, double* F_host, double* theta_host_Nt);
 /* fp32 contexts, precision of the site chain.  The links are fp32 in memory and in the link
  * products; the site chain -- K(x), the three SU(2) steps, K <- G K -- is ill-conditioned where the projected block k
  * of K or the expanded g^omega is small, and a BLACK half-sweep inherits the rounding of the RED one through its K.

@@ -73,6 +73,8 @@ def _load():
         "orc_relax_from": (None, [N, _int, _vp, _int, _dbl, _int, _int, ctypes.c_uint64, _vp]),
         "orc_heatbath_half": (None, [N, _int, _vp, _dbl, ctypes.c_uint64, ctypes.c_uint32, _int, _vp]),
         "orc_fix": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp]),
+        "orc_fix_lag": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _int, _vp, _vp]),
+        "orc_fix_slices_lag": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _int, _vp, _vp, _vp]),
         "orc_fix_slices": (_int, [N, _int, _vp, _int, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp, _vp, _vp]),
         "orc_anneal_micro": (None, [N, _int, _vp, _dbl, _dbl, _int, _int, ctypes.c_uint64, _vp]),
     }
@@ -167,23 +169,29 @@ def heatbath_half(U, dims, T: float, seed: int, step: int, parity: int, gauge: i
 
 
 def fix(U, dims, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int, seed: int = 0,
-        gauge: int = LANDAU):
-    """Alg. 1 outer loop: returns (sweeps done, theta, F)"""
+        gauge: int = LANDAU, lag: int = 0):
+    """Alg. 1 outer loop: returns (sweeps done, theta, F).  lag = 0: the paper's loop; lag = 1:
+    the loop ends one sweep after the check that met the tolerance (C21)"""
     N, V = _dims(dims)
     th, F = ctypes.c_double(), ctypes.c_double()
-    n = _load().orc_fix(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
-                        int(max_sweeps), int(seed), ctypes.byref(th), ctypes.byref(F))
+    n = _load().orc_fix_lag(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
+                            int(max_sweeps), int(seed), int(lag), ctypes.byref(th), ctypes.byref(F))
     return int(n), th.value, F.value
 
 
 def fix_slices(U, dims, update: int, param: float, theta_tol: float, check_every: int, max_sweeps: int, seed: int = 0,
-               gauge: int = COULOMB):
+               gauge: int = COULOMB, lag: int = 0):
     """Alg. 1 with the stop rule per timeslice (C20): returns (max sweeps, theta = max_t theta_t, F, sweeps per slice)"""
     N, V = _dims(dims)
     th, F = ctypes.c_double(), ctypes.c_double()
     per = np.zeros(int(dims[3]), dtype=np.int32)
-    n = _load().orc_fix_slices(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
-                               int(max_sweeps), int(seed), per.ctypes.data, ctypes.byref(th), ctypes.byref(F))
+    if lag == 0:
+        n = _load().orc_fix_slices(N, gauge, _field(U, V), int(update), float(param), float(theta_tol), int(check_every),
+                                   int(max_sweeps), int(seed), per.ctypes.data, ctypes.byref(th), ctypes.byref(F))
+    else:
+        n = _load().orc_fix_slices_lag(N, gauge, _field(U, V), int(update), float(param), float(theta_tol),
+                                       int(check_every), int(max_sweeps), int(seed), int(lag), per.ctypes.data,
+                                       ctypes.byref(th), ctypes.byref(F))
     return int(n), th.value, F.value, per
 
 

@@ -592,24 +592,35 @@ void orc_anneal_micro(const int N[4], int gauge, double *U, double T_start, doub
 /* ------------------------------------------------------------------------------------------------ */
 /* Alg. 1 outer loop ("while precision theta not reached"), with the paper's cadence of   */
 /* the check (F and theta are evaluated after every `check_every`-th iteration; C11):    */
-/* sweep in chunks of check_every (the last chunk is cut at max_sweeps) until theta < theta_tol        */
-/* (Coulomb: max over timeslices, C12).  The sweep counter of the stochastic decisions (C18) runs on    */
-/* through the chunks: a fixing run never replays its decisions.  Returns the number of sweeps done.   */
+/* theta (Coulomb: max over timeslices, C12) is evaluated before the first sweep and after every sweep */
+/* whose number is a multiple of check_every; the loop ends `lag` sweeps after the first check that    */
+/* finds theta < theta_tol, or at max_sweeps.  lag = 0 is the paper's loop; lag = 1 (C21) is the loop   */
+/* of an implementation that learns theta of the state after sweep n only while sweep n+1 runs (so a   */
+/* check at the last allowed sweep cannot take place).  The sweep counter of the stochastic decisions  */
+/* (C18) runs on through the whole loop.  Returns the number of sweeps done; theta and F of the final  */
+/* state.                                                                                              */
 /* ------------------------------------------------------------------------------------------------ */
+int orc_fix_lag(const int N[4], int gauge, double *U, int update, double param, double theta_tol, int check_every,
+                int max_sweeps, uint64_t seed, int lag, double *theta_out, double *F_out)
+{
+    int done = 0, stop_at = -1;
+    if (orc_theta_report(N, gauge, U) >= theta_tol) {
+        while (done < max_sweeps && done != stop_at) {
+            orc_relax_from(N, gauge, U, update, param, 1, done, seed, NULL);
+            done += 1;
+            if (stop_at < 0 && done % check_every == 0 && (lag == 0 || done < max_sweeps))
+                if (orc_theta_report(N, gauge, U) < theta_tol) stop_at = done + lag;
+        }
+    }
+    if (theta_out) *theta_out = orc_theta_report(N, gauge, U);
+    if (F_out) *F_out = orc_functional(N, gauge, U);
+    return done;
+}
+
 int orc_fix(const int N[4], int gauge, double *U, int update, double param, double theta_tol, int check_every,
             int max_sweeps, uint64_t seed, double *theta_out, double *F_out)
 {
-    int done = 0;
-    double th = orc_theta_report(N, gauge, U);
-    while (th >= theta_tol && done < max_sweeps) {
-        int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
-        orc_relax_from(N, gauge, U, update, param, n, done, seed, NULL);
-        done += n;
-        th = orc_theta_report(N, gauge, U);
-    }
-    if (theta_out) *theta_out = th;
-    if (F_out) *F_out = orc_functional(N, gauge, U);
-    return done;
+    return orc_fix_lag(N, gauge, U, update, param, theta_tol, check_every, max_sweeps, seed, 0, theta_out, F_out);
 }
 
 /* ------------------------------------------------------------------------------------------------ */
@@ -634,6 +645,43 @@ void orc_relax_slices(const int N[4], int gauge, double *U, int update, double p
                 if (active[s / Vs] && lat_parity(N, s) == parity)
                     orc_site_relax(N, gauge, U, s, update, param, seed, (uint32_t)(sweep0 + sweep), NULL);
         }
+}
+
+/* lag as in orc_fix_lag: a slice found below the tolerance at the check after sweep n is updated for `lag` more
+ * sweeps and frozen from sweep n + lag + 1 on */
+int orc_fix_slices_lag(const int N[4], int gauge, double *U, int update, double param, double theta_tol,
+                       int check_every, int max_sweeps, uint64_t seed, int lag, int *sweeps_per_slice,
+                       double *theta_out, double *F_out)
+{
+    const int Nt = N[3];
+    unsigned char *active = (unsigned char *)malloc((size_t)Nt);
+    double *sl = (double *)malloc(sizeof(double) * (size_t)Nt);
+    int *count = (int *)calloc((size_t)Nt, sizeof(int));
+    int *last = (int *)malloc(sizeof(int) * (size_t)Nt); /* last sweep (1-based) in which the slice is updated; -1: open */
+    int done = 0, any = 0;
+    orc_theta(N, gauge, U, sl);
+    for (int t = 0; t < Nt; ++t) { last[t] = sl[t] >= theta_tol ? -1 : 0; any |= last[t] < 0; }
+    while (any && done < max_sweeps) {
+        for (int t = 0; t < Nt; ++t) active[t] = last[t] < 0 || done + 1 <= last[t];
+        orc_relax_slices(N, gauge, U, update, param, 1, done, seed, active);
+        done += 1;
+        for (int t = 0; t < Nt; ++t) count[t] += active[t];
+        if (done % check_every == 0 && (lag == 0 || done < max_sweeps)) {
+            orc_theta(N, gauge, U, sl);
+            for (int t = 0; t < Nt; ++t)
+                if (last[t] < 0 && sl[t] < theta_tol) last[t] = done + lag; /* frozen slices stay frozen */
+        }
+        any = 0;
+        for (int t = 0; t < Nt; ++t) any |= last[t] < 0 || done < last[t];
+    }
+    orc_theta(N, gauge, U, sl);
+    double m = sl[0];
+    for (int t = 1; t < Nt; ++t) if (sl[t] > m) m = sl[t];
+    if (theta_out) *theta_out = m;
+    if (F_out) *F_out = orc_functional(N, gauge, U);
+    if (sweeps_per_slice) memcpy(sweeps_per_slice, count, sizeof(int) * (size_t)Nt);
+    free(active); free(sl); free(count); free(last);
+    return done;
 }
 
 int orc_fix_slices(const int N[4], int gauge, double *U, int update, double param, double theta_tol, int check_every,

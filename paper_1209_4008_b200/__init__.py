@@ -56,6 +56,8 @@ SIGNATURES = {
     "gf_set_pdl": (_i, [_vp, _i]),
     "gf_set_prefetch": (_i, [_vp, _i]),
     "gf_set_coulomb_reading": (_i, [_vp, _i]),
+    "gf_set_monitor": (_i, [_vp, _i]),
+    "gf_monitor_last": (_i, [_vp, _pi, _pd, _pd, _pd]),
     "gf_set_chain": (_i, [_vp, _i, _d, _d]),
     "gf_chain_count": (_i, [_vp, ctypes.POINTER(_ull), ctypes.POINTER(_ull)]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
@@ -251,6 +253,19 @@ def gf_set_prefetch(ctx, sites: int) -> None:
 
 def gf_set_coulomb_reading(ctx, reading_b: bool) -> None:
     _check(ctx, load_library().gf_set_coulomb_reading(ctx, -1 if reading_b is None else int(bool(reading_b))))
+
+
+def gf_set_monitor(ctx, fused: int) -> None:
+    """0: separate check kernel, 1: fused where it applies and pays (default), 2: fused wherever it applies"""
+    _check(ctx, load_library().gf_set_monitor(ctx, int(fused)))
+
+
+def gf_monitor_last(ctx, Nt: int):
+    """last check of a fused fixing loop: (sweep n, theta, F, [theta_t]) of the state after sweep n"""
+    n, th, F = ctypes.c_int(), ctypes.c_double(), ctypes.c_double()
+    sl = (ctypes.c_double * Nt)()
+    _check(ctx, load_library().gf_monitor_last(ctx, ctypes.byref(n), ctypes.byref(th), ctypes.byref(F), sl))
+    return n.value, th.value, F.value, list(sl)
 
 
 def gf_set_chain(ctx, chain: int, watch_threshold: float = 0.0, fix_threshold: float = 0.0) -> None:

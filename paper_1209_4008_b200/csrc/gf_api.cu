@@ -2,6 +2,7 @@
 // No arithmetic of the method lives here; every step runs in the kernels of gf_sweep.cuh / gf_aux.cu.
 #include <cstdarg>
 #include <cstdio>
+#include <climits>
 #include <cstring>
 #include <new>
 
@@ -36,6 +37,13 @@ struct gf_ctx {
     double* d_out;                    // reduction results: [0] total, [1] max slice, [2..2+Nt) slices
     double* h_out;                    // pinned mirror of d_out
     int bx;
+    // fused F / theta monitor of gf_fix / gf_fix_slices (lazily allocated; sized for one launch shape)
+    int monitor;                      // 0: the paper's separate check kernel, 1: fused where it applies and pays (default), 2: fused where it applies
+    char* d_mon;                      // MonitorState, theta_t[2 Nt], frozen_from[Nt] | group | partials
+    char* h_mon;                      // pinned: two copies of the prefix up to `frozen`
+    size_t mon_prefix, mon_bytes;
+    int mon_blocks, mon_groups;       // partials per plane, duty blocks per timeslice the buffer was sized for
+    cudaEvent_t mon_event[2];
     // host-buffer path staging (lazily allocated)
     double* d_canon;
     void* d_native;
@@ -101,6 +109,8 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     c->d_canon = nullptr; c->d_native = nullptr;
     c->err[0] = 0;
     c->bx = reduce_blocks_per_slice(c->L);
+    c->monitor = 1; c->d_mon = nullptr; c->h_mon = nullptr; c->mon_prefix = c->mon_bytes = 0; c->mon_blocks = c->mon_groups = 0;
+    c->mon_event[0] = c->mon_event[1] = nullptr;
     const size_t npart = (size_t)c->bx * 2 * Nt;
     c->d_partials = nullptr; c->d_out = nullptr; c->h_out = nullptr;
     if ((e = cudaMalloc(&c->d_partials, npart * sizeof(double))) != cudaSuccess ||
@@ -122,6 +132,9 @@ extern "C" void gf_destroy(gf_ctx* c)
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_out) cudaFree(c->d_out);
     if (c->d_rough) cudaFree(c->d_rough);
+    if (c->d_mon) cudaFree(c->d_mon);
+    if (c->h_mon) cudaFreeHost(c->h_mon);
+    for (int i = 0; i < 2; ++i) if (c->mon_event[i]) cudaEventDestroy(c->mon_event[i]);
     if (c->h_out) cudaFreeHost(c->h_out);
     if (c->d_canon) cudaFree(c->d_canon);
     if (c->d_native) cudaFree(c->d_native);
@@ -198,6 +211,29 @@ extern "C" int gf_set_trial_buffer(gf_ctx* c, unsigned* d_trials)
 {
     if (c == nullptr) return GF_EINVAL;
     c->d_trials = d_trials;
+    return GF_OK;
+}
+
+extern "C" int gf_set_monitor(gf_ctx* c, int fused)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (fused < 0 || fused > 2) return fail(c, GF_EINVAL, "gf_set_monitor: mode must be 0 (separate check), 1 (automatic) or 2 (fused wherever it applies)");
+    c->monitor = fused;
+    return GF_OK;
+}
+
+extern "C" int gf_monitor_last(gf_ctx* c, int* check_sweep, double* theta_host, double* F_host, double* theta_host_Nt)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (c->d_mon == nullptr) return fail(c, GF_EINVAL, "gf_monitor_last: no fused fixing loop has run on this context");
+    cudaError_t e = cudaStreamSynchronize(c->last_stream);
+    if (e == cudaSuccess) e = cudaMemcpy(c->h_mon, c->d_mon, c->mon_prefix, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gf_monitor_last");
+    const MonitorState* hs = reinterpret_cast<const MonitorState*>(c->h_mon);
+    if (check_sweep) *check_sweep = hs->checks > 0 ? hs->check_sweep : 0;
+    if (theta_host) *theta_host = hs->theta;
+    if (F_host) *F_host = hs->F;
+    if (theta_host_Nt) memcpy(theta_host_Nt, c->h_mon + sizeof(MonitorState), sizeof(double) * (size_t)c->Nt);
     return GF_OK;
 }
 
@@ -631,6 +667,196 @@ extern "C" int gf_theta_slices(gf_ctx* c, const void* U, double* theta_host_Nt)
     return GF_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Alg. 1 with its stop rule, monitored from inside the sweeps (SweepMonitor, gf_sweep.cuh): theta(S_n) and F(S_n) of
+// the state after sweep n are complete when the BLACK half-sweep of sweep n+1 has run, so the loop stops one sweep
+// after the sweep that met the tolerance (oracle: orc_fix / orc_fix_slices with lag = 1), and no launch waits for the
+// host: sweeps are enqueued in batches, the device state is copied out behind each batch, and the host reads the copy
+// of the batch before the one just enqueued.  Launches past the stop return at once.
+// ---------------------------------------------------------------------------------------------------------
+static int update_to_mode(int update, int* mode, int* variant)
+{
+    *variant = 0;
+    switch (update) {
+    case GF_UPDATE_OVERRELAX2: *mode = MODE_OVERRELAX; return GF_OK;
+    case GF_UPDATE_OVERRELAX1: *mode = MODE_VARIANT; *variant = VARIANT_OVERRELAX1; return GF_OK;
+    case GF_UPDATE_STOCHASTIC: *mode = MODE_VARIANT; *variant = VARIANT_STOCHASTIC; return GF_OK;
+    default: return GF_EINVAL;
+    }
+}
+
+// can this context run the fused monitor with the current launch shape?  every block must lie inside one timeslice;
+// fp32 contexts form theta from the fp32 K of the sweep, which resolves it down to ~1e-12 only
+// and it pays while checks are frequent: a monitored sweep costs ~4 % more than a plain one and a checked one ~20 %
+// (32^4 fp32: 185 / 214 against 178 us), the separate check ~110 us per check -- break-even near one check per 10 sweeps
+static bool monitor_applies(const gf_ctx* c, int mode, double tol, int check_every)
+{
+    if (!c->monitor) return false;
+    if (c->monitor == 1 && check_every > 10) return false;
+    const unsigned Hs = c->L.H / (unsigned)c->Nt;
+    const unsigned tps = (unsigned)auto_tps(c, mode), block = (unsigned)auto_block(c);
+    if ((Hs * tps) % block != 0) return false;
+    if (c->precision == GF_FP32 && tol < 1e-10) return false;
+    return true;
+}
+
+static int monitor_alloc(gf_ctx* c, int blocks, int groups)
+{
+    const size_t Nt = (size_t)c->Nt;
+    const size_t prefix = ((sizeof(MonitorState) + 2 * Nt * sizeof(double) + Nt * sizeof(int) + 63) / 64) * 64;
+    const size_t bytes = prefix + 3 * Nt * (size_t)groups * sizeof(double) + 5 * (size_t)blocks * sizeof(double);
+    cudaError_t e;
+    if (c->d_mon != nullptr && (bytes > c->mon_bytes || blocks != c->mon_blocks || groups != c->mon_groups)) {
+        cudaFree(c->d_mon);
+        c->d_mon = nullptr;
+    }
+    if (c->d_mon == nullptr) {
+        if ((e = cudaMalloc(&c->d_mon, bytes)) != cudaSuccess) { c->d_mon = nullptr; return cuda_fail(c, e, "monitor: allocation"); }
+        c->mon_bytes = bytes; c->mon_blocks = blocks; c->mon_groups = groups; c->mon_prefix = prefix;
+    }
+    if (c->h_mon == nullptr) {
+        if ((e = cudaMallocHost(&c->h_mon, 2 * prefix)) != cudaSuccess) { c->h_mon = nullptr; return cuda_fail(c, e, "monitor: pinned allocation"); }
+        for (int i = 0; i < 2; ++i)
+            if ((e = cudaEventCreateWithFlags(&c->mon_event[i], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(c, e, "monitor: event");
+    }
+    return GF_OK;
+}
+
+static int fix_fused(gf_ctx* c, void* U, int update, double param, double tol, int check_every, int max_sweeps,
+                     unsigned long long seed, cudaStream_t st, bool slices, int* sweeps_done, int* per_slice,
+                     double* theta_host, double* F_host, const char* who)
+{
+    int mode, variant;
+    if (update_to_mode(update, &mode, &variant) != GF_OK) return fail(c, GF_EINVAL, "%s: unknown update %d", who, update);
+    const int Nt = c->Nt;
+    const unsigned Hs = c->L.H / (unsigned)Nt;
+    const int tps = auto_tps(c, mode), block = auto_block(c);
+    const int bps = (int)(Hs * (unsigned)tps / (unsigned)block), blocks = bps * Nt;
+    const int groups = bps < 8 ? bps : 8;
+    int rc = monitor_alloc(c, blocks, groups);
+    if (rc != GF_OK) return rc;
+    // the check before the first sweep: the separate reduction (the BLACK sites of S_0 have no sweep behind them)
+    if ((rc = reduce_to_host(c, U, true, who)) != GF_OK) return rc;
+    const bool coulomb = c->gauge == GF_COULOMB;
+    char* h0 = c->h_mon;
+    memset(h0, 0, c->mon_prefix);
+    MonitorState* hs = reinterpret_cast<MonitorState*>(h0);
+    double* h_theta_t = reinterpret_cast<double*>(h0 + sizeof(MonitorState));
+    int* h_from = reinterpret_cast<int*>(h0 + sizeof(MonitorState) + 2 * (size_t)Nt * sizeof(double));
+    int active = 0;
+    for (int t = 0; t < Nt; ++t) {
+        h_theta_t[t] = c->h_out[2 + t];
+        const bool fr = slices && c->h_out[2 + t] < tol;
+        h_from[t] = fr ? 1 : INT_MAX;
+        active += fr ? 0 : 1;
+    }
+    hs->theta = coulomb ? c->h_out[1] : c->h_out[0];
+    hs->any_active = active;
+    hs->stop_sweep = -1;
+    hs->stop_from = INT_MAX;
+    const bool fixed_already = slices ? active == 0 : hs->theta < tol;
+    int done = 0;
+    if (!fixed_already && max_sweeps > 0) {
+        cudaError_t e = cudaMemcpyAsync(c->d_mon, h0, c->mon_prefix, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, who);
+        void* gfield;
+        if ((rc = reading_b_begin(c, mode, st, &gfield, who)) != GF_OK) return rc;
+        SweepParams p = base_params(c, U);
+        p.G = gfield;
+        p.omega = param;
+        p.variant = variant;
+        p.key0 = (uint32_t)seed;
+        p.key1 = (uint32_t)(seed >> 32);
+        char* d = c->d_mon;
+        SweepMonitor m;
+        memset(&m, 0, sizeof m);
+        m.state = reinterpret_cast<MonitorState*>(d);
+        m.theta_t = reinterpret_cast<double*>(d + sizeof(MonitorState));
+        m.frozen_from = reinterpret_cast<int*>(d + sizeof(MonitorState) + 2 * (size_t)Nt * sizeof(double));
+        m.group = reinterpret_cast<double*>(d + c->mon_prefix);
+        double* part = m.group + 3 * (size_t)Nt * groups; // planes: F[0], F[1], post[0], post[1], pre
+        m.groups = groups;
+        m.blocks_per_slice = bps;
+        m.slices = slices ? 1 : 0;
+        m.coulomb = coulomb ? 1 : 0;
+        m.tol = tol;
+        const double V = 2.0 * (double)c->L.H, nd = coulomb ? 3.0 : 4.0;
+        m.scale_theta_t = 1.0 / (3.0 * V / Nt);
+        m.scale_theta = 1.0 / (3.0 * V);
+        m.scale_F = 1.0 / (3.0 * nd * V);
+        const int batch_sweeps = 32;
+        int enq = 0, batch = 0, launched = 0;
+        bool stopped = false;
+        while (rc == GF_OK && enq < max_sweeps && !stopped) {
+            const int nb = batch_sweeps < max_sweeps - enq ? batch_sweeps : max_sweeps - enq;
+            for (int i = enq + 1; i <= enq + nb && rc == GF_OK; ++i) { // sweep i (1-based)
+                const bool prev_check = i - 1 >= 1 && (i - 1) % check_every == 0; // theta(S_{i-1}) is being completed
+                const bool this_check = i % check_every == 0 && i < max_sweeps;   // theta(S_i) needs RED_{i+1}
+                const bool reunit = reunit_due(c, mode == MODE_VARIANT && variant == VARIANT_STOCHASTIC);
+                p.ph.step = (uint32_t)(i - 1);
+                for (int parity = 0; parity < 2 && rc == GF_OK; ++parity) { // RED, BLACK
+                    set_phase(c, p, parity, reunit);
+                    p.mon = m;
+                    p.mon.sweep = i;
+                    if (parity == 0) {
+                        p.mon.pre_part = prev_check ? part + 4 * (size_t)blocks : nullptr;
+                    } else {
+                        if (this_check) {
+                            p.mon.F_part = part + (size_t)(i & 1) * blocks;
+                            p.mon.post_part = part + (size_t)(2 + (i & 1)) * blocks;
+                        }
+                        if (prev_check) {
+                            p.mon.red_F = part + (size_t)((i - 1) & 1) * blocks;
+                            p.mon.red_post = part + (size_t)(2 + ((i - 1) & 1)) * blocks;
+                            p.mon.red_pre = part + 4 * (size_t)blocks;
+                            p.mon.check_sweep = i - 1;
+                        }
+                    }
+                    e = launch_sweep(c, mode, p, st);
+                    if (e != cudaSuccess) { rc = cuda_fail(c, e, who); break; }
+                    c->launches += 1;
+                    c->half_sweeps += 1;
+                    launched += 1;
+                }
+                c->call_sweeps += 1;
+            }
+            if (rc != GF_OK) break;
+            enq += nb;
+            // the device state behind this batch, into the pinned copy of this batch; read the copy of the batch before
+            char* hb = c->h_mon + (size_t)(batch & 1) * c->mon_prefix;
+            if ((e = cudaMemcpyAsync(hb, c->d_mon, c->mon_prefix, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+                (e = cudaEventRecord(c->mon_event[batch & 1], st)) != cudaSuccess) { rc = cuda_fail(c, e, who); break; }
+            if (batch >= 1) {
+                if ((e = cudaEventSynchronize(c->mon_event[(batch - 1) & 1])) != cudaSuccess) { rc = cuda_fail(c, e, who); break; }
+                stopped = reinterpret_cast<const MonitorState*>(c->h_mon + (size_t)((batch - 1) & 1) * c->mon_prefix)->stop_from != INT_MAX;
+            }
+            ++batch;
+        }
+        // after a failed launch the temporal links are still transformed with the g(x) accumulated so far (reading B)
+        if (rc == GF_OK || launched > 0) {
+            char first[512];
+            if (rc != GF_OK) memcpy(first, c->err, sizeof first);
+            const int rc2 = reading_b_end(c, U, gfield, st, who);
+            if (rc != GF_OK) memcpy(c->err, first, sizeof first);
+            else rc = rc2;
+        }
+        if (rc != GF_OK) return rc;
+        if ((e = cudaMemcpyAsync(h0, c->d_mon, c->mon_prefix, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(c, e, who);
+        done = hs->stop_from != INT_MAX && hs->stop_from - 1 < enq ? hs->stop_from - 1 : enq;
+    }
+    if (sweeps_done) *sweeps_done = done;
+    if (per_slice)
+        for (int t = 0; t < Nt; ++t) per_slice[t] = h_from[t] - 1 < done ? h_from[t] - 1 : done;
+    // theta and F of the field as it is returned: the separate reductions, once
+    if (theta_host) {
+        if ((rc = reduce_to_host(c, U, true, who)) != GF_OK) return rc;
+        *theta_host = coulomb ? c->h_out[1] : c->h_out[0];
+    }
+    if (F_host) return gf_functional(c, U, F_host);
+    return GF_OK;
+}
+
 extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta_tol, int check_every, int max_sweeps,
                       unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host, void* stream)
 {
@@ -643,7 +869,15 @@ extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta
     double th = 0.0;
     int rc = begin_call(c, (cudaStream_t)stream);
     if (rc == GF_OK) rc = relax_chunk(c, U, update, param, 0, 0, seed, (cudaStream_t)stream, "gf_fix"); // argument check
-    if (rc == GF_OK) rc = gf_theta(c, U, &th);
+    if (rc != GF_OK) return rc;
+    {
+        int mode, variant;
+        update_to_mode(update, &mode, &variant);
+        if (monitor_applies(c, mode, theta_tol, check_every))
+            return fix_fused(c, U, update, param, theta_tol, check_every, max_sweeps, seed, (cudaStream_t)stream, false,
+                             sweeps_done, nullptr, theta_host, F_host, "gf_fix");
+    }
+    rc = gf_theta(c, U, &th);
     // Alg. 1: "while precision theta not reached", checked every check_every-th sweep
     while (rc == GF_OK && th >= theta_tol && done < max_sweeps) {
         const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
@@ -679,6 +913,9 @@ extern "C" int gf_fix_slices(gf_ctx* c, void* U, int update, double param, doubl
         return fail(c, GF_EINVAL, "gf_fix_slices: parameter %g out of range for update %d", param, update);
     cudaStream_t st = (cudaStream_t)stream;
     if (begin_call(c, st) != GF_OK) return GF_ECUDA;
+    if (monitor_applies(c, mode, theta_tol, check_every))
+        return fix_fused(c, U, update, param, theta_tol, check_every, max_sweeps, seed, st, true, sweeps_done,
+                         sweeps_per_slice, theta_host, F_host, "gf_fix_slices");
     const int Nt = c->Nt;
     unsigned char* active = new (std::nothrow) unsigned char[Nt];
     int* count = new (std::nothrow) int[Nt];

@@ -11,6 +11,7 @@
 // Memory: every link is read once and written once per half-sweep (C6), each access a coalesced 128-bit
 // vector per thread (gf_device.cuh); all loads of a thread are issued before the first use.
 #pragma once
+#include <climits>
 #include <type_traits>
 
 #include "gf_device.cuh"
@@ -37,6 +38,50 @@ struct SweepPhase {
 enum { CHAIN_FP32 = 0, CHAIN_DOUBLE = 1, CHAIN_HYBRID = 2 };
 constexpr int ROUGH_RING = 4;
 
+// Device-resident state of the fused F / theta monitor (gf_fix, gf_fix_slices): written by the reduction duty of a BLACK
+// half-sweep, read by every later launch (stop, frozen) and, at batch boundaries, by the host.
+struct MonitorState {
+    unsigned ticket;      // duty blocks that have delivered their group partial
+    int stop_from;        // every half-sweep of a sweep >= stop_from returns at once (INT_MAX: none).  Stamped with the
+                          // sweep it takes effect from: the duty that decides runs inside a BLACK half-sweep whose
+                          // later blocks must still do their work
+    int stop_sweep;       // sweep index n whose check decided the stop (stop_from = n + 2), -1: none
+    int checks;           // checks completed
+    int check_sweep;      // sweep index of the last completed check
+    int any_active;       // slices mode: slices still active after the last check
+    double theta, F;      // of the last check: theta of eq. 2.5 (Coulomb: max over the timeslices), F of eq. 2.1
+};
+
+// Fused monitor of a launch (MON kernels).  The state S_n after sweep n is covered by two kernels: the BLACK half-sweep
+// of sweep n ends with K(x) of the updated links in the registers of its (BLACK) sites, and the RED half-sweep of
+// sweep n + 1 builds K(x) of its (RED) sites from the links of S_n before it updates them.  Both write one partial of
+// sum_x tr[Delta Delta^dagger] per block (post / pre); every link passes through registers once per half-sweep (C6),
+// so BLACK_n also writes the partials of F(S_n).  The first blocks of BLACK_{n+1} then reduce these partials in a
+// fixed order (no atomics on data: deterministic) and the last of them to finish forms theta(S_n), F(S_n), compares
+// with the tolerance and raises `stop` / freezes timeslices, which takes effect from RED_{n+2}: the fixing loop ends
+// one sweep after the sweep that met the tolerance, without a separate pass over the field and without a host sync.
+struct SweepMonitor {
+    double* F_part;           // [blocks] this launch writes: sum of Re tr of the links it stores, mu < nd (NULL: not)
+    double* post_part;        // [blocks] this launch writes: sum tr[Delta Delta^dagger] from the final K (NULL: not)
+    double* pre_part;         // [blocks] this launch writes: the same from the initial K (NULL: not)
+    const double* red_F;      // reduction duty (all three NULL: none): partials of F(S_n), written by BLACK_n
+    const double* red_post;   //   of the BLACK sites of S_n, written by BLACK_n
+    const double* red_pre;    //   of the RED sites of S_n, written by RED_{n+1}
+    double* group;            // [3][Nt][groups] scratch of the duty
+    double* theta_t;          // [Nt] per-timeslice theta of the last check (Coulomb)
+    int* frozen_from;         // [Nt] slices mode: first sweep (1-based) in which the slice is not updated (INT_MAX: open)
+    MonitorState* state;
+    int sweep;                // 1-based index of the sweep this launch belongs to
+    int check_sweep;          // n of the duty
+    int groups;               // duty blocks per timeslice
+    int blocks_per_slice;     // partials per timeslice
+    int slices;               // != 0: freeze single timeslices (gf_fix_slices), else one stop word
+    int coulomb;              // theta = max over timeslices
+    int zero;                 // 0 (a value the compiler cannot know: ties the stop test to the link loads)
+    double tol;
+    double scale_theta_t, scale_theta, scale_F; // 1/(3 Vs), 1/(3 V), 1/(3 nd V)
+};
+
 struct SweepParams {
     void* U;        // native field
     Lattice L;
@@ -58,6 +103,7 @@ struct SweepParams {
     int* rough;                // CHAIN_HYBRID: ring of ROUGH_RING flags, one per half-sweep
     unsigned long long* dc_count; // diagnostic: [0] launches that ran the double chain, [1] sites redone in double
     SweepPhase ph;
+    SweepMonitor mon;          // MON kernels only
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -374,6 +420,9 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
     if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
 }
 
+__device__ __forceinline__ int tie_bits(float x) { return __float_as_int(x); }
+__device__ __forceinline__ int tie_bits(double x) { return __double2hiint(x); }
+
 // ---------------------------------------------------------------------------------------------------------
 // the half-sweep kernel
 // ---------------------------------------------------------------------------------------------------------
@@ -390,20 +439,23 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
 // start that breaks north_star's 5e-5 per link at ~1e-5 of the sites; a per-site repair cannot help the BLACK sites
 // (their error is in their input).  So the chain runs in double (CT = double: K accumulated exactly from the fp32
 // links, G rounded to fp32 once) while the field is rough, and in fp32 once it is smooth: every half-sweep records
-// whether any of its steps had a conditioning number |k|^2 |h|^2 below watch_thr2 (rough[slot]), and a half-sweep
-// takes the double chain iff one of the two half-sweeps before it was rough (or the host forces it: the first sweep
-// of every call).  The decision is a deterministic function of the field; on a nearly fixed field (|k| ~ 10, |h| ~ 1)
+// whether any of its steps had a conditioning number |k|^2 |h|^2 below watch_thr2, and a half-sweep takes the
+// double chain iff one of the two half-sweeps before it was rough (or the host forces it: the first sweep of every
+// call).  The decision is a deterministic function of the field; on a nearly fixed field (|k| ~ 10, |h| ~ 1)
 // no launch takes the double chain.  The heatbath kernels keep the fp32 chain and repair single sites instead
 // (fixup_site_f64 above).
 // DC (fp32 heatbath kernels only): the double chain at every site, for annealing runs in which every link has to meet
 // the per-link bound (gf_set_chain(ctx, 1, ..)); the default heatbath kernel keeps the fp32 chain.
-template <typename T, int R, int TPS, int MODE, bool CB = false, bool DC = false>
+// MON (relaxation kernels only): fused F / theta monitor, SweepMonitor above.  0: none; 1: the launch only honours the
+// stop / the frozen timeslices (the sweeps between two checks); 2: it also writes partials and / or has the duty.
+template <typename T, int R, int TPS, int MODE, bool CB = false, bool DC = false, int MON = 0>
 struct SweepKernel {
     static constexpr int NMU = 4 / TPS;
     static constexpr bool FP32 = sizeof(T) == 4;
     static constexpr bool HYB = FP32 && MODE != MODE_HEATBATH;        // relaxation sweeps: chain type chosen per launch
     static constexpr bool FIX = FP32 && MODE == MODE_HEATBATH && !DC; // heatbath: fp32 chain, weak sites redone in double
     static_assert(!DC || (FP32 && MODE == MODE_HEATBATH), "DC is a variant of the fp32 heatbath kernel");
+    static_assert(MON == 0 || MODE != MODE_HEATBATH, "the monitor belongs to the relaxation sweeps");
     using IO = LinkIO<T, R>;
     using GIO = LinkIO<T, 18>;
 
@@ -443,10 +495,12 @@ struct SweepKernel {
 
     // the site chain on the type CT: K(x) from the loaded links, then the three subgroup steps (each applies its G to
     // the links at once, Alg. 1's data flow, C8)
+    // mon_skip (MON): the launch is past its stop or the timeslice is frozen; returns false if nothing was updated
     template <typename CT>
-    static __device__ __forceinline__ void chain(const SweepParams& p, const SweepPhase& ph, cx<T> (&F)[NMU][9],
+    static __device__ __forceinline__ bool chain(const SweepParams& p, const SweepPhase& ph, cx<T> (&F)[NMU][9],
                                                  cx<T> (&B)[NMU][9], cx<T> (&Gt)[9], uint32_t sc,
-                                                 const EarlyRandom (&early)[3], int lane_mu0, unsigned mask, bool& watch)
+                                                 const EarlyRandom (&early)[3], int lane_mu0, unsigned mask, bool& watch,
+                                                 double& th_pre, double& th_post, int mon_skip)
     {
         // K(x) = sum_{mu < nd} [ U_mu(x) + U_mu(x-mu)^dagger ]   (eq. 2.3; C2)
         cx<CT> K[9];
@@ -474,10 +528,124 @@ struct SweepKernel {
                 }
             }
         }
+        if (MON) {
+            // The test is tied to K (zero is 0, but only the host knows), i.e. to every link load having been issued and
+            // answered -- which the first subgroup step needs anyway.  A test on the flag alone is moved ahead of the link
+            // loads by ptxas (it sinks them below the branch), and every block then waits for the flag before it asks
+            // for its links: +15 % on the whole sweep.
+            mon_skip |= tie_bits(K[0].re) & p.mon.zero;
+            if (mon_skip) return false;
+        }
         const bool record = lane_mu0 == 0;
+        if (MON == 2 && p.mon.pre_part != nullptr) th_pre = record ? site_theta(K) : 0.0;
         subgroup<CT, 0, 1, 0>(p, ph, K, F, B, sc, record, early[0], lane_mu0, Gt, watch); // Cabibbo-Marinari subgroups, order of C4
         subgroup<CT, 0, 2, 1>(p, ph, K, F, B, sc, record, early[1], lane_mu0, Gt, watch);
         subgroup<CT, 1, 2, 2>(p, ph, K, F, B, sc, record, early[2], lane_mu0, Gt, watch);
+        if (MON == 2 && p.mon.post_part != nullptr) th_post = record ? site_theta(K) : 0.0;
+        return true;
+    }
+
+    // tr[Delta Delta^dagger] at one site from its K (eq. 2.5; C3): Delta = traceless part of (K - K^dagger)/(2i)
+    template <typename CT>
+    static __device__ __forceinline__ double site_theta(const cx<CT> (&K)[9])
+    {
+        const CT tr3 = (K[0].im + K[4].im + K[8].im) * CT(1.0 / 3.0);
+        CT acc = CT(0);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const CT d = K[4 * a].im - tr3;
+            acc += d * d;
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = a + 1; b < 3; ++b) {
+                const CT dr = CT(0.5) * (K[3 * a + b].im + K[3 * b + a].im);
+                const CT di = CT(0.5) * (K[3 * a + b].re - K[3 * b + a].re);
+                acc += CT(2) * (dr * dr + di * di); // Delta is Hermitian: |D_ab|^2 = |D_ba|^2
+            }
+        return (double)acc;
+    }
+
+    // sum over the block; the result is valid in thread 0.  Fixed tree: deterministic.
+    static __device__ __forceinline__ double block_sum(double v, double* smem)
+    {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+        if (blockDim.x <= 32) return v;
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) smem[threadIdx.x >> 5] = v;
+        __syncthreads();
+        double acc = 0.0;
+        if (threadIdx.x == 0)
+            for (unsigned w = 0; w < (blockDim.x + 31) / 32; ++w) acc += smem[w];
+        return acc;
+    }
+
+    // The reduction duty of a BLACK half-sweep (SweepMonitor): duty block j = (t, g) adds its share of the partials
+    // of timeslice t, the last block to deliver adds the groups, forms theta and F of S_n and decides.
+    static __device__ __noinline__ void monitor_duty(const SweepMonitor& m, int Nt, unsigned j)
+    {
+        __shared__ double smem[3][MAX_BLOCK / 32];
+        __shared__ unsigned last;
+        const int t = (int)j / m.groups, g = (int)j % m.groups;
+        const int chunk = (m.blocks_per_slice + m.groups - 1) / m.groups;
+        const int i0 = g * chunk, i1 = min(i0 + chunk, m.blocks_per_slice);
+        double f = 0.0, po = 0.0, pr = 0.0;
+        if (!(m.slices && m.frozen_from[t] <= m.check_sweep + 1)) { // the slice was still updated in sweep n + 1
+            const size_t base = (size_t)t * m.blocks_per_slice;
+            for (int i = i0 + (int)threadIdx.x; i < i1; i += (int)blockDim.x) {
+                f += m.red_F[base + i];
+                po += m.red_post[base + i];
+                pr += m.red_pre[base + i];
+            }
+        }
+        f = block_sum(f, smem[0]);
+        po = block_sum(po, smem[1]);
+        pr = block_sum(pr, smem[2]);
+        if (threadIdx.x == 0) {
+            double* grp = m.group + ((size_t)t * m.groups + g) * 3;
+            grp[0] = f; grp[1] = po; grp[2] = pr;
+            __threadfence();
+            last = atomicAdd(&m.state->ticket, 1u) == (unsigned)(Nt * m.groups) - 1u;
+        }
+        __syncthreads();
+        if (!last) return;
+        __threadfence();
+        // per-timeslice sums in a fixed order (thread t', t' + blockDim, ...), kept in theta_t / group[..][0]
+        for (int tt = (int)threadIdx.x; tt < Nt; tt += (int)blockDim.x) {
+            if (m.slices && m.frozen_from[tt] <= m.check_sweep + 1) continue; // a frozen slice keeps its last values
+            const volatile double* grp = m.group + (size_t)tt * m.groups * 3;
+            double ft = 0.0, tht = 0.0;
+            for (int gg = 0; gg < m.groups; ++gg) { ft += grp[3 * gg]; tht += grp[3 * gg + 1] + grp[3 * gg + 2]; }
+            m.theta_t[tt] = tht * m.scale_theta_t;
+            m.theta_t[Nt + tt] = ft; // raw F of the slice
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double sum_th = 0.0, max_th = 0.0, sum_F = 0.0;
+            int active = 0;
+            for (int tt = 0; tt < Nt; ++tt) {
+                const double th = m.theta_t[tt];
+                sum_th += th;
+                if (tt == 0 || th > max_th) max_th = th;
+                sum_F += m.theta_t[Nt + tt];
+                if (m.slices) {
+                    if (m.frozen_from[tt] == INT_MAX && th < m.tol) m.frozen_from[tt] = m.check_sweep + 2;
+                    active += m.frozen_from[tt] == INT_MAX ? 1 : 0;
+                }
+            }
+            MonitorState* st = m.state;
+            st->theta = m.coulomb ? max_th : sum_th / (double)Nt; // slices of equal volume: the mean of theta_t is theta
+            st->F = sum_F * m.scale_F;
+            st->check_sweep = m.check_sweep;
+            st->checks += 1;
+            st->any_active = active;
+            const bool done = m.slices ? active == 0 : st->theta < m.tol;
+            if (done && st->stop_from == INT_MAX) { st->stop_sweep = m.check_sweep; st->stop_from = m.check_sweep + 2; }
+            st->ticket = 0u;
+            __threadfence();
+        }
     }
 
     // L2 prefetch for the block that runs `prefetch` sites further along the traversal: the few fat warps of
@@ -507,8 +675,11 @@ struct SweepKernel {
     // share it; this thread owns the directions lane_mu0 .. lane_mu0 + NMU - 1.  `mask`: the lanes of the warp that
     // run this call together (whole sites: TPS divides 32).  `first`: first site update of this thread in the launch
     // (the one-shot kernel: always; it waits for the previous grid there)
+    // mon_skip (MON): the launch is past its stop, or the site's timeslice is frozen: nothing is updated.  The words
+    // are read by the caller ahead of the link loads and tested behind them, so that the test costs no latency.
     static __device__ __forceinline__ void site_update(const SweepParams& p, const SweepPhase& ph, unsigned slot,
-                                                       int lane_mu0, unsigned mask, bool first)
+                                                       int lane_mu0, unsigned mask, bool first, const int* mon_stop,
+                                                       const int* mon_frozen, double (&mon_out)[3])
     {
         const Site s = decode_site(p.L, slot, ph.parity);
         const size_t H = p.L.H;
@@ -528,12 +699,15 @@ struct SweepKernel {
         }
         // fp32 relaxation sweeps, hybrid chain: were the two half-sweeps before this one rough?  Two L2 hits, issued
         // ahead of the link loads so that the choice is there when the first link arrives
-        int rough_a = 0, rough_b = 0;
-        if (HYB && p.chain == CHAIN_HYBRID && !ph.rough_force) {
-            const volatile int* rough = p.rough;
-            rough_a = rough[(ph.rough_slot + ROUGH_RING - 1) % ROUGH_RING];
-            rough_b = rough[(ph.rough_slot + ROUGH_RING - 2) % ROUGH_RING];
+        int rough_now = 0;
+        if (HYB && p.chain == CHAIN_HYBRID && !ph.rough_force) rough_now = *((const volatile int*)p.rough + ph.rough_slot);
+        int mon_skip = 0;
+#ifndef GF_EXP_MON_NOFLAG
+        if (MON) { // written by earlier launches only (stamped): plain L2 loads
+            mon_skip = p.mon.sweep >= __ldcg(mon_stop);
+            if (mon_frozen != nullptr) mon_skip |= p.mon.sweep >= __ldcg(mon_frozen);
         }
+#endif
         // the relaxation kernels prefetch before their loads (placed after them the fp64 kernel spills twice as
         // much); the heatbath kernel issues its loads first and hides the prefetch and the generator behind them
         if (MODE != MODE_HEATBATH) issue_prefetch(p, ph, s, hb, lane_mu0, base, H);
@@ -573,21 +747,30 @@ struct SweepKernel {
             if (owns_t) reunitarise(Gt);
         }
 
+        double th_pre = 0.0, th_post = 0.0;
         bool watch = false; // fp32: some step of this site had a small conditioning number
         if constexpr (HYB) {
-            const bool dchain = p.chain == CHAIN_DOUBLE || (p.chain == CHAIN_HYBRID && (ph.rough_force | rough_a | rough_b) != 0);
-            if (dchain) chain<double>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch);
-            else chain<float>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch);
+            const bool dchain = p.chain == CHAIN_DOUBLE || (p.chain == CHAIN_HYBRID && (ph.rough_force | rough_now) != 0);
+            const bool updated = dchain ? chain<double>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch, th_pre, th_post, mon_skip)
+                                        : chain<float>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch, th_pre, th_post, mon_skip);
+            if (MON && !updated) return;
             if (p.chain == CHAIN_HYBRID) {
-                if (watch) p.rough[ph.rough_slot] = 1; // same value from every writer
+                // ring of flags, rough[s] = "half-sweep s runs the double chain": a rough half-sweep marks the next two;
+                // the slot three ahead was read by the previous half-sweep and is written by the next two: clear it
+                if (watch) { // same value from every writer
+                    p.rough[(ph.rough_slot + 1) % ROUGH_RING] = 1;
+                    p.rough[(ph.rough_slot + 2) % ROUGH_RING] = 1;
+                }
                 if (slot == p.h_begin && lane_mu0 == 0) {
-                    p.rough[(ph.rough_slot + 1) % ROUGH_RING] = 0; // read by the previous launch, written by the next
+                    p.rough[(ph.rough_slot + 3) % ROUGH_RING] = 0;
                     if (dchain && p.dc_count != nullptr) atomicAdd(p.dc_count, 1ull);
                 }
             }
         } else {
-            (void)rough_a; (void)rough_b;
-            chain<typename std::conditional<DC, double, T>::type>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch);
+            (void)rough_now;
+            const bool updated = chain<typename std::conditional<DC, double, T>::type>(p, ph, F, B, Gt, sc, early, lane_mu0, mask, watch,
+                                                                                        th_pre, th_post, mon_skip);
+            if (MON && !updated) return;
             if constexpr (FIX) {
                 if (watch) {
                     fixup_site_f64<R, TPS, MODE, CB>(p, ph, slot, lane_mu0); // stores the links itself
@@ -596,6 +779,18 @@ struct SweepKernel {
             }
         }
 
+        if (MON == 2) {
+            mon_out[1] = th_post;
+            mon_out[2] = th_pre;
+            if (p.mon.F_part != nullptr) { // eq. 2.1 (C1) on the links this thread stores
+                T f = T(0);
+#pragma unroll
+                for (int m = 0; m < NMU; ++m)
+                    if (lane_mu0 + m < p.nd && !(CB && lane_mu0 + m == 3))
+                        f += (F[m][0].re + F[m][4].re + F[m][8].re) + (B[m][0].re + B[m][4].re + B[m][8].re);
+                mon_out[0] = (double)f;
+            }
+        }
 #pragma unroll
         for (int m = 0; m < NMU; ++m) {
             const int mu = lane_mu0 + m;
@@ -610,10 +805,41 @@ struct SweepKernel {
     {
         const unsigned blk = p.ph.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
         const unsigned gtid = blk * blockDim.x + threadIdx.x;
-        // threads past the range leave at once: they come in whole sites (TPS divides 32), and exited threads may be
-        // named in the mask of the shuffles that combine K
-        if (gtid / TPS >= p.h_count) return;
-        site_update(p, p.ph, p.h_begin + gtid / TPS, (int)(gtid % TPS) * NMU, 0xffffffffu, true);
+        double mon_out[3] = {0.0, 0.0, 0.0};
+        if (!MON) {
+            // threads past the range leave at once: they come in whole sites (TPS divides 32), and exited threads may be
+            // named in the mask of the shuffles that combine K
+            if (gtid / TPS >= p.h_count) return;
+            site_update(p, p.ph, p.h_begin + gtid / TPS, (int)(gtid % TPS) * NMU, 0xffffffffu, true, nullptr, nullptr, mon_out);
+            return;
+        }
+        // monitored launch: the host launches it only where the threads of a timeslice fill whole blocks, so every
+        // thread has a site and a block lies inside one timeslice -- no range test, the control flow stays uniform
+        const unsigned slot = p.h_begin + gtid / TPS;
+        const int* fr = nullptr;
+        if (p.mon.slices) fr = p.mon.frozen_from + slot / (p.L.H / (unsigned)p.L.Nt);
+        site_update(p, p.ph, slot, (int)(gtid % TPS) * NMU, 0xffffffffu, true, &p.mon.state->stop_from, fr, mon_out);
+        if (MON < 2) return;
+        if (p.mon.F_part != nullptr || p.mon.post_part != nullptr || p.mon.pre_part != nullptr) {
+            __shared__ double smem[3][MAX_BLOCK / 32];
+            const unsigned part = (p.h_begin * TPS) / blockDim.x + blk; // index of this block's partials: its place in the lattice
+            if (p.mon.F_part != nullptr) {
+                const double v = block_sum(mon_out[0], smem[0]);
+                if (threadIdx.x == 0) p.mon.F_part[part] = v;
+            }
+            if (p.mon.post_part != nullptr) {
+                const double v = block_sum(mon_out[1], smem[1]);
+                if (threadIdx.x == 0) p.mon.post_part[part] = v;
+            }
+            if (p.mon.pre_part != nullptr) {
+                const double v = block_sum(mon_out[2], smem[2]);
+                if (threadIdx.x == 0) p.mon.pre_part[part] = v;
+            }
+        }
+#ifndef GF_EXP_MON_NODUTY
+        if (p.mon.red_post != nullptr && blockIdx.x < (unsigned)(p.L.Nt * p.mon.groups) && p.mon.sweep < __ldcg(&p.mon.state->stop_from))
+            monitor_duty(p.mon, p.L.Nt, blockIdx.x);
+#endif
     }
 };
 
@@ -637,10 +863,10 @@ constexpr int sweep_max_registers()
     return 255;
 }
 
-template <typename T, int R, int TPS, int MODE, bool CB = false, bool DC = false>
+template <typename T, int R, int TPS, int MODE, bool CB = false, bool DC = false, int MON = 0>
 __global__ void __maxnreg__((sweep_max_registers<T, R, TPS, MODE, CB>())) gf_half_sweep_kernel(const __grid_constant__ SweepParams p)
 {
-    SweepKernel<T, R, TPS, MODE, CB, DC>::run(p);
+    SweepKernel<T, R, TPS, MODE, CB, DC, MON>::run(p);
 }
 
 } // namespace gf

@@ -414,3 +414,121 @@ def test_no_write_outside_the_field(gfm, precision, R, gauge):
     assert bool(torch.isnan(cbuf[:8192]).all()) and bool(torch.isnan(cbuf[8192 + V * 72:]).all())
     assert not bool(torch.isnan(canon).any())
     gfm.gf_destroy(ctx)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# fused F / theta monitor of the fixing loops (C21)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,gauge,R", [("fp64", "landau", 18), ("fp64", "coulomb", 18), ("fp64", "landau", 12),
+                                               ("fp32", "landau", 18), ("fp32", "coulomb", 18)])
+def test_fused_monitor_values_match_the_oracle(gfm, precision, gauge, R):
+    """theta, theta_t and F that the sweep kernels accumulate for the state after sweep n are those of orc_theta /
+    orc_functional on that state: fp64 theta 1e-6 (measured 1e-12), F 1e-10; fp32 within its storage rounding"""
+    dims = (8, 8, 8, 8)  # (V_s / 2) * threads per site divisible by the 32-thread block: the fused form applies
+    U = gf_inputs.smooth_random(dims, 0.4, 61)
+    og = ORC_GAUGE[gauge]
+    fx = gfm.GaugeFixer(dims, precision=precision, gauge=gauge, reals_per_link=R)
+    fx.load(U)
+    # a tolerance out of reach in 9 sweeps (fp32: the smallest the fused form takes); checks after sweeps 3 and 6 (none
+    # at the last allowed sweep 9: it needs sweep 10)
+    n, th_end, F_end = fx.fix(0.0 if precision == "fp64" else 1e-10, gfm.GF_UPDATE_OVERRELAX2, 1.7, check_every=3, max_sweeps=9)
+    assert n == 9
+    k, th, F, th_t = gfm.gf_monitor_last(fx.ctx, dims[3])
+    assert k == 6
+    ref = U.copy()
+    oracle.overrelax(ref, dims, 1.7, 6, og)
+    tol_th, tol_F = (1e-6, 1e-10) if precision == "fp64" else (2e-3, 1e-5)
+    assert th == pytest.approx(oracle.theta(ref, dims, og), rel=tol_th)
+    assert F == pytest.approx(oracle.functional(ref, dims, og), rel=tol_F)
+    if gauge == "coulomb":
+        np.testing.assert_allclose(th_t, oracle.theta_slices(ref, dims, og), rtol=tol_th)
+    oracle.overrelax(ref, dims, 1.7, 3, og)
+    assert th_end == pytest.approx(oracle.theta(ref, dims, og), rel=1e-6 if precision == "fp64" else 2e-2)
+    assert F_end == pytest.approx(oracle.functional(ref, dims, og), rel=tol_F)
+    assert np.abs(fx.download() - ref).max() <= (1e-11 if precision == "fp64" else 3e-4)
+    fx.close()
+
+
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+@pytest.mark.parametrize("every", [1, 7])
+def test_fused_fix_loop_matches_oracle_with_lag_one(gfm, gauge, every):
+    """gf_fix with the fused monitor ends one sweep after the check that met the tolerance (orc_fix_lag, lag = 1);
+    the separate check kernel (gf_set_monitor 0) is the paper's loop (lag = 0); bit-identical fields between the fused
+    loop and plain sweeping for the same number of sweeps"""
+    dims = (8, 8, 8, 8)
+    U = gf_inputs.smooth_random(dims, 0.3, 62)
+    og = ORC_GAUGE[gauge]
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge=gauge)
+    fx.load(U)
+    n, th, F = fx.fix(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=every, max_sweeps=3000)
+    ref = U.copy()
+    n_ref, th_ref, F_ref = oracle.fix(ref, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-9, every, 3000, 0, og, lag=1)
+    assert n == n_ref and 0 < n < 3000
+    assert th == pytest.approx(th_ref, rel=1e-5) and F == pytest.approx(F_ref, rel=1e-10)
+    got = fx.download()
+    assert np.abs(got - ref).max() < 1e-9
+    assert fx.fix(1e-9, check_every=every)[0] == 0  # already fixed: no sweep
+    fx.load(U)
+    fx.overrelax(1.6, n)
+    assert np.array_equal(fx.download(), got)  # the monitor changes no link
+    gfm.gf_set_monitor(fx.ctx, 0)
+    fx.load(U)
+    n0 = fx.fix(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=every, max_sweeps=3000)[0]
+    ref = U.copy()
+    assert n0 == oracle.fix(ref, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-9, every, 3000, 0, og, lag=0)[0] == n - 1
+    # cut by max_sweeps: the check at the last allowed sweep cannot take place
+    gfm.gf_set_monitor(fx.ctx, 1)
+    fx.load(U)
+    assert fx.fix(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=every, max_sweeps=n - 1)[0] == n - 1
+    fx.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_fused_fix_slices_matches_oracle_with_lag_one(gfm, precision):
+    """Coulomb gauge, per-timeslice stop rule with the fused monitor: a slice found below the tolerance after sweep n is
+    frozen from sweep n + 2 on (orc_fix_slices_lag, lag = 1); with check_every = 1 every slice stops within one sweep of
+    meeting the tolerance"""
+    dims = (8, 8, 8, 6)
+    U = gf_inputs.smooth_random(dims, 0.5, 63)
+    fx = gfm.GaugeFixer(dims, precision=precision, gauge="coulomb")
+    fx.load(U)
+    tol = 1e-9 if precision == "fp64" else 1e-8
+    n, th, F, per = fx.fix_slices(tol, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=1, max_sweeps=3000)
+    ref = U.copy()
+    n_ref, th_ref, F_ref, per_ref = oracle.fix_slices(ref, dims, oracle.UPDATE_OVERRELAX2, 1.5, tol, 1, 3000, lag=1)
+    sl = fx.theta_slices()
+    assert max(sl) < tol and n == max(per) and len(set(per)) > 1
+    if precision == "fp64":
+        assert per == per_ref.tolist() and n == n_ref
+        assert th == pytest.approx(th_ref, rel=1e-5) and F == pytest.approx(F_ref, rel=1e-10)
+        assert np.abs(fx.download() - ref).max() < 1e-9
+        ref0 = U.copy()
+        per0 = oracle.fix_slices(ref0, dims, oracle.UPDATE_OVERRELAX2, 1.5, tol, 1, 3000, lag=0)[3]
+        assert per == (per0 + 1).tolist()  # one sweep past the crossing, per slice
+    else:
+        assert np.abs(np.array(per) - per_ref).max() <= 3 and F == pytest.approx(F_ref, rel=1e-5)
+    assert fx.fix_slices(tol, check_every=1)[0] == 0
+    fx.close()
+
+
+def test_fused_monitor_stochastic_and_fallback(gfm):
+    """the variants run under the monitor too (stochastic relaxation: decisions continue through the loop, C18); a
+    lattice whose blocks straddle timeslices falls back to the separate check (lag 0)"""
+    dims = (8, 8, 8, 4)
+    U = gf_inputs.smooth_random(dims, 0.3, 64)
+    fx = gfm.GaugeFixer(dims, precision="fp64")
+    fx.load(U)
+    n, th, F = fx.fix(1e-8, gfm.GF_UPDATE_STOCHASTIC, 0.5, check_every=2, max_sweeps=3000, seed=5)
+    ref = U.copy()
+    n_ref, th_ref, F_ref = oracle.fix(ref, dims, oracle.UPDATE_STOCHASTIC, 0.5, 1e-8, 2, 3000, 5, lag=1)
+    assert n == n_ref and F == pytest.approx(F_ref, rel=1e-10) and np.abs(fx.download() - ref).max() < 1e-9
+    fx.close()
+    dims = (6, 6, 6, 4)  # V_s / 2 = 108 sites, two threads per site: 216 threads do not fill 32-thread blocks evenly
+    U = gf_inputs.smooth_random(dims, 0.3, 54)
+    fx = gfm.GaugeFixer(dims, precision="fp64")
+    fx.load(U)
+    n = fx.fix(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=3, max_sweeps=2000)[0]
+    assert n == oracle.fix(U, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-9, 3, 2000, lag=0)[0]
+    with pytest.raises(gfm.GFError):
+        gfm.gf_monitor_last(fx.ctx, 4)
+    fx.close()

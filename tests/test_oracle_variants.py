@@ -236,3 +236,87 @@ def test_heatbath_half_is_the_annealing_half_sweep():
     assert (np.abs(b - U0).reshape(V * 4, -1).max(axis=1) > 1e-6).all()
     oracle.heatbath_half(b, dims, 0.9, 7, 0, 1, trials=tb)
     assert np.array_equal(a, b) and np.array_equal(ta, tb)
+
+
+def test_fix_lag_one_stops_one_sweep_after_the_check():
+    """C21: orc_fix_lag(lag = 1) ends one sweep after the first checked sweep below the tolerance; its field is plain
+    sweeping for that many sweeps; lag = 0 is orc_fix; no check takes place at the last allowed sweep (lag = 1)"""
+    dims = (4, 4, 4, 4)
+    U0 = gf_inputs.smooth_random(dims, 0.3, 46)
+    tol = 1e-8
+    scan, th = U0.copy(), []
+    for n in range(1, 400):
+        oracle.overrelax(scan, dims, 1.6, 1)
+        th.append(oracle.theta(scan, dims))
+        if th[-1] < 1e-10:
+            break
+    for every in (1, 3, 10):
+        first = next(n for n in range(every, len(th) + 1, every) if th[n - 1] < tol)  # first checked sweep below tol
+        for lag in (0, 1):
+            V = U0.copy()
+            n, thn, F = oracle.fix(V, dims, oracle.UPDATE_OVERRELAX2, 1.6, tol, every, 1000, lag=lag)
+            assert n == first + lag, (every, lag)
+            W = U0.copy()
+            oracle.overrelax(W, dims, 1.6, n)
+            assert np.array_equal(V, W)
+            assert thn == oracle.theta(W, dims) and F == oracle.functional(W, dims)
+        V = U0.copy()  # the check at sweep `first` cannot take place if that is the last allowed sweep
+        assert oracle.fix(V, dims, oracle.UPDATE_OVERRELAX2, 1.6, tol, every, first, lag=1)[0] == first
+        V = U0.copy()
+        assert oracle.fix(V, dims, oracle.UPDATE_OVERRELAX2, 1.6, tol, every, first + 5, lag=1)[0] == first + 1
+    assert oracle.fix(scan, dims, oracle.UPDATE_OVERRELAX2, 1.6, tol, 1, 50, lag=1)[0] == 0  # already fixed
+
+
+def test_fix_slices_lag():
+    """orc_fix_slices_lag: lag = 0 is orc_fix_slices (sweep by sweep instead of chunk by chunk); lag = 1 gives every
+    slice exactly one more sweep than lag = 0 at check_every = 1 (unless it was fixed from the start)"""
+    dims = (4, 4, 4, 6)
+    U0 = gf_inputs.smooth_random(dims, 0.5, 47)
+    a, b = U0.copy(), U0.copy()
+    na, tha, Fa, pa = oracle.fix_slices(a, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 4, 3000)
+    lib = oracle._load()
+    import ctypes
+    N, V = oracle._dims(dims)
+    th, F = ctypes.c_double(), ctypes.c_double()
+    per = np.zeros(dims[3], dtype=np.int32)
+    nb = lib.orc_fix_slices_lag(N, oracle.COULOMB, b.ctypes.data, 0, 1.5, 1e-9, 4, 3000, 0, 0, per.ctypes.data,
+                                ctypes.byref(th), ctypes.byref(F))
+    assert nb == na and np.array_equal(per, pa) and np.array_equal(a, b) and th.value == tha
+    c, d = U0.copy(), U0.copy()
+    n0, _, _, p0 = oracle.fix_slices(c, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 1, 3000, lag=0)
+    n1, th1, _, p1 = oracle.fix_slices(d, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 1, 3000, lag=1)
+    assert np.array_equal(p1, p0 + 1) and n1 == n0 + 1 and th1 < 1e-9
+
+
+def test_black_sites_keep_K_of_the_finished_sweep_in_the_chain():
+    """What the fused monitor rests on (C21): after its three subgroup steps the K <- G K chain of a BLACK site IS
+    K(x) of the state after the sweep -- no later update of the half-sweep touches its links (C6) -- so
+    sum over BLACK sites of tr[Delta Delta^dagger] from the chain plus the sum over RED sites from K built before
+    the next sweep's RED update equals orc_theta of the state in between."""
+    dims = (4, 4, 2, 4)
+    V = int(np.prod(dims))
+    U = gf_inputs.smooth_random(dims, 0.4, 48)
+    omega = 1.7
+    oracle.overrelax_half(U, dims, omega, 0)
+    before_black = U.copy()
+    oracle.overrelax_half(U, dims, omega, 1)  # U is now S_1
+    s = np.arange(V)
+    par = (s % 4 + (s // 4) % 4 + (s // 16) % 2 + s // 32) & 1
+
+    def delta2(K):
+        D = (K - K.conj().T) / 2j
+        D = D - np.trace(D) / 3 * np.eye(3)
+        return float((np.abs(D) ** 2).sum())
+
+    total = 0.0
+    for x in range(V):
+        if par[x] == 1:  # the chain of the BLACK update, restated with the oracle's pieces on the state before it
+            K = oracle.build_K(before_black, dims, x)
+            for i, j in ((0, 1), (0, 2), (1, 2)):
+                g = oracle.su2_maximiser(oracle.su2_project(K, i, j))
+                K = oracle.su2_embed(oracle.su2_overrelax(g, omega), i, j) @ K
+            assert delta2(K) == pytest.approx(oracle.site_theta(U, dims, x), rel=1e-9, abs=1e-26)
+            total += delta2(K)
+        else:            # what the RED half-sweep of the next sweep builds before it updates
+            total += delta2(oracle.build_K(U, dims, x))
+    assert total / (3 * V) == pytest.approx(oracle.theta(U, dims), rel=1e-12)
