@@ -158,6 +158,45 @@ int gf_fix_slices(gf_ctx* ctx, void* U_native_dev, int update, double param, dou
                   int max_sweeps, unsigned long long seed, int* sweeps_done, int* sweeps_per_slice,
                   double* theta_host, double* F_host, void* stream);
 
+/* ---- one configuration sharded over several contexts: t-slabs ("future multi-GPU") --- */
+
+/* A context that owns the timeslices [t_begin, t_end) of an Nx*Ny*Nz*Nt_global lattice.  Its native field
+ * (gf_field_bytes) holds the owned slices followed by ONE ghost slice: a copy of the temporal links U_t(x, t_begin - 1)
+ * of the slab below (periodic: the last slab for the first), the only links a site update of this slab shares with
+ * another slab (as U_t(x - t) of its first slice, read for K(x) and multiplied by g(x)^dagger).  gf_pack / gf_unpack
+ * exchange the owned slices only (canonical: the (t_end - t_begin) slices, local t); Nt-sized outputs (gf_theta_slices,
+ * gf_fix_slices) have t_end - t_begin entries; gf_functional / gf_theta are those of the owned sites (gf_theta needs
+ * a current ghost); the Philox counters carry the site of the WHOLE lattice, so a sharded run takes the decisions of
+ * the unsharded one.  Not available on a slab: Coulomb reading B, the fused monitor, the host-buffer path.
+ * GF_EINVAL: t_begin or t_end odd (the local checkerboard must be the global one), fewer than 2 slices, bounds
+ * outside [0, Nt_global]; otherwise as gf_create. */
+int gf_create_slab(gf_ctx** out, int Nx, int Ny, int Nz, int Nt_global, int t_begin, int t_end, int precision, int gauge);
+/* Bytes of one face message: the temporal links of one parity block of one timeslice, (Nx Ny Nz / 2) * reals_per_link *
+ * sizeof(real).  Per half-sweep one such message crosses every slab boundary in each direction. */
+size_t gf_slab_face_bytes(const gf_ctx* ctx);
+/* Gather / scatter a face between the native field and a contiguous device buffer of gf_slab_face_bytes.
+ * which = 0: the last owned slice; which = 1: the ghost slice.  block_parity: parity of the sites the links start at.
+ * Protocol of a half-sweep of parity p on slab r (block_parity = 1 - p throughout): pack(r-1, which 0) -> message ->
+ * unpack(r, which 1); half-sweep; pack(r, which 1) -> message -> unpack(r-1, which 0).  GF_EINVAL on a plain context. */
+int gf_slab_pack_face(gf_ctx* ctx, const void* U_native_dev, int which, int block_parity, void* buf_dev, void* stream);
+int gf_slab_unpack_face(gf_ctx* ctx, void* U_native_dev, int which, int block_parity, const void* buf_dev, void* stream);
+/* One half-sweep (Alg. 1's inner "for all x of sublattice") of parity 0 (RED) / 1 (BLACK) on the owned
+ * timeslices [t_first, t_first + t_count) -- any context; what a driver interleaves with the face exchange (first
+ * slice, interior).  `sweep` (>= 0): index of the sweep within the driver's loop: the counter of the stochastic
+ * decisions (C18), of the re-orthonormalisation cadence (C15) and of the hybrid chain; gf_begin_sweeps starts such a
+ * loop (what the start of gf_relax does: fp32 contexts forget the roughness of whatever ran before, the first sweep
+ * runs the double chain).  update / param / seed as gf_relax.  Coulomb contexts run reading
+ * A here.  gf_anneal_half: the same for one heatbath half-sweep at temperature T, `step` the annealing step (C13/C14).
+ * GF_EINVAL: bad parity, sweep < 0, timeslices outside the owned range, parameter out of range, reading B forced. */
+int gf_begin_sweeps(gf_ctx* ctx, void* stream);
+int gf_relax_half(gf_ctx* ctx, void* U_native_dev, int update, double param, int parity, int sweep,
+                  unsigned long long seed, int t_first, int t_count, void* stream);
+int gf_anneal_half(gf_ctx* ctx, void* U_native_dev, double T, int parity, int step, unsigned long long seed,
+                   int t_first, int t_count, void* stream);
+/* Un-normalised sums over the owned sites, to be added over the slabs: F_raw = sum_{x, mu < Nd} Re tr U_mu(x) (eq. 2.1),
+ * theta_raw = sum_x tr[Delta Delta^dagger] (eq. 2.5; needs a current ghost).  Each output may be NULL.  Synchronises. */
+int gf_raw_sums(gf_ctx* ctx, const void* U_native_dev, double* F_raw_host, double* theta_raw_host);
+
 /* ---- host-buffer convenience path (what a user with a configuration in host memory calls) ---------------- */
 
 /* U_canon_host (canonical fp64, V*72 doubles) is copied to the device, packed, swept `nsweeps` times at

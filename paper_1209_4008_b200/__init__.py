@@ -56,6 +56,14 @@ SIGNATURES = {
     "gf_set_pdl": (_i, [_vp, _i]),
     "gf_set_prefetch": (_i, [_vp, _i]),
     "gf_set_coulomb_reading": (_i, [_vp, _i]),
+    "gf_create_slab": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, _i, _i, _i, _i]),
+    "gf_slab_face_bytes": (_sz, [_vp]),
+    "gf_slab_pack_face": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
+    "gf_slab_unpack_face": (_i, [_vp, _vp, _i, _i, _vp, _vp]),
+    "gf_begin_sweeps": (_i, [_vp, _vp]),
+    "gf_relax_half": (_i, [_vp, _vp, _i, _d, _i, _i, _ull, _i, _i, _vp]),
+    "gf_anneal_half": (_i, [_vp, _vp, _d, _i, _i, _ull, _i, _i, _vp]),
+    "gf_raw_sums": (_i, [_vp, _vp, _pd, _pd]),
     "gf_set_monitor": (_i, [_vp, _i]),
     "gf_monitor_last": (_i, [_vp, _pi, _pd, _pd, _pd]),
     "gf_set_chain": (_i, [_vp, _i, _d, _d]),
@@ -126,6 +134,48 @@ def gf_create(Nx: int, Ny: int, Nz: int, Nt: int, precision: int = GF_FP64, gaug
     rc = lib.gf_create(ctypes.byref(ctx), Nx, Ny, Nz, Nt, precision, gauge)
     _check(None, rc)
     return ctx
+
+
+def gf_create_slab(Nx: int, Ny: int, Nz: int, Nt_global: int, t_begin: int, t_end: int, precision: int = GF_FP64,
+                   gauge: int = GF_LANDAU):
+    lib = load_library()
+    ctx = _vp()
+    _check(None, lib.gf_create_slab(ctypes.byref(ctx), Nx, Ny, Nz, Nt_global, t_begin, t_end, precision, gauge))
+    return ctx
+
+
+def gf_slab_face_bytes(ctx) -> int:
+    return int(load_library().gf_slab_face_bytes(ctx))
+
+
+def gf_slab_pack_face(ctx, U, which: int, block_parity: int, buf, stream=None) -> None:
+    _check(ctx, load_library().gf_slab_pack_face(ctx, _ptr(U), int(which), int(block_parity), _ptr(buf), _stream(stream)))
+
+
+def gf_slab_unpack_face(ctx, U, which: int, block_parity: int, buf, stream=None) -> None:
+    _check(ctx, load_library().gf_slab_unpack_face(ctx, _ptr(U), int(which), int(block_parity), _ptr(buf), _stream(stream)))
+
+
+def gf_begin_sweeps(ctx, stream=None) -> None:
+    _check(ctx, load_library().gf_begin_sweeps(ctx, _stream(stream)))
+
+
+def gf_relax_half(ctx, U, update: int, param: float, parity: int, sweep: int, seed: int, t_first: int, t_count: int,
+                  stream=None) -> None:
+    _check(ctx, load_library().gf_relax_half(ctx, _ptr(U), int(update), float(param), int(parity), int(sweep), int(seed),
+                                            int(t_first), int(t_count), _stream(stream)))
+
+
+def gf_anneal_half(ctx, U, T: float, parity: int, step: int, seed: int, t_first: int, t_count: int, stream=None) -> None:
+    _check(ctx, load_library().gf_anneal_half(ctx, _ptr(U), float(T), int(parity), int(step), int(seed), int(t_first),
+                                             int(t_count), _stream(stream)))
+
+
+def gf_raw_sums(ctx, U):
+    """(F_raw, theta_raw) over the owned sites"""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(ctx, load_library().gf_raw_sums(ctx, _ptr(U), ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 def gf_destroy(ctx) -> None:

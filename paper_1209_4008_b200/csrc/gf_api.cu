@@ -13,7 +13,9 @@
 using namespace gf;
 
 struct gf_ctx {
-    int Nx, Ny, Nz, Nt;
+    int Nx, Ny, Nz, Nt;               // Nt: timeslices this context owns (a t-slab: t_begin .. t_begin + Nt - 1 of Nt_global)
+    int slab, t_begin, Nt_global;     // slab != 0: L.Nt = Nt + 1, the extra (last) slice is the ghost of slice t_begin - 1
+    unsigned Hs, H_own;               // half-sites per timeslice; half-sites owned (= Nt * Hs; L.H counts the ghost too)
     int precision, gauge, R;
     Lattice L;
     int tps, block;
@@ -51,6 +53,8 @@ struct gf_ctx {
 };
 
 static char g_create_err[512] = "";
+static int update_to_mode(int update, int* mode, int* variant);
+static int reduce_to_host(gf_ctx* c, const void* U, bool theta, const char* who);
 
 static int fail(gf_ctx* ctx, int code, const char* fmt, ...)
 {
@@ -71,7 +75,8 @@ static size_t real_size(const gf_ctx* c) { return c->precision == GF_FP64 ? 8 : 
 
 extern "C" const char* gf_last_error(const gf_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
 
-extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int gauge)
+static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int gauge, int slab, int t_begin,
+                       int Nt_global)
 {
     if (out == nullptr) return fail(nullptr, GF_EINVAL, "gf_create: out is NULL");
     *out = nullptr;
@@ -79,7 +84,7 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     for (int d = 0; d < 4; ++d)
         if (N[d] < 2 || (N[d] & 1))
             return fail(nullptr, GF_EINVAL, "gf_create: extent %d is %d; every extent must be even and >= 2 (C5)", d, N[d]);
-    const unsigned long long V = (unsigned long long)Nx * Ny * Nz * Nt;
+    const unsigned long long V = (unsigned long long)Nx * Ny * Nz * (Nt + (slab ? 1 : 0)); // the allocation: ghost slice included
     if (V >= (1ull << 31)) return fail(nullptr, GF_EINVAL, "gf_create: volume %llu >= 2^31", V);
     if (precision != GF_FP32 && precision != GF_FP64) return fail(nullptr, GF_EINVAL, "gf_create: unknown precision %d", precision);
     if (gauge != GF_LANDAU && gauge != GF_COULOMB) return fail(nullptr, GF_EINVAL, "gf_create: unknown gauge %d", gauge);
@@ -94,7 +99,10 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     if (c == nullptr) return fail(nullptr, GF_ENOMEM, "gf_create: host allocation failed");
     c->Nx = Nx; c->Ny = Ny; c->Nz = Nz; c->Nt = Nt;
     c->precision = precision; c->gauge = gauge; c->R = 18;
-    c->L.Nxh = Nx / 2; c->L.Ny = Ny; c->L.Nz = Nz; c->L.Nt = Nt; c->L.H = (unsigned)(V / 2);
+    c->slab = slab; c->t_begin = t_begin; c->Nt_global = Nt_global;
+    c->L.Nxh = Nx / 2; c->L.Ny = Ny; c->L.Nz = Nz; c->L.Nt = Nt + (slab ? 1 : 0); c->L.H = (unsigned)(V / 2);
+    c->Hs = (unsigned)(Nx / 2) * (unsigned)Ny * (unsigned)Nz;
+    c->H_own = c->Hs * (unsigned)Nt;
     c->tps = 0;   // 0 = automatic: resolved per (precision, storage, mode) by auto_tps()
     c->block = 0; // 0 = automatic
     c->reunit_every = -1; // automatic: reunit_due()
@@ -124,6 +132,22 @@ extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int preci
     }
     *out = c;
     return GF_OK;
+}
+
+extern "C" int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int gauge)
+{
+    return create_impl(out, Nx, Ny, Nz, Nt, precision, gauge, 0, 0, Nt);
+}
+
+extern "C" int gf_create_slab(gf_ctx** out, int Nx, int Ny, int Nz, int Nt_global, int t_begin, int t_end, int precision,
+                              int gauge)
+{
+    if (out != nullptr) *out = nullptr;
+    if (Nt_global < 2 || (Nt_global & 1) || t_begin < 0 || t_end > Nt_global || t_end - t_begin < 2 || (t_begin & 1) ||
+        ((t_end - t_begin) & 1))
+        return fail(nullptr, GF_EINVAL, "gf_create_slab: slab [%d, %d) of %d timeslices; bounds must be even, the slab at least 2 slices "
+                                        "(the local checkerboard must be the global one)", t_begin, t_end, Nt_global);
+    return create_impl(out, Nx, Ny, Nz, t_end - t_begin, precision, gauge, 1, t_begin, Nt_global);
 }
 
 extern "C" void gf_destroy(gf_ctx* c)
@@ -272,7 +296,7 @@ extern "C" unsigned long long gf_launch_count(const gf_ctx* c) { return c ? c->l
 static bool uses_reading_b(const gf_ctx* c, int mode)
 {
     (void)mode;
-    if (c->gauge != GF_COULOMB) return false;
+    if (c->gauge != GF_COULOMB || c->slab) return false; // a slab would have to exchange its g(x) face for the final pass
     return c->coulomb_b < 0 ? c->precision == GF_FP32 : c->coulomb_b != 0;
 }
 
@@ -332,7 +356,8 @@ static SweepParams base_params(gf_ctx* c, void* U)
     p.omega = 1.0;
     p.ph.T = 1.0;
     p.h_begin = 0;
-    p.h_count = c->L.H;
+    p.h_count = c->H_own;
+    p.site_offset = c->slab ? (uint32_t)c->t_begin * 2u * c->Hs : 0u;
     p.ld_policy = c->ld_policy;
     p.st_policy = c->st_policy;
     p.pdl = c->pdl;
@@ -348,7 +373,7 @@ extern "C" int gf_pack(gf_ctx* c, const double* canon, void* native, void* strea
     if (c == nullptr) return GF_EINVAL;
     if (canon == nullptr || native == nullptr) return fail(c, GF_EINVAL, "gf_pack: NULL pointer");
     c->last_stream = (cudaStream_t)stream;
-    cudaError_t e = launch_pack(c->precision, c->R, c->L, c->Nx, canon, native, c->last_stream);
+    cudaError_t e = launch_pack(c->precision, c->R, c->L, c->H_own, canon, native, c->last_stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "gf_pack");
     c->launches += 1;
     return GF_OK;
@@ -359,7 +384,7 @@ extern "C" int gf_unpack(gf_ctx* c, const void* native, double* canon, void* str
     if (c == nullptr) return GF_EINVAL;
     if (canon == nullptr || native == nullptr) return fail(c, GF_EINVAL, "gf_unpack: NULL pointer");
     c->last_stream = (cudaStream_t)stream;
-    cudaError_t e = launch_unpack(c->precision, c->R, c->L, c->Nx, native, canon, c->last_stream);
+    cudaError_t e = launch_unpack(c->precision, c->R, c->L, c->H_own, native, canon, c->last_stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "gf_unpack");
     c->launches += 1;
     return GF_OK;
@@ -438,7 +463,7 @@ static int run_sweeps_core(gf_ctx* c, void* U, int mode, int variant, double par
                 c->launches += 1;
                 if (launched) *launched += 1;
             } else {
-                const unsigned Hs = c->L.H / (unsigned)c->Nt; // half-sites per timeslice
+                const unsigned Hs = c->Hs; // half-sites per timeslice
                 for (int t = 0; t < c->Nt;) {
                     if (!active[t]) { ++t; continue; }
                     int t1 = t;
@@ -463,7 +488,7 @@ extern "C" int gf_convert(gf_ctx* src, const void* U_src, gf_ctx* dst, void* U_d
 {
     if (src == nullptr || dst == nullptr) return GF_EINVAL;
     if (U_src == nullptr || U_dst == nullptr) return fail(dst, GF_EINVAL, "gf_convert: NULL field");
-    if (src->Nx != dst->Nx || src->Ny != dst->Ny || src->Nz != dst->Nz || src->Nt != dst->Nt)
+    if (src->Nx != dst->Nx || src->Ny != dst->Ny || src->Nz != dst->Nz || src->Nt != dst->Nt || src->slab != dst->slab)
         return fail(dst, GF_EINVAL, "gf_convert: the two contexts describe different lattices");
     if (U_src == U_dst) return fail(dst, GF_EINVAL, "gf_convert: source and destination must be different buffers");
     dst->last_stream = (cudaStream_t)stream;
@@ -621,14 +646,108 @@ extern "C" int gf_anneal(gf_ctx* c, void* U, double T_start, double T_end, int n
     return gf_anneal_micro(c, U, T_start, T_end, nsteps, 0, seed, stream);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// single half-sweeps and t-slab faces: what a driver needs to run one configuration sharded in t over several
+// contexts (paper_1209_4008_b200/slab.py).  A slab context owns the timeslices
+// [t_begin, t_end) and keeps, as one more slice behind them, a ghost copy of the temporal links of slice t_begin - 1:
+// the only links a site of the slab shares with another slab (U_t(x - t) of its first slice).  Per half-sweep of
+// parity p the ghost is refreshed from the neighbour's last slice (parity block 1 - p: the links whose upper end is
+// active), the half-sweep updates it in place, and it is written back.
+// ---------------------------------------------------------------------------------------------------------
+extern "C" size_t gf_slab_face_bytes(const gf_ctx* c)
+{
+    if (c == nullptr) return 0;
+    return (size_t)c->Hs * (size_t)c->R * real_size(c);
+}
+
+static int face_impl(gf_ctx* c, void* U, int which, int block_parity, void* buf, bool pack, cudaStream_t st, const char* who)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (!c->slab) return fail(c, GF_EINVAL, "%s: not a slab context (gf_create_slab)", who);
+    if (U == nullptr || buf == nullptr) return fail(c, GF_EINVAL, "%s: NULL pointer", who);
+    if ((which != 0 && which != 1) || (block_parity != 0 && block_parity != 1)) return fail(c, GF_EINVAL, "%s: which and block_parity must be 0 or 1", who);
+    c->last_stream = st;
+    const int t = which == 0 ? c->Nt - 1 : c->Nt; // last owned slice / ghost slice
+    cudaError_t e = launch_face(c->precision, c->R, c->L, c->Hs, t, block_parity, pack, U, buf, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, who);
+    c->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_slab_pack_face(gf_ctx* c, const void* U, int which, int block_parity, void* buf_dev, void* stream)
+{
+    return face_impl(c, const_cast<void*>(U), which, block_parity, buf_dev, true, (cudaStream_t)stream, "gf_slab_pack_face");
+}
+
+extern "C" int gf_slab_unpack_face(gf_ctx* c, void* U, int which, int block_parity, const void* buf_dev, void* stream)
+{
+    return face_impl(c, U, which, block_parity, const_cast<void*>(buf_dev), false, (cudaStream_t)stream, "gf_slab_unpack_face");
+}
+
+// one half-sweep on the owned timeslices [t_first, t_first + t_count)
+static int half_impl(gf_ctx* c, void* U, int mode, int variant, double param, double T, int parity, int sweep,
+                     unsigned long long seed, int t_first, int t_count, cudaStream_t st, const char* who)
+{
+    if (U == nullptr) return fail(c, GF_EINVAL, "%s: U is NULL", who);
+    if (parity != 0 && parity != 1) return fail(c, GF_EINVAL, "%s: parity must be 0 (RED) or 1 (BLACK)", who);
+    if (sweep < 0) return fail(c, GF_EINVAL, "%s: sweep = %d < 0", who, sweep);
+    if (t_first < 0 || t_count < 0 || t_first + t_count > c->Nt) return fail(c, GF_EINVAL, "%s: timeslices [%d, %d) outside [0, %d)", who, t_first, t_first + t_count, c->Nt);
+    if (uses_reading_b(c, mode)) return fail(c, GF_EINVAL, "%s: single half-sweeps run Coulomb reading A (gf_set_coulomb_reading(ctx, 0))", who);
+    c->last_stream = st;
+    if (t_count == 0) return GF_OK;
+    SweepParams p = base_params(c, U);
+    p.omega = param;
+    p.variant = variant;
+    p.key0 = (uint32_t)seed;
+    p.key1 = (uint32_t)(seed >> 32);
+    c->call_sweeps = (unsigned long long)sweep;
+    const bool hot = mode == MODE_HEATBATH || (mode == MODE_VARIANT && variant == VARIANT_STOCHASTIC);
+    set_phase(c, p, parity, reunit_due(c, hot));
+    p.ph.step = (uint32_t)sweep;
+    p.ph.T = T;
+    p.trials = c->d_trials;
+    p.h_begin = (unsigned)t_first * c->Hs;
+    p.h_count = (unsigned)t_count * c->Hs;
+    cudaError_t e = launch_sweep(c, mode, p, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, who);
+    c->launches += 1;
+    c->half_sweeps += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_begin_sweeps(gf_ctx* c, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    return begin_call(c, (cudaStream_t)stream);
+}
+
+extern "C" int gf_relax_half(gf_ctx* c, void* U, int update, double param, int parity, int sweep, unsigned long long seed,
+                             int t_first, int t_count, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    int mode, variant;
+    if (update_to_mode(update, &mode, &variant) != GF_OK) return fail(c, GF_EINVAL, "gf_relax_half: unknown update %d", update);
+    if (update == GF_UPDATE_STOCHASTIC ? !(param >= 0.0 && param <= 1.0) : !(param >= 1.0 && param < 2.0))
+        return fail(c, GF_EINVAL, "gf_relax_half: parameter %g out of range for update %d", param, update);
+    return half_impl(c, U, mode, variant, param, 1.0, parity, sweep, seed, t_first, t_count, (cudaStream_t)stream, "gf_relax_half");
+}
+
+extern "C" int gf_anneal_half(gf_ctx* c, void* U, double T, int parity, int step, unsigned long long seed, int t_first,
+                              int t_count, void* stream)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (!(T > 0.0)) return fail(c, GF_EINVAL, "gf_anneal_half: temperature must be > 0 (got %g)", T);
+    return half_impl(c, U, MODE_HEATBATH, 0, 1.0, T, parity, step, seed, t_first, t_count, (cudaStream_t)stream, "gf_anneal_half");
+}
+
 // runs one reduction on last_stream and brings the Nt+2 results to h_out
 static int reduce_to_host(gf_ctx* c, const void* U, bool theta, const char* who)
 {
     if (U == nullptr) return fail(c, GF_EINVAL, "%s: U is NULL", who);
     const int nd = c->gauge == GF_COULOMB ? 3 : 4;
     cudaStream_t st = c->last_stream;
-    cudaError_t e = theta ? launch_theta(c->precision, c->R, c->L, nd, U, c->d_partials, c->d_out, st)
-                          : launch_functional(c->precision, c->R, c->L, nd, U, c->d_partials, c->d_out, st);
+    cudaError_t e = theta ? launch_theta(c->precision, c->R, c->L, c->Nt, nd, U, c->d_partials, c->d_out, st)
+                          : launch_functional(c->precision, c->R, c->L, c->Nt, nd, U, c->d_partials, c->d_out, st);
     if (e != cudaSuccess) return cuda_fail(c, e, who);
     c->launches += 2;
     e = cudaMemcpyAsync(c->h_out, c->d_out, (size_t)(c->Nt + 2) * sizeof(double), cudaMemcpyDeviceToHost, st);
@@ -654,6 +773,22 @@ extern "C" int gf_theta(gf_ctx* c, const void* U, double* theta_host)
     int rc = reduce_to_host(c, U, true, "gf_theta");
     if (rc != GF_OK) return rc;
     *theta_host = c->gauge == GF_COULOMB ? c->h_out[1] : c->h_out[0];
+    return GF_OK;
+}
+
+extern "C" int gf_raw_sums(gf_ctx* c, const void* U, double* F_raw_host, double* theta_raw_host)
+{
+    if (c == nullptr) return GF_EINVAL;
+    const double V = 2.0 * (double)c->H_own, nd = c->gauge == GF_COULOMB ? 3.0 : 4.0;
+    int rc;
+    if (F_raw_host) {
+        if ((rc = reduce_to_host(c, U, false, "gf_raw_sums")) != GF_OK) return rc;
+        *F_raw_host = c->h_out[0] * (3.0 * nd * V);
+    }
+    if (theta_raw_host) {
+        if ((rc = reduce_to_host(c, U, true, "gf_raw_sums")) != GF_OK) return rc;
+        *theta_raw_host = c->h_out[0] * (3.0 * V);
+    }
     return GF_OK;
 }
 
@@ -691,9 +826,9 @@ static int update_to_mode(int update, int* mode, int* variant)
 // (32^4 fp32: 185 / 214 against 178 us), the separate check ~110 us per check -- break-even near one check per 10 sweeps
 static bool monitor_applies(const gf_ctx* c, int mode, double tol, int check_every)
 {
-    if (!c->monitor) return false;
+    if (!c->monitor || c->slab) return false; // slabs: the driver owns the loop (exchange + all-reduce per check)
     if (c->monitor == 1 && check_every > 10) return false;
-    const unsigned Hs = c->L.H / (unsigned)c->Nt;
+    const unsigned Hs = c->Hs;
     const unsigned tps = (unsigned)auto_tps(c, mode), block = (unsigned)auto_block(c);
     if ((Hs * tps) % block != 0) return false;
     if (c->precision == GF_FP32 && tol < 1e-10) return false;
@@ -729,7 +864,7 @@ static int fix_fused(gf_ctx* c, void* U, int update, double param, double tol, i
     int mode, variant;
     if (update_to_mode(update, &mode, &variant) != GF_OK) return fail(c, GF_EINVAL, "%s: unknown update %d", who, update);
     const int Nt = c->Nt;
-    const unsigned Hs = c->L.H / (unsigned)Nt;
+    const unsigned Hs = c->Hs;
     const int tps = auto_tps(c, mode), block = auto_block(c);
     const int bps = (int)(Hs * (unsigned)tps / (unsigned)block), blocks = bps * Nt;
     const int groups = bps < 8 ? bps : 8;
@@ -780,7 +915,7 @@ static int fix_fused(gf_ctx* c, void* U, int update, double param, double tol, i
         m.slices = slices ? 1 : 0;
         m.coulomb = coulomb ? 1 : 0;
         m.tol = tol;
-        const double V = 2.0 * (double)c->L.H, nd = coulomb ? 3.0 : 4.0;
+        const double V = 2.0 * (double)c->H_own, nd = coulomb ? 3.0 : 4.0;
         m.scale_theta_t = 1.0 / (3.0 * V / Nt);
         m.scale_theta = 1.0 / (3.0 * V);
         m.scale_F = 1.0 / (3.0 * nd * V);
@@ -952,9 +1087,10 @@ static int overrelax_host_impl(gf_ctx* c, void* U_host, size_t elem, double omeg
                                double* theta_host, const char* who)
 {
     if (c == nullptr) return GF_EINVAL;
+    if (c->slab) return fail(c, GF_EINVAL, "%s: not available on a slab context", who);
     if (U_host == nullptr) return fail(c, GF_EINVAL, "%s: U_canon_host is NULL", who);
-    const size_t canon_bytes = (size_t)c->L.H * 2 * 72 * sizeof(double); // staging sized for the larger element
-    const size_t copy_bytes = (size_t)c->L.H * 2 * 72 * elem;
+    const size_t canon_bytes = (size_t)c->H_own * 2 * 72 * sizeof(double); // staging sized for the larger element
+    const size_t copy_bytes = (size_t)c->H_own * 2 * 72 * elem;
     cudaError_t e;
     if (c->d_canon == nullptr && (e = cudaMalloc(&c->d_canon, canon_bytes)) != cudaSuccess) { c->d_canon = nullptr; return cuda_fail(c, e, "host path: staging allocation"); }
     if (c->d_native == nullptr && (e = cudaMalloc(&c->d_native, gf_field_bytes(c))) != cudaSuccess) { c->d_native = nullptr; return cuda_fail(c, e, "host path: staging allocation"); }
@@ -963,7 +1099,7 @@ static int overrelax_host_impl(gf_ctx* c, void* U_host, size_t elem, double omeg
     int rc;
     if (elem == 8) rc = gf_pack(c, c->d_canon, c->d_native, st);
     else {
-        e = launch_pack_f32(c->precision, c->R, c->L, (const float*)c->d_canon, c->d_native, st);
+        e = launch_pack_f32(c->precision, c->R, c->L, c->H_own, (const float*)c->d_canon, c->d_native, st);
         if (e != cudaSuccess) return cuda_fail(c, e, "host path: pack");
         c->launches += 1;
         rc = GF_OK;
@@ -972,7 +1108,7 @@ static int overrelax_host_impl(gf_ctx* c, void* U_host, size_t elem, double omeg
     if (rc != GF_OK) return rc;
     if (elem == 8) rc = gf_unpack(c, c->d_native, c->d_canon, st);
     else {
-        e = launch_unpack_f32(c->precision, c->R, c->L, c->d_native, (float*)c->d_canon, st);
+        e = launch_unpack_f32(c->precision, c->R, c->L, c->H_own, c->d_native, (float*)c->d_canon, st);
         if (e != cudaSuccess) return cuda_fail(c, e, "host path: unpack");
         c->launches += 1;
     }

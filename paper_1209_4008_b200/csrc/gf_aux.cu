@@ -13,12 +13,13 @@ constexpr int AUX_BLOCK = 256;
 // pack / unpack.  One thread per (half-site h, link block l = parity*4 + mu).
 // ---------------------------------------------------------------------------------------------------------
 template <typename T, int R, typename S>
-__global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, const S* __restrict__ canon, T* __restrict__ native)
+__global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, unsigned H_own, const S* __restrict__ canon, T* __restrict__ native)
 {
+    // H_own < L.H on a slab context: the ghost slice (the last one) has no canonical counterpart
     const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= (unsigned long long)L.H * 8ull) return;
-    const unsigned h = (unsigned)(gid % L.H);
-    const int l = (int)(gid / L.H), parity = l >> 2, mu = l & 3;
+    if (gid >= (unsigned long long)H_own * 8ull) return;
+    const unsigned h = (unsigned)(gid % H_own);
+    const int l = (int)(gid / H_own), parity = l >> 2, mu = l & 3;
     const Site s = decode_site(L, h, parity);
     const S* src = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
     cx<T> u[9];
@@ -28,12 +29,12 @@ __global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, const S* __r
 }
 
 template <typename T, int R, typename S>
-__global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* __restrict__ native, S* __restrict__ canon)
+__global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, unsigned H_own, const T* __restrict__ native, S* __restrict__ canon)
 {
     const unsigned long long gid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= (unsigned long long)L.H * 8ull) return;
-    const unsigned h = (unsigned)(gid % L.H);
-    const int l = (int)(gid / L.H), parity = l >> 2, mu = l & 3;
+    if (gid >= (unsigned long long)H_own * 8ull) return;
+    const unsigned h = (unsigned)(gid % H_own);
+    const int l = (int)(gid / H_own), parity = l >> 2, mu = l & 3;
     const Site s = decode_site(L, h, parity);
     cx<T> u[9];
     LinkIO<T, R>::load(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
@@ -44,46 +45,89 @@ __global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, const T* _
 
 // canon_f32: the canonical field holds float instead of double (host-buffer path of fp32 contexts)
 template <typename S>
-static cudaError_t launch_pack_t(int prec, int R, const Lattice& L, const S* canon, void* native, cudaStream_t st)
+static cudaError_t launch_pack_t(int prec, int R, const Lattice& L, unsigned H_own, const S* canon, void* native, cudaStream_t st)
 {
-    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned long long n = (unsigned long long)H_own * 8ull;
     const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
-    if (prec == 0 && R == 18) pack_kernel<float, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
-    else if (prec == 0 && R == 12) pack_kernel<float, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (float*)native);
-    else if (prec == 1 && R == 18) pack_kernel<double, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
-    else if (prec == 1 && R == 12) pack_kernel<double, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, canon, (double*)native);
+    if (prec == 0 && R == 18) pack_kernel<float, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, canon, (float*)native);
+    else if (prec == 0 && R == 12) pack_kernel<float, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, canon, (float*)native);
+    else if (prec == 1 && R == 18) pack_kernel<double, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, canon, (double*)native);
+    else if (prec == 1 && R == 12) pack_kernel<double, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, canon, (double*)native);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 
 template <typename S>
-static cudaError_t launch_unpack_t(int prec, int R, const Lattice& L, const void* native, S* canon, cudaStream_t st)
+static cudaError_t launch_unpack_t(int prec, int R, const Lattice& L, unsigned H_own, const void* native, S* canon, cudaStream_t st)
 {
-    const unsigned long long n = (unsigned long long)L.H * 8ull;
+    const unsigned long long n = (unsigned long long)H_own * 8ull;
     const unsigned grid = (unsigned)((n + AUX_BLOCK - 1) / AUX_BLOCK);
-    if (prec == 0 && R == 18) unpack_kernel<float, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
-    else if (prec == 0 && R == 12) unpack_kernel<float, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const float*)native, canon);
-    else if (prec == 1 && R == 18) unpack_kernel<double, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
-    else if (prec == 1 && R == 12) unpack_kernel<double, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, (const double*)native, canon);
+    if (prec == 0 && R == 18) unpack_kernel<float, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, (const float*)native, canon);
+    else if (prec == 0 && R == 12) unpack_kernel<float, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, (const float*)native, canon);
+    else if (prec == 1 && R == 18) unpack_kernel<double, 18, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, (const double*)native, canon);
+    else if (prec == 1 && R == 12) unpack_kernel<double, 12, S><<<grid, AUX_BLOCK, 0, st>>>(L, H_own, (const double*)native, canon);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 
-cudaError_t launch_pack(int prec, int R, const Lattice& L, int, const double* canon, void* native, cudaStream_t st)
+cudaError_t launch_pack(int prec, int R, const Lattice& L, unsigned H_own, const double* canon, void* native, cudaStream_t st)
 {
-    return launch_pack_t<double>(prec, R, L, canon, native, st);
+    return launch_pack_t<double>(prec, R, L, H_own, canon, native, st);
 }
-cudaError_t launch_unpack(int prec, int R, const Lattice& L, int, const void* native, double* canon, cudaStream_t st)
+cudaError_t launch_unpack(int prec, int R, const Lattice& L, unsigned H_own, const void* native, double* canon, cudaStream_t st)
 {
-    return launch_unpack_t<double>(prec, R, L, native, canon, st);
+    return launch_unpack_t<double>(prec, R, L, H_own, native, canon, st);
 }
-cudaError_t launch_pack_f32(int prec, int R, const Lattice& L, const float* canon, void* native, cudaStream_t st)
+cudaError_t launch_pack_f32(int prec, int R, const Lattice& L, unsigned H_own, const float* canon, void* native, cudaStream_t st)
 {
-    return launch_pack_t<float>(prec, R, L, canon, native, st);
+    return launch_pack_t<float>(prec, R, L, H_own, canon, native, st);
 }
-cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, const void* native, float* canon, cudaStream_t st)
+cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, unsigned H_own, const void* native, float* canon, cudaStream_t st)
 {
-    return launch_unpack_t<float>(prec, R, L, native, canon, st);
+    return launch_unpack_t<float>(prec, R, L, H_own, native, canon, st);
+}
+
+// t-slab faces (NEXT-4): the temporal links of one parity block of one timeslice, gathered plane by plane into a
+// contiguous message / scattered back.  One thread per 128-bit vector of the slice.
+template <typename T, int R, bool PACK>
+__global__ void __launch_bounds__(AUX_BLOCK) face_kernel(Lattice L, unsigned Hs, int t, int block_parity, T* __restrict__ native,
+                                                         T* __restrict__ buf)
+{
+    constexpr int VEC = 16 / sizeof(T);                 // reals per 128-bit vector
+    const unsigned idx = blockIdx.x * blockDim.x + threadIdx.x; // real pair / quad index inside the face
+    const unsigned nvec = Hs * (unsigned)(R / VEC);     // fp32 R18: the 64-bit tail plane is handled below
+    T* blk = native + (size_t)(block_parity * 4 + 3) * R * L.H;
+    if (idx < nvec) {
+        const unsigned plane = idx / Hs, i = idx % Hs;
+        T* a = blk + ((size_t)plane * L.H + (size_t)t * Hs + i) * VEC;
+        T* b = buf + (size_t)idx * VEC;
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) { if (PACK) b[k] = a[k]; else a[k] = b[k]; }
+    }
+    if (sizeof(T) == 4 && R == 18 && idx < Hs) { // trailing float2 plane at real offset 16 H
+        T* a = blk + (size_t)16 * L.H + ((size_t)t * Hs + idx) * 2;
+        T* b = buf + (size_t)16 * Hs + (size_t)idx * 2;
+        if (PACK) { b[0] = a[0]; b[1] = a[1]; } else { a[0] = b[0]; a[1] = b[1]; }
+    }
+}
+
+cudaError_t launch_face(int prec, int R, const Lattice& L, unsigned Hs, int t, int block_parity, bool pack, void* native,
+                        void* buf, cudaStream_t st)
+{
+    const unsigned nvec = Hs * (unsigned)(R / (prec == 0 ? 4 : 2));
+    const unsigned grid = (nvec + AUX_BLOCK - 1) / AUX_BLOCK;
+#define GF_FACE(T, RR)                                                                                              \
+    do {                                                                                                            \
+        if (pack) face_kernel<T, RR, true><<<grid, AUX_BLOCK, 0, st>>>(L, Hs, t, block_parity, (T*)native, (T*)buf);  \
+        else face_kernel<T, RR, false><<<grid, AUX_BLOCK, 0, st>>>(L, Hs, t, block_parity, (T*)native, (T*)buf);      \
+    } while (0)
+    if (prec == 0 && R == 18) GF_FACE(float, 18);
+    else if (prec == 0 && R == 12) GF_FACE(float, 12);
+    else if (prec == 1 && R == 18) GF_FACE(double, 18);
+    else if (prec == 1 && R == 12) GF_FACE(double, 12);
+    else return cudaErrorInvalidValue;
+#undef GF_FACE
+    return cudaGetLastError();
 }
 
 // native -> native between precisions / storage formats (mixed-precision fixing: fp32 sweeps, fp64 polish)
@@ -311,12 +355,13 @@ __global__ void __launch_bounds__(AUX_BLOCK) final_kernel(int Nt, int per_slice,
     }
 }
 
+// nt: timeslices reduced (L.Nt, or the owned slices of a slab context: its ghost slice is left out)
 template <bool THETA>
-static cudaError_t launch_reduction(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+static cudaError_t launch_reduction(int prec, int R, const Lattice& L, int nt, int nd, const void* native, double* partials,
                                     double* out, cudaStream_t st)
 {
     const int bx = reduce_blocks_per_slice(L);
-    const dim3 grid((unsigned)bx, (unsigned)(2 * L.Nt));
+    const dim3 grid((unsigned)bx, (unsigned)(2 * nt));
 #define GF_RED(T, RR)                                                                                   \
     do {                                                                                                \
         if (THETA) theta_kernel<T, RR><<<grid, AUX_BLOCK, 0, st>>>(L, nd, (const T*)native, partials);   \
@@ -330,23 +375,23 @@ static cudaError_t launch_reduction(int prec, int R, const Lattice& L, int nd, c
 #undef GF_RED
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const double V = 2.0 * (double)L.H, Vs = V / (double)L.Nt;
+    const double Vs = 2.0 * (double)L.H / (double)L.Nt, V = Vs * (double)nt;
     const double scale_total = THETA ? 1.0 / (3.0 * V) : 1.0 / (3.0 * nd * V);
     const double scale_slice = THETA ? 1.0 / (3.0 * Vs) : 1.0 / (3.0 * nd * Vs);
-    final_kernel<<<1, AUX_BLOCK, 0, st>>>(L.Nt, 2 * bx, partials, scale_total, scale_slice, out);
+    final_kernel<<<1, AUX_BLOCK, 0, st>>>(nt, 2 * bx, partials, scale_total, scale_slice, out);
     return cudaGetLastError();
 }
 
-cudaError_t launch_functional(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+cudaError_t launch_functional(int prec, int R, const Lattice& L, int nt, int nd, const void* native, double* partials,
                               double* out, cudaStream_t st)
 {
-    return launch_reduction<false>(prec, R, L, nd, native, partials, out, st);
+    return launch_reduction<false>(prec, R, L, nt, nd, native, partials, out, st);
 }
 
-cudaError_t launch_theta(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+cudaError_t launch_theta(int prec, int R, const Lattice& L, int nt, int nd, const void* native, double* partials,
                          double* out, cudaStream_t st)
 {
-    return launch_reduction<true>(prec, R, L, nd, native, partials, out, st);
+    return launch_reduction<true>(prec, R, L, nt, nd, native, partials, out, st);
 }
 
 } // namespace gf

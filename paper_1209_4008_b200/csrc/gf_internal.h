@@ -18,13 +18,18 @@ GF_DECLARE_SWEEP(f64_r18)
 #undef GF_DECLARE_SWEEP
 
 // gf_aux.cu: layout conversion and reductions.  prec: 0 fp32, 1 fp64; R: 12 or 18.
-cudaError_t launch_pack(int prec, int R, const Lattice& L, int Nx, const double* canon, void* native,
+// H_own: half-sites with a canonical counterpart (L.H, or less on a slab context whose last slice is a ghost)
+cudaError_t launch_pack(int prec, int R, const Lattice& L, unsigned H_own, const double* canon, void* native,
                         cudaStream_t stream);
-cudaError_t launch_unpack(int prec, int R, const Lattice& L, int Nx, const void* native, double* canon,
+cudaError_t launch_unpack(int prec, int R, const Lattice& L, unsigned H_own, const void* native, double* canon,
                           cudaStream_t stream);
 
-cudaError_t launch_pack_f32(int prec, int R, const Lattice& L, const float* canon, void* native, cudaStream_t stream);
-cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, const void* native, float* canon, cudaStream_t stream);
+cudaError_t launch_pack_f32(int prec, int R, const Lattice& L, unsigned H_own, const float* canon, void* native, cudaStream_t stream);
+cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, unsigned H_own, const void* native, float* canon, cudaStream_t stream);
+
+// t-slab faces: temporal links of parity block `block_parity` of local timeslice t <-> contiguous buffer
+cudaError_t launch_face(int prec, int R, const Lattice& L, unsigned Hs, int t, int block_parity, bool pack, void* native,
+                        void* buf, cudaStream_t stream);
 
 cudaError_t launch_convert(int sprec, int sR, int dprec, int dR, const Lattice& L, const void* src, void* dst,
                            cudaStream_t stream);
@@ -37,9 +42,9 @@ cudaError_t launch_coulomb_finish(int prec, int R, const Lattice& L, void* nativ
 //   functional: out[0] = sum_{x, mu<nd} Re tr U_mu(x) / (3 nd V)
 //   theta:      out[0] = theta over the whole lattice (eq. 2.5); out[1] = max_t theta_t; out[2+t] = theta_t
 int reduce_blocks_per_slice(const Lattice& L);
-cudaError_t launch_functional(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+cudaError_t launch_functional(int prec, int R, const Lattice& L, int nt, int nd, const void* native, double* partials,
                               double* out, cudaStream_t stream);
-cudaError_t launch_theta(int prec, int R, const Lattice& L, int nd, const void* native, double* partials,
+cudaError_t launch_theta(int prec, int R, const Lattice& L, int nt, int nd, const void* native, double* partials,
                          double* out, cudaStream_t stream);
 
 } // namespace gf

@@ -94,6 +94,8 @@ struct SweepParams {
     double omega;   // overrelaxation parameter; MODE_VARIANT: omega (first order) or probability p
     int variant;    // MODE_VARIANT: VARIANT_*
     uint32_t key0, key1;       // Philox key = seed (C14)
+    uint32_t site_offset;      // canonical index of local site 0 in the whole lattice (t-slab contexts; else 0): the Philox
+                               // counters carry the site of the whole lattice, so a sharded run draws the same numbers
     unsigned* trials;          // optional: KP trial counts, index 3*s + subgroup
     void* G;                   // Coulomb reading B (C12): accumulated g(x), 2 parity blocks of 18 reals per site
     // fp32 kernels: precision of the site chain (K(x), the three SU(2) steps, K <- G K), DESIGN.md sec. 4
@@ -351,7 +353,7 @@ __device__ __forceinline__ void fixup_subgroup(const SweepParams& p, const Sweep
         EarlyRandom early;
         early_random(p.key0, p.key1, site_canon, ph.step, c2, early);
         const unsigned ntr = su2_heatbath_step<double, double>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond);
-        if (record && p.trials != nullptr) p.trials[3u * (size_t)site_canon + SUB] = ntr;
+        if (record && p.trials != nullptr) p.trials[3u * (size_t)(site_canon - p.site_offset) + SUB] = ntr;
     }
     a = {h[0], h[3]};
     b = {h[2], h[1]}; // C4
@@ -381,7 +383,7 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
 #pragma unroll
             for (int c = 0; c < 3; ++c) K[3 * r + c] = K[3 * r + c] + f[3 * r + c] + conj(b[3 * c + r]);
     }
-    const uint32_t sc = canonical_index(s);
+    const uint32_t sc = canonical_index(s) + p.site_offset;
     const bool record = lane_mu0 == 0;
     cx<double> a0, b0, a1, b1, a2, b2;
     fixup_subgroup<0, 1, 0, MODE>(p, ph, K, sc, record, a0, b0);
@@ -476,7 +478,7 @@ struct SweepKernel {
             (void)early;
         } else {
             unsigned ntr = su2_heatbath_step<CT, T>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond);
-            if (record && p.trials != nullptr) p.trials[3u * (size_t)site_canon + SUB] = ntr;
+            if (record && p.trials != nullptr) p.trials[3u * (size_t)(site_canon - p.site_offset) + SUB] = ntr;
         }
         if (FP32) watch = watch || ((float)cond < p.watch_thr2);
         const cx<CT> ac = {h[0], h[3]}, bc = {h[2], h[1]}; // C4
@@ -724,7 +726,7 @@ struct SweepKernel {
         if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)ph.parity * 18 * H, H, s.h, Gt, pol.ld);
         if (MODE == MODE_HEATBATH) issue_prefetch(p, ph, s, hb, lane_mu0, base, H);
         // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
-        const uint32_t sc = canonical_index(s);
+        const uint32_t sc = canonical_index(s) + p.site_offset;
         EarlyRandom early[3];
         if (MODE == MODE_HEATBATH) {
 #pragma unroll
