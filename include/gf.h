@@ -211,6 +211,17 @@ int gf_overrelax_host(gf_ctx* ctx, double* U_canon_host, double omega, int nswee
 int gf_overrelax_host_f32(gf_ctx* ctx, float* U_canon_host, double omega, int nsweeps, double* F_host,
                           double* theta_host);
 
+/* An ensemble of n configurations in host memory (the shape of production gauge fixing), pipelined: configuration
+ * i+1 is copied to the device and configuration i-1 copied back while configuration i is swept -- three staging slots in
+ * the context, one stream per direction of the PCIe link and one for the kernels.  U_canon_host: n pointers to canonical
+ * fields of element_bytes = 8 (double) or 4 (float) per real, each updated in place exactly as gf_overrelax_host /
+ * gf_overrelax_host_f32 would (bit-identical); pinned memory lets the copies overlap, pageable memory is correct but
+ * serial.  F_host_n / theta_host_n (n doubles each, may be NULL): F and theta after the last sweep.  Synchronous.
+ * GF_EINVAL: n < 0, a NULL configuration, element_bytes not 4 or 8, omega outside [1,2), nsweeps < 0, a slab context.
+ * GF_ENOMEM: the staging slots (3 x (canonical + native field)) cannot be allocated. */
+int gf_overrelax_host_batch(gf_ctx* ctx, void* const* U_canon_host, int n, int element_bytes, double omega, int nsweeps,
+                            double* F_host_n, double* theta_host_n);
+
 /* ---- tuning and diagnostics ------------------------------------------------------------------------------ */
 
 /* Launch shape of the sweep kernels: threads_per_site in {1,2,4} (1: one thread holds all 8 links of a site;

@@ -49,6 +49,7 @@ SIGNATURES = {
     "gf_theta_slices": (_i, [_vp, _vp, _pd]),
     "gf_overrelax_host": (_i, [_vp, _vp, _d, _i, _pd, _pd]),
     "gf_overrelax_host_f32": (_i, [_vp, _vp, _d, _i, _pd, _pd]),
+    "gf_overrelax_host_batch": (_i, [_vp, ctypes.POINTER(_vp), _i, _i, _d, _i, _pd, _pd]),
     "gf_set_tuning": (_i, [_vp, _i, _i]),
     "gf_set_reunit": (_i, [_vp, _i]),
     "gf_set_l2_reversal": (_i, [_vp, _i]),
@@ -275,6 +276,21 @@ def gf_overrelax_host_f32(ctx, U_canon_host, omega: float, nsweeps: int):
     _check(ctx, load_library().gf_overrelax_host_f32(ctx, _ptr(U_canon_host), float(omega), int(nsweeps),
                                                     ctypes.byref(F), ctypes.byref(th)))
     return F.value, th.value
+
+
+def gf_overrelax_host_batch(ctx, U_canon_hosts, omega: float, nsweeps: int):
+    """U_canon_hosts: list of host arrays (numpy complex128 / complex64 (V,4,3,3), or pinned torch tensors of float64 /
+    float32), all of one element type, each updated in place.  Returns ([F], [theta])."""
+    n = len(U_canon_hosts)
+    if n == 0:
+        return [], []
+    first = U_canon_hosts[0]
+    itemsize = first.element_size() if hasattr(first, "element_size") else first.dtype.itemsize
+    elem = 4 if itemsize in (4,) or str(getattr(first, "dtype", "")) in ("complex64", "torch.float32") else 8
+    ptrs = (_vp * n)(*[_ptr(u) for u in U_canon_hosts])
+    F, th = (ctypes.c_double * n)(), (ctypes.c_double * n)()
+    _check(ctx, load_library().gf_overrelax_host_batch(ctx, ptrs, n, elem, float(omega), int(nsweeps), F, th))
+    return list(F), list(th)
 
 
 def gf_set_tuning(ctx, threads_per_site: int = 0, block: int = 0) -> None:

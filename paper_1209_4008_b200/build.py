@@ -2,9 +2,9 @@
 
     python -m paper_1209_4008_b200.build [--force] [--verbose]
 
-Objects go to paper_1209_4008_b200/_build/, the library to paper_1209_4008_b200/libgf.so.  The four
-(precision, reals-per-link) instances of the sweep kernels are separate translation units and compile in
-parallel.  A unit is rebuilt when any source or header is newer than its object.
+Objects go to paper_1209_4008_b200/_build/, the library to paper_1209_4008_b200/libgf.so.  The instances of the
+sweep kernels are twelve translation units ((precision, reals-per-link) x {relaxation, monitored, heatbath}) and
+compile in parallel.  A unit is rebuilt when any source or header is newer than its object.
 """
 from __future__ import annotations
 
@@ -23,15 +23,16 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
-# (object name, source, extra defines)
+# (object name, source, extra defines).  The sweep kernels of one (precision, reals-per-link) are three units
+# (gf_sweep_inst.cu: relaxation + launcher, monitored relaxation, heatbath), twelve in all.
 UNITS = [
     ("gf_api.o", "gf_api.cu", []),
     ("gf_aux.o", "gf_aux.cu", []),
-    ("gf_sweep_f32_r12.o", "gf_sweep_inst.cu", ["-DGF_INST_FP64=0", "-DGF_INST_R=12"]),
-    ("gf_sweep_f32_r18.o", "gf_sweep_inst.cu", ["-DGF_INST_FP64=0", "-DGF_INST_R=18"]),
-    ("gf_sweep_f64_r12.o", "gf_sweep_inst.cu", ["-DGF_INST_FP64=1", "-DGF_INST_R=12"]),
-    ("gf_sweep_f64_r18.o", "gf_sweep_inst.cu", ["-DGF_INST_FP64=1", "-DGF_INST_R=18"]),
 ]
+for _fp64, _R in ((0, 12), (0, 18), (1, 12), (1, 18)):
+    for _part in range(3):
+        UNITS.append((f"gf_sweep_f{64 if _fp64 else 32}_r{_R}_p{_part}.o", "gf_sweep_inst.cu",
+                      [f"-DGF_INST_FP64={_fp64}", f"-DGF_INST_R={_R}", f"-DGF_INST_PART={_part}"]))
 
 
 def _deps():

@@ -1,7 +1,9 @@
-// gf_sweep_inst.cu -- one translation unit per (precision, reals-per-link): compiled four times by build.py with
-//   -DGF_INST_FP64={0,1} -DGF_INST_R={12,18}
-// so the seventy-two half-sweep kernels build in parallel.  Each unit exports one launcher and one
-// attribute query, declared in gf_internal.h.
+// gf_sweep_inst.cu -- the half-sweep kernels of one (precision, reals-per-link), compiled by build.py as three translation
+// units per pair so that the instantiations build in parallel:
+//   -DGF_INST_FP64={0,1} -DGF_INST_R={12,18} -DGF_INST_PART={0,1,2}
+//   part 0: relaxation kernels (overrelaxation, variants) and the launcher / attribute query (declared in gf_internal.h)
+//   part 1: relaxation kernels with the fused F / theta monitor
+//   part 2: heatbath kernels
 #include "gf_internal.h"
 #include "gf_sweep.cuh"
 
@@ -24,6 +26,10 @@ namespace gf {
 
 typedef void (*sweep_fn)(const SweepParams);
 
+// the kernels of the other parts, by their selectors (NULL: no such kernel)
+sweep_fn GF_NAME(pick_monitor)(int tps, int mode, bool cb, int mon);
+sweep_fn GF_NAME(pick_heatbath)(int tps, bool cb, bool dc);
+
 template <int MODE, bool CB, bool DC, int MON>
 static sweep_fn pick_tps(int tps)
 {
@@ -34,35 +40,16 @@ static sweep_fn pick_tps(int tps)
     return nullptr;
 }
 
-// dc: fp32 heatbath kernel with the double chain at every site (the relaxation kernels pick their chain at run time)
-// mon: relaxation kernel with the fused F / theta monitor (1: stop test only, 2: partials and duty)
-template <int MODE, bool CB>
-static sweep_fn pick_mon(int tps, int mon)
-{
-    if (mon == 2) return pick_tps<MODE, CB, false, 2>(tps);
-    if (mon == 1) return pick_tps<MODE, CB, false, 1>(tps);
-    return pick_tps<MODE, CB, false, 0>(tps);
-}
-
-template <bool CB>
-static sweep_fn pick_mode(int tps, int mode, bool dc, int mon)
-{
-    if (mode == MODE_OVERRELAX) return pick_mon<MODE_OVERRELAX, CB>(tps, mon);
-    if (mode == MODE_VARIANT) return pick_mon<MODE_VARIANT, CB>(tps, mon);
-    if (mode == MODE_HEATBATH && mon == 0) {
-#if !GF_INST_FP64
-        if (dc) return pick_tps<MODE_HEATBATH, CB, true, 0>(tps);
-#endif
-        (void)dc;
-        return pick_tps<MODE_HEATBATH, CB, false, 0>(tps);
-    }
-    return nullptr;
-}
-
-// cb: Coulomb reading B
+#if GF_INST_PART == 0
+// cb: Coulomb reading B; dc: fp32 heatbath kernel with the double chain at every site (the relaxation kernels pick
+// their chain at run time); mon: relaxation kernel with the fused F / theta monitor (1: stop test only, 2: partials, duty)
 static sweep_fn pick(int tps, int mode, bool cb, bool dc, int mon)
 {
-    return cb ? pick_mode<true>(tps, mode, dc, mon) : pick_mode<false>(tps, mode, dc, mon);
+    if (mode == MODE_HEATBATH) return mon == 0 ? GF_NAME(pick_heatbath)(tps, cb, dc) : nullptr;
+    if (mon != 0) return GF_NAME(pick_monitor)(tps, mode, cb, mon);
+    if (mode == MODE_OVERRELAX) return cb ? pick_tps<MODE_OVERRELAX, true, false, 0>(tps) : pick_tps<MODE_OVERRELAX, false, false, 0>(tps);
+    if (mode == MODE_VARIANT) return cb ? pick_tps<MODE_VARIANT, true, false, 0>(tps) : pick_tps<MODE_VARIANT, false, false, 0>(tps);
+    return nullptr;
 }
 
 cudaError_t GF_NAME(launch_sweep)(int tps, int mode, int block, const SweepParams& p, cudaStream_t stream)
@@ -98,5 +85,34 @@ cudaError_t GF_NAME(sweep_attributes)(int tps, int mode, bool reading_b, bool dc
     if (fn == nullptr) return cudaErrorInvalidValue;
     return cudaFuncGetAttributes(attr, fn);
 }
+#endif // part 0
+
+#if GF_INST_PART == 1
+template <int MODE, bool CB>
+static sweep_fn pick_mon(int tps, int mon)
+{
+    if (mon == 2) return pick_tps<MODE, CB, false, 2>(tps);
+    if (mon == 1) return pick_tps<MODE, CB, false, 1>(tps);
+    return nullptr;
+}
+
+sweep_fn GF_NAME(pick_monitor)(int tps, int mode, bool cb, int mon)
+{
+    if (mode == MODE_OVERRELAX) return cb ? pick_mon<MODE_OVERRELAX, true>(tps, mon) : pick_mon<MODE_OVERRELAX, false>(tps, mon);
+    if (mode == MODE_VARIANT) return cb ? pick_mon<MODE_VARIANT, true>(tps, mon) : pick_mon<MODE_VARIANT, false>(tps, mon);
+    return nullptr;
+}
+#endif // part 1
+
+#if GF_INST_PART == 2
+sweep_fn GF_NAME(pick_heatbath)(int tps, bool cb, bool dc)
+{
+#if !GF_INST_FP64
+    if (dc) return cb ? pick_tps<MODE_HEATBATH, true, true, 0>(tps) : pick_tps<MODE_HEATBATH, false, true, 0>(tps);
+#endif
+    (void)dc;
+    return cb ? pick_tps<MODE_HEATBATH, true, false, 0>(tps) : pick_tps<MODE_HEATBATH, false, false, 0>(tps);
+}
+#endif // part 2
 
 } // namespace gf
