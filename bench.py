@@ -10,11 +10,13 @@ Metric: site-updates/s (one site-update = the full SU(3) update of one site: 3 S
 GFlop/s = site-updates/s x 2253 (paper flop model).
 
 Workloads (BASELINE.json configs; seeded synthetic fields, recipe in DESIGN.md "Inputs"):
-    32^4-f32-r18 (default, the headline config), 32^4-f32-r12, 32^4-f64-r18, 64^4-f64-r18, 64^4-f32-r18,
-    16^3x32-f32-r18, 16^3x32-f64-r18, 48^3x64-f32-r18-coulomb-anneal
-N > 1 (torchrun): the path does not shard on one GPU's problem ("replicas only"): every rank runs an
-independent replica of the workload on its own GPU, no data-path collective; value = all ranks' site-updates /
-max-over-ranks time.
+    32^4-f32-r18 (default, the headline config), 32^4-f32-r12, 32^4-f64-r18, 32^4-f64-r12, 64^4-f64-r18, 64^4-f32-r18,
+    16^3x32-f32-r18, 16^3x32-f64-r18, 48^3x64-f32-r18-coulomb, and the annealing sweeps 48^3x64-f32-r18-coulomb-anneal,
+    48^3x64-f64-r18-coulomb-anneal, 32^4-f64-r18-anneal, 32^4-f32-r12-anneal
+N > 1 (torchrun): by default every rank runs an independent replica of the workload on its own GPU ("replicas": the
+shape of production gauge fixing, ensembles of configurations; no data-path collective); --shard t runs ONE
+configuration cut into t-slabs over the ranks (paper_1209_4008_b200/slab.py: one face message up and one down per
+half-sweep and slab boundary, strong scaling).  value = site-updates of the whole job / max-over-ranks time.
 
 --impl reference times the fp64 CPU oracle (oracle/, as it stands) on the host cores on the same config.
 """
@@ -49,10 +51,17 @@ WORKLOADS = {
                                     eps=0.5, seed=5),
     "48^3x64-f32-r18-coulomb-anneal": dict(dims=(48, 48, 48, 64), precision="fp32", R=18, gauge="coulomb",
                                            omega=1.7, eps=0.5, seed=5, anneal=True),
+    "48^3x64-f64-r18-coulomb-anneal": dict(dims=(48, 48, 48, 64), precision="fp64", R=18, gauge="coulomb",
+                                           omega=1.7, eps=0.5, seed=5, anneal=True),
+    "32^4-f64-r18-anneal": dict(dims=(32, 32, 32, 32), precision="fp64", R=18, gauge="landau", omega=1.7, eps=0.4, seed=3,
+                                anneal=True),
+    "32^4-f32-r12-anneal": dict(dims=(32, 32, 32, 32), precision="fp32", R=12, gauge="landau", omega=1.7, eps=0.4, seed=3,
+                                anneal=True),
 }
 # further workloads timed after the main one in the default run (lattices above 32^4: at most 3 steps each)
 ALSO_DEFAULT = ["32^4-f32-r12", "32^4-f64-r18", "32^4-f64-r12", "64^4-f32-r18", "64^4-f64-r18",
-                "48^3x64-f32-r18-coulomb", "48^3x64-f32-r18-coulomb-anneal", "16^3x32-f32-r18", "16^3x32-f64-r18"]
+                "48^3x64-f32-r18-coulomb", "48^3x64-f32-r18-coulomb-anneal", "48^3x64-f64-r18-coulomb-anneal",
+                "32^4-f64-r18-anneal", "32^4-f32-r12-anneal", "16^3x32-f32-r18", "16^3x32-f64-r18"]
 
 
 def volume(dims):
@@ -104,56 +113,66 @@ def device_canonical(U, gdims, dims, tiled):
 
 
 class ClockSampler:
-    """samples nvidia-smi clocks and throttle reasons while the timed region runs (B200_PROFILING.md)"""
-
-    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-             "clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons polled through NVML from a thread of this process (10 ms period), started
+    before the warm-up; summary() reports the samples that fall inside the timed region (B200_PROFILING.md)"""
 
     def __init__(self, index: int):
         self.index = index
-        self.proc = None
-        self.lines = []
+        self.samples = []  # (time.perf_counter(), sm MHz, power W, reasons bitmask)
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._err = None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thread = threading.Thread(target=self._read, daemon=True)
-            self.thread.start()
-        except OSError:
-            self.proc = None
+            import pynvml
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            pynvml.nvmlInit()
+            uuid_env = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            h = None
+            if uuid_env and not uuid_env.split(",")[0].isdigit():
+                try:
+                    h = pynvml.nvmlDeviceGetHandleByUUID(uuid_env.split(",")[self.index].encode())
+                except Exception:
+                    h = None
+            if h is None:
+                phys = int(uuid_env.split(",")[self.index]) if uuid_env and uuid_env.split(",")[0].isdigit() else self.index
+                h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+        except Exception as exc:  # NVML missing: report it, the run itself does not depend on it
+            self._err = f"NVML unavailable: {exc}"
+            return
+
+        def poll():
+            while not self._stop.is_set():
+                try:
+                    self.samples.append((time.perf_counter(), float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)),
+                                         pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0,
+                                         int(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h))))
+                except Exception:
+                    pass
+                self._stop.wait(0.01)
+
+        self._thread = threading.Thread(target=poll, daemon=True)
+        self._thread.start()
 
     def stop(self):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.lines:
-            f = [x.strip() for x in line.split(",")]
-            if len(f) < 7:
-                continue
-            try:
-                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
-            except ValueError:
-                continue
-            for name, val in zip(names, f[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join(timeout=2)
+
+    def summary(self, t0: float, t1: float):
+        if self._err is not None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [self._err], "samples": 0}
+        inside = [x for x in self.samples if t0 <= x[0] <= t1]
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+        reasons = sorted({n for x in inside for bit, n in names.items() if x[3] & bit})
+        sm = sorted(x[1] for x in inside)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": self.max_mhz,
+                "power_w_max": max((x[2] for x in inside), default=None), "samples": len(inside),
+                "samples_with_sw_power_cap": sum(1 for x in inside if x[3] & 0x4), "reasons": reasons,
+                "how": "NVML polled every 10 ms in-process, samples inside the timed region"}
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -184,6 +203,8 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
     Returns (seconds for K steps, seconds inside the sweep launches, launches, last F, last theta, clocks)."""
     import torch
 
+    if sampler is not None:
+        sampler.start()  # before the warm-up: the timed region of a fast workload is shorter than a sampler's start-up
     for _ in range(warmup):
         run_step(gfm, fx, w, sweeps, stream)
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
@@ -191,15 +212,18 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
     torch.cuda.synchronize()
     if barrier is not None:
         barrier()
-    if sampler is not None:
-        sampler.start()
     launches0 = gfm.gf_launch_count(fx.ctx)
+    h0 = time.perf_counter()
     t0.record(stream)
     for k in range(steps):
         F, th = run_step(gfm, fx, w, sweeps, stream, evs[k])
     t1.record(stream)
     torch.cuda.synchronize()
-    clocks = sampler.stop() if sampler is not None else None
+    h1 = time.perf_counter()
+    clocks = None
+    if sampler is not None:
+        sampler.stop()
+        clocks = sampler.summary(h0, h1)
     if barrier is not None:
         barrier()
     total = t0.elapsed_time(t1) * 1e-3
@@ -207,19 +231,56 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
     return total, in_sweeps, gfm.gf_launch_count(fx.ctx) - launches0, F, th, clocks
 
 
-def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None, total_s=None):
-    """dominant kernel = the half-sweep kernel: algorithmic bytes per launch = (V/2) * 16 R s"""
+def l2_copy_peak(nbytes: int) -> float:
+    """GB/s (read + write) of a device copy whose source and destination together are the size of the field and stay in
+    L2: the roof of a workload whose field is L2-resident (its half-sweep reads and writes the field once)"""
+    import torch
+
+    n = max(1, nbytes // 2 // 4)
+    a = torch.empty(n, dtype=torch.float32, device="cuda").normal_()
+    b = torch.empty_like(a)
+    for _ in range(5):
+        b.copy_(a)
+    best = 0.0
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(20):
+            b.copy_(a)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, 20 * 2 * n * 4 / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return best
+
+
+def roofline_entry(w, sweeps, steps, in_sweeps_s, traffic=None, total_s=None, l2_peak=None):
+    """dominant kernel = the half-sweep kernel: algorithmic bytes per launch = (V/2) * 16 R s.
+    achieved / frac: ALGORITHMIC bytes over the live CUDA-event duration, against the measured copy peak (for a field
+    that fits L2: against a measured L2-resident copy of the same size).  dram_*: the same duration with the DRAM bytes
+    one launch moved under ncu (profiles/r2_traffic.csv) -- below the algorithmic figure wherever L2 keeps part of the
+    field between half-sweeps (32^4: 0.87 of the bytes; 64^4 and 48^3x64: 0.98-1.0)."""
     peak, which = measured_peaks()
     per_launch_bytes = (volume(w["dims"]) // 2) * model_bytes_per_site_update(w["R"], w["precision"], w["gauge"],
                                                                               bool(w.get("anneal")))
     nlaunch = 2 * sweeps * steps
     avg_s = in_sweeps_s / nlaunch
     achieved = per_launch_bytes / avg_s / 1e9
-    return {"bound": "hbm", "kernel": "gf_half_sweep_kernel", "achieved": round(achieved, 1), "peak": peak,
-            "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": traffic,
-            "bytes_per_launch": per_launch_bytes, "avg_launch_us": round(avg_s * 1e6, 3), "peak_source": which,
-            "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
-            "share_of_step": round(in_sweeps_s / total_s, 4) if total_s else None}
+    out = {"bound": "hbm", "kernel": "gf_half_sweep_kernel", "achieved": round(achieved, 1), "peak": peak,
+           "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": traffic,
+           "bytes_per_launch": per_launch_bytes, "avg_launch_us": round(avg_s * 1e6, 3), "peak_source": which,
+           "achieved_kind": "effective: algorithmic bytes / CUDA-event time",
+           "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
+           "share_of_step": round(in_sweeps_s / total_s, 4) if total_s else None}
+    if traffic:
+        dram = traffic / avg_s / 1e9
+        out.update({"dram_achieved": round(dram, 1), "dram_frac": round(dram / peak, 4),
+                    "dram_frac_of_nominal_8TBs": round(dram / 8000.0, 4),
+                    "dram_kind": "ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch / the live CUDA-event time"})
+    if l2_peak:
+        out.update({"bound": "l2", "peak": round(l2_peak, 1), "frac": round(achieved / l2_peak, 4),
+                    "peak_source": "measured in this run: device copy with source + destination = field size, L2-resident "
+                                   "(torch b.copy_(a), best of 5 x 20)", "hbm_peak": peak})
+    return out
 
 
 def max_over_ranks(seconds: float, device) -> float:
@@ -239,24 +300,24 @@ def whole_job_value(world: int, V: int, sweeps: int, steps: int, seconds: float)
     return world * V * sweeps * steps / seconds
 
 
-def time_e2e(gfm, w, U_host_pinned, sweeps, steps, warmup):
-    """the host-buffer C-ABI call: H2D of the canonical field, pack, sweeps, F, theta, unpack, D2H -- all inside"""
+def time_e2e(gfm, w, hosts, sweeps, steps, warmup):
+    """the host-buffer C-ABI call on an ensemble: gf_overrelax_host_batch -- H2D of every canonical field, pack, sweeps,
+    F, theta, unpack, D2H, all inside the timed region; the copies of neighbouring configurations overlap the sweeps"""
     import torch
 
     prec = gfm.GF_FP64 if w["precision"] == "fp64" else gfm.GF_FP32
     ctx = gfm.gf_create(*w["dims"], prec, gfm.GF_COULOMB if w["gauge"] == "coulomb" else gfm.GF_LANDAU)
     gfm.gf_set_storage(ctx, w["R"])
-    call = gfm.gf_overrelax_host_f32 if U_host_pinned.dtype == torch.float32 else gfm.gf_overrelax_host
     for _ in range(warmup):
-        call(ctx, U_host_pinned, w["omega"], sweeps)
+        gfm.gf_overrelax_host_batch(ctx, hosts, w["omega"], sweeps)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for _ in range(steps):
-        call(ctx, U_host_pinned, w["omega"], sweeps)
+        gfm.gf_overrelax_host_batch(ctx, hosts, w["omega"], sweeps)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     gfm.gf_destroy(ctx)
-    nbytes = U_host_pinned.numel() * U_host_pinned.element_size()
+    nbytes = hosts[0].numel() * hosts[0].element_size()
     return dt, nbytes, nbytes + 16
 
 
@@ -336,6 +397,83 @@ def _print_json(line: dict) -> None:
         os.write(_JSON_FD, data)
 
 
+def field_bytes_of(wl):
+    return 4 * volume(wl["dims"]) * wl["R"] * (8 if wl["precision"] == "fp64" else 4)
+
+
+def main_shard(args, w, gfm, rank, world, local_rank, barrier, sweeps, steps, warmup):
+    """--shard t: ONE configuration cut into t-slabs over the ranks (strong scaling).  Each rank holds
+    its slab and a ghost slice; per half-sweep one face message goes up and one comes down per slab boundary
+    (torch.distributed point-to-point over NCCL).  Unmeasured on multi-GPU hardware in this run (no such node)."""
+    import numpy as np
+    import torch
+
+    import gf_inputs
+    from paper_1209_4008_b200 import slab
+
+    dims = w["dims"]
+    if w.get("anneal"):
+        raise SystemExit("bench.py --shard t: overrelaxation workloads only")
+    gdims = tuple(d // 2 for d in dims) if volume(dims) > 32**4 else dims
+    tiled = gdims != dims
+    import torch.distributed as dist
+
+    if dist.is_available() and dist.is_initialized():
+        run, (t0, t1) = slab.dist_slab(dims, w["precision"], w["gauge"], w["R"], overlap=True)
+    else:  # a plain one-GPU run: the whole lattice as one slab whose ghost is its own last slice
+        run, bounds = slab.local_slabs(dims, 1, w["precision"], w["gauge"], w["R"])
+        t0, t1 = bounds[0]
+    U = gf_inputs.smooth_random(gdims, w["eps"], w["seed"])
+    Vs = dims[0] * dims[1] * dims[2]
+    if tiled:
+        Nx, Ny, Nz, Nt = gdims
+        U = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(-1, 4, 3, 3)
+    eng = next(iter(run.eng.values()))
+    eng.load(np.ascontiguousarray(U[t0 * Vs: t1 * Vs]))
+    del U
+    kind = ("relax", 0, w["omega"], 0)
+
+    def step(s0):
+        for s in range(s0, s0 + sweeps):
+            run.sweep(kind, s)
+        return run.functional_theta()
+
+    run.begin()
+    done = 0
+    for _ in range(warmup):
+        step(done)
+        done += sweeps
+    torch.cuda.synchronize()
+    if barrier is not None:
+        barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        F, th = step(done)
+        done += sweeps
+    e1.record()
+    torch.cuda.synchronize()
+    if barrier is not None:
+        barrier()
+    total = max_over_ranks(e0.elapsed_time(e1) * 1e-3, "cuda")
+    if rank != 0:
+        return
+    V = volume(dims)
+    value = V * sweeps * steps / total
+    face = gfm.gf_slab_face_bytes(eng.ctx)
+    _print_json({
+        "metric": "site-updates/s", "value": value, "unit": "site-updates/s", "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": total / steps * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f64" if w["precision"] == "fp64" else "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "dims": list(dims), "gauge": w["gauge"], "reals_per_link": w["R"], "omega": w["omega"],
+                   "step": f"{sweeps} overrelaxation sweeps + F + theta (all-reduce of two sums)",
+                   "parallelism": f"one configuration in {world} t-slabs of {t1 - t0} timeslices; per half-sweep and slab boundary "
+                                  f"one face of {face} bytes up and one down (torch.distributed P2P), interior swept meanwhile"},
+        "gflops_paper_model": value * FLOP_PER_SITE / 1e9, "F": F, "theta": th, "gpu_launches": gfm.gf_launch_count(eng.ctx),
+        "e2e": None, "roofline": None, "cpu_baseline": None,
+    })
+
+
 def main():
     _reserve_stdout()
     ap = argparse.ArgumentParser()
@@ -352,9 +490,12 @@ def main():
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r1_traffic.csv"),
+    ap.add_argument("--e2e-configs", type=int, default=6, help="configurations per step of the end-to-end (host buffer) leg")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "t"],
+                    help="N > 1: independent replicas (default) or one configuration in t-slabs over the ranks")
+    ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r2_traffic.csv"),
                     help="ncu dram__bytes_read.sum / dram__bytes_write.sum per launch of the half-sweep kernel, per "
-                         "workload, from one `ncu --set full` capture (profiles/r1_ncu_half_sweep.md)")
+                         "workload (profiles/r2_traffic.md)")
     args = ap.parse_args()
     w = WORKLOADS[args.workload]
 
@@ -384,6 +525,13 @@ def main():
     stream = torch.cuda.Stream()
     sweeps, steps, warmup = args.sweeps_per_step, args.steps, max(args.warmup, 3)
 
+    if args.shard == "t":
+        main_shard(args, w, gfm, rank, world, local_rank, barrier, sweeps, steps, warmup)
+        if world > 1 or under_torchrun:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
     traffic = {}
     if os.path.exists(args.traffic_csv):
         import csv
@@ -401,14 +549,18 @@ def main():
         gfm.gf_set_tuning(fx.ctx, args.tps, args.block)
         del canon
         torch.cuda.synchronize()
+        fits = field_bytes_of(wl) <= L2_BYTES
         total, in_sw, launches, F, th, clocks = time_device(gfm, fx, wl, sweeps, steps, warmup, stream, bar, sampler)
         regs, spill = gfm.gf_kernel_info(fx.ctx, 1 if wl.get("anneal") else 0)
+        dc_launches, dc_sites = gfm.gf_chain_count(fx.ctx) if wl["precision"] == "fp32" else (0, 0)
         fx.close()
         del fx
         torch.cuda.empty_cache()
+        l2_peak = l2_copy_peak(field_bytes_of(wl)) if fits else None
         return dict(U=U if not tiled else None, total=total, in_sweeps=in_sw, launches=launches, F=F, theta=th,
-                    clocks=clocks, regs=regs, spill=spill, tiled=tiled, gdims=gdims,
-                    roofline=roofline_entry(wl, sweeps, steps, in_sw, traffic.get(name), total))
+                    clocks=clocks, regs=regs, spill=spill, tiled=tiled, gdims=gdims, fits_l2=fits,
+                    double_chain_launches=dc_launches, double_sites=dc_sites,
+                    roofline=roofline_entry(wl, sweeps, steps, in_sw, None if fits else traffic.get(name), total, l2_peak))
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
     m = measure(args.workload, w, sampler, barrier)
@@ -425,37 +577,41 @@ def main():
     # ---- rank 0, N = 1 extras: end-to-end through the host-buffer call, further workloads, the CPU baseline ----
     e2e = None
     if not args.no_e2e and not w.get("anneal"):
+        import numpy as np
+
         U = m["U"] if m["U"] is not None else base_field(dict(w, dims=m["gdims"]))[0]
         if m["tiled"]:
-            import numpy as np
-
             Nx, Ny, Nz, Nt = m["gdims"]
             U = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(-1, 4, 3, 3)
-        # an fp32 context takes its configuration as float (gf_overrelax_host_f32), an fp64 one as double
-        host = torch.from_numpy(U.view("float64").reshape(-1))
+        # an ensemble of nconf configurations in pinned host memory; an fp32 context takes them as float, an fp64 one as double
+        nconf = max(1, args.e2e_configs if field_bytes_of(w) < (2 << 30) else 2)
+        base = torch.from_numpy(U.view("float64").reshape(-1))
         if w["precision"] == "fp32":
-            host = host.to(torch.float32)
-        host = host.pin_memory()
-        e_steps = max(1, min(steps, 5))
-        dt, h2d, d2h = time_e2e(gfm, w, host, sweeps, e_steps, 1)
-        e2e = {"value": world * V * sweeps * e_steps / dt, "unit": "site-updates/s", "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "steps": e_steps, "ms_per_step": dt / e_steps * 1e3,
-               "call": ("gf_overrelax_host_f32" if w["precision"] == "fp32" else "gf_overrelax_host") +
-                       " (canonical field in pinned host memory in, fixed field + F + theta out; element type = the "
-                       "context's precision)"}
-        del host
+            base = base.to(torch.float32)
+        hosts = [base.clone().pin_memory() for _ in range(nconf)]
+        del base
+        e_steps = max(1, min(steps, 3))
+        dt, h2d, d2h = time_e2e(gfm, w, hosts, sweeps, e_steps, 1)
+        e2e = {"value": world * nconf * V * sweeps * e_steps / dt, "unit": "site-updates/s", "h2d_bytes_per_step": nconf * h2d,
+               "d2h_bytes_per_step": nconf * d2h, "steps": e_steps, "ms_per_step": dt / e_steps * 1e3,
+               "configurations_per_step": nconf, "ms_per_configuration": dt / e_steps / nconf * 1e3,
+               "call": f"gf_overrelax_host_batch: {nconf} canonical configurations in pinned host memory in, the fixed fields + "
+                       "F + theta out; upload of configuration i+1 and download of i-1 overlap the sweeps of i (three slots, "
+                       "three streams); element type = the context's precision"}
+        del hosts
 
     also = []
     for name in [n for n in args.also.split(",") if n and n != args.workload]:
         wl = WORKLOADS[name]
         Va = volume(wl["dims"])
-        a_steps = steps if Va <= 32**4 else min(steps, 3)
+        a_steps = min(steps, 5) if Va <= 32**4 else min(steps, 2)
         a = measure(name, wl, steps=a_steps)
         va = Va * sweeps * a_steps / a["total"]
         also.append({"workload": name, "value": va, "unit": "site-updates/s", "gflops_paper_model": va * FLOP_PER_SITE / 1e9,
                      "steps": a_steps, "ms_per_step": a["total"] / a_steps * 1e3,
-                     "fits_l2": 4 * Va * wl["R"] * (8 if wl["precision"] == "fp64" else 4) <= L2_BYTES, "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
-                     "regs_per_thread": a["regs"], "spill_bytes": a["spill"]})
+                     "fits_l2": a["fits_l2"], "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
+                     "regs_per_thread": a["regs"], "spill_bytes": a["spill"],
+                     "double_chain_launches": a["double_chain_launches"], "sites_redone_in_double": a["double_sites"]})
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -472,7 +628,15 @@ def main():
                "sample": f"{n} sweeps + F + theta on a {'x'.join(map(str, sdims))} lattice from the same generator "
                          f"(eps={w['eps']}, seed={w['seed']}), fp64, gcc -O2 -fopenmp"}
 
-    field_bytes = 4 * V * w["R"] * (8 if w["precision"] == "fp64" else 4)
+    field_bytes = field_bytes_of(w)
+    if field_bytes <= L2_BYTES:
+        l2_note = f"field {field_bytes / 2**20:.0f} MiB fits L2 (126 MiB): roofline against a measured L2-resident copy, not HBM"
+    elif field_bytes <= 4 * L2_BYTES:
+        l2_note = (f"inputs larger than L2: field {field_bytes / 2**20:.0f} MiB vs 126 MiB L2, no flush; L2-ASSISTED: the "
+                   "evict-last stores keep part of the field dirty in L2 between half-sweeps, the DRAM bytes of a launch are "
+                   "~0.87 of the algorithmic ones (roofline.dram_*); the 64^4 workloads in `also` are the L2-free figures")
+    else:
+        l2_note = f"inputs larger than L2: field {field_bytes / 2**20:.0f} MiB vs 126 MiB L2, no flush"
     line = {
         "metric": "site-updates/s", "value": value, "unit": "site-updates/s", "n_gpus": world, "steps": steps,
         "warmup": warmup, "ms_per_step": total / steps * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -483,14 +647,14 @@ def main():
                                          "gf_functional + gf_theta",
             "input": f"smooth-random eps={w['eps']} seed={w['seed']}" + (" on half extents, repeated 2x per direction"
                                                                           if m["tiled"] else ""),
-            "l2": f"inputs larger than L2: field {field_bytes / 2**20:.0f} MiB vs 126 MiB L2, no flush"
-                  if field_bytes > L2_BYTES else f"field {field_bytes / 2**20:.0f} MiB fits L2 (126 MiB): not a bandwidth figure",
+            "l2": l2_note,
             "parallelism": "replicas only" if world > 1 else "single GPU",
         },
         "gflops_paper_model": value * FLOP_PER_SITE / 1e9,
         "paper_context": "300 GFlops on GTX 580 (PAPER.md:13), another machine: context, not the target",
         "F": m["F"], "theta": m["theta"],
         "regs_per_thread": m["regs"], "spill_bytes": m["spill"],
+        "double_chain_launches": m["double_chain_launches"],
         "roofline": m["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
         "clocks": m["clocks"], "also": also,
     }

@@ -106,6 +106,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precisi
     c->precision = precision; c->gauge = gauge; c->R = 18;
     c->slab = slab; c->t_begin = t_begin; c->Nt_global = Nt_global;
     c->L.Nxh = Nx / 2; c->L.Ny = Ny; c->L.Nz = Nz; c->L.Nt = Nt + (slab ? 1 : 0); c->L.H = (unsigned)(V / 2);
+    c->L.Hp = (c->L.H + 31u) & ~31u;
     c->Hs = (unsigned)(Nx / 2) * (unsigned)Ny * (unsigned)Nz;
     c->H_own = c->Hs * (unsigned)Nt;
     c->tps = 0;   // 0 = automatic: resolved per (precision, storage, mode) by auto_tps()
@@ -199,7 +200,7 @@ extern "C" int gf_set_storage(gf_ctx* c, int R)
 extern "C" size_t gf_field_bytes(const gf_ctx* c)
 {
     if (c == nullptr) return 0;
-    return (size_t)8 * c->L.H * (size_t)c->R * real_size(c);
+    return (size_t)8 * c->L.Hp * (size_t)c->R * real_size(c); // whole tiles of 32 sites per link block
 }
 
 extern "C" int gf_set_tuning(gf_ctx* c, int tps, int block)
@@ -533,7 +534,7 @@ static int reading_b_begin(gf_ctx* c, int mode, cudaStream_t st, void** gfield, 
     *gfield = nullptr;
     if (!uses_reading_b(c, mode)) return GF_OK;
     cudaError_t e;
-    if (c->d_gfield == nullptr && (e = cudaMalloc(&c->d_gfield, (size_t)c->L.H * 2 * 18 * real_size(c))) != cudaSuccess) {
+    if (c->d_gfield == nullptr && (e = cudaMalloc(&c->d_gfield, (size_t)c->L.Hp * 2 * 18 * real_size(c))) != cudaSuccess) {
         c->d_gfield = nullptr;
         (void)cudaGetLastError();
         if (c->coulomb_b < 0) { // automatic choice and no room for the g(x) field: reading A needs none

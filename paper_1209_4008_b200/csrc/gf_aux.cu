@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) pack_kernel(Lattice L, unsigned H_o
     cx<T> u[9];
 #pragma unroll
     for (int e = 0; e < 9; ++e) u[e] = {(T)src[2 * e], (T)src[2 * e + 1]};
-    LinkIO<T, R>::store(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
+    LinkIO<T, R>::store(native + (size_t)l * R * L.Hp, L.Hp, h, u, make_l2_policy(POLICY_NORMAL));
 }
 
 template <typename T, int R, typename S>
@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) unpack_kernel(Lattice L, unsigned H
     const int l = (int)(gid / H_own), parity = l >> 2, mu = l & 3;
     const Site s = decode_site(L, h, parity);
     cx<T> u[9];
-    LinkIO<T, R>::load(native + (size_t)l * R * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
+    LinkIO<T, R>::load(native + (size_t)l * R * L.Hp, L.Hp, h, u, make_l2_policy(POLICY_NORMAL));
     S* dst = canon + ((size_t)canonical_index(s) * 4 + mu) * 18;
 #pragma unroll
     for (int e = 0; e < 9; ++e) { dst[2 * e] = (S)u[e].re; dst[2 * e + 1] = (S)u[e].im; }
@@ -87,35 +87,36 @@ cudaError_t launch_unpack_f32(int prec, int R, const Lattice& L, unsigned H_own,
     return launch_unpack_t<float>(prec, R, L, H_own, native, canon, st);
 }
 
-// t-slab faces (NEXT-4): the temporal links of one parity block of one timeslice, gathered plane by plane into a
-// contiguous message / scattered back.  One thread per 128-bit vector of the slice.
+// t-slab faces (NEXT-4): the temporal links of one parity block of one timeslice, gathered into a contiguous message
+// (plane-major: real k of site i at k/VEC * Hs * VEC + i * VEC + k % VEC, fp32 R18 tail plane behind the float4 planes)
+// / scattered back.  One thread per site of the face.
 template <typename T, int R, bool PACK>
 __global__ void __launch_bounds__(AUX_BLOCK) face_kernel(Lattice L, unsigned Hs, int t, int block_parity, T* __restrict__ native,
                                                          T* __restrict__ buf)
 {
-    constexpr int VEC = 16 / sizeof(T);                 // reals per 128-bit vector
-    const unsigned idx = blockIdx.x * blockDim.x + threadIdx.x; // real pair / quad index inside the face
-    const unsigned nvec = Hs * (unsigned)(R / VEC);     // fp32 R18: the 64-bit tail plane is handled below
-    T* blk = native + (size_t)(block_parity * 4 + 3) * R * L.H;
-    if (idx < nvec) {
-        const unsigned plane = idx / Hs, i = idx % Hs;
-        T* a = blk + ((size_t)plane * L.H + (size_t)t * Hs + i) * VEC;
-        T* b = buf + (size_t)idx * VEC;
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Hs) return;
+    constexpr int VEC = 16 / sizeof(T), NV = R / VEC; // whole 128-bit vectors per link; fp32 R18: plus two reals
+    T* blk = native + (size_t)(block_parity * 4 + 3) * R * L.Hp;
+    const size_t h = (size_t)t * Hs + i;
+    T* a = blk + (h >> 5) * (size_t)(R * TILE) + (h & 31) * VEC; // plane 0 of this site inside its tile
 #pragma unroll
-        for (int k = 0; k < VEC; ++k) { if (PACK) b[k] = a[k]; else a[k] = b[k]; }
+    for (int v = 0; v < NV; ++v) {
+        T* b = buf + ((size_t)v * Hs + i) * VEC;
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) { if (PACK) b[k] = a[v * TILE * VEC + k]; else a[v * TILE * VEC + k] = b[k]; }
     }
-    if (sizeof(T) == 4 && R == 18 && idx < Hs) { // trailing float2 plane at real offset 16 H
-        T* a = blk + (size_t)16 * L.H + ((size_t)t * Hs + idx) * 2;
-        T* b = buf + (size_t)16 * Hs + (size_t)idx * 2;
-        if (PACK) { b[0] = a[0]; b[1] = a[1]; } else { a[0] = b[0]; a[1] = b[1]; }
+    if (sizeof(T) == 4 && R == 18) {
+        T* a2 = blk + (h >> 5) * (size_t)(R * TILE) + 16 * TILE + (h & 31) * 2;
+        T* b = buf + (size_t)16 * Hs + (size_t)i * 2;
+        if (PACK) { b[0] = a2[0]; b[1] = a2[1]; } else { a2[0] = b[0]; a2[1] = b[1]; }
     }
 }
 
 cudaError_t launch_face(int prec, int R, const Lattice& L, unsigned Hs, int t, int block_parity, bool pack, void* native,
                         void* buf, cudaStream_t st)
 {
-    const unsigned nvec = Hs * (unsigned)(R / (prec == 0 ? 4 : 2));
-    const unsigned grid = (nvec + AUX_BLOCK - 1) / AUX_BLOCK;
+    const unsigned grid = (Hs + AUX_BLOCK - 1) / AUX_BLOCK;
 #define GF_FACE(T, RR)                                                                                              \
     do {                                                                                                            \
         if (pack) face_kernel<T, RR, true><<<grid, AUX_BLOCK, 0, st>>>(L, Hs, t, block_parity, (T*)native, (T*)buf);  \
@@ -140,14 +141,14 @@ __global__ void __launch_bounds__(AUX_BLOCK) convert_kernel(Lattice L, const TS*
     const int l = (int)(gid / L.H);
     const uint64_t pol = make_l2_policy(POLICY_NORMAL);
     cx<TS> u[9];
-    LinkIO<TS, RS>::load(src + (size_t)l * RS * L.H, L.H, h, u, pol);
+    LinkIO<TS, RS>::load(src + (size_t)l * RS * L.Hp, L.Hp, h, u, pol);
     cx<TD> v[9];
 #pragma unroll
     for (int e = 0; e < 9; ++e) v[e] = {(TD)u[e].re, (TD)u[e].im};
     // widening: the fp32 links are unitary to 1e-7 only; Gram-Schmidt in the wider type makes the fp64 field an
     // SU(3) field to rounding, so that the polish starts from a proper configuration (C15)
     if (sizeof(TD) > sizeof(TS)) reunitarise(v);
-    LinkIO<TD, RD>::store(dst + (size_t)l * RD * L.H, L.H, h, v, pol);
+    LinkIO<TD, RD>::store(dst + (size_t)l * RD * L.Hp, L.Hp, h, v, pol);
 }
 
 template <typename TS, int RS>
@@ -184,7 +185,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) coulomb_init_kernel(Lattice L, T* _
     cx<T> u[9];
 #pragma unroll
     for (int e = 0; e < 9; ++e) u[e] = {(e % 4 == 0) ? T(1) : T(0), T(0)};
-    LinkIO<T, 18>::store(G + (size_t)parity * 18 * L.H, L.H, h, u, make_l2_policy(POLICY_NORMAL));
+    LinkIO<T, 18>::store(G + (size_t)parity * 18 * L.Hp, L.Hp, h, u, make_l2_policy(POLICY_NORMAL));
 }
 
 template <typename T, int R>
@@ -200,10 +201,10 @@ __global__ void __launch_bounds__(AUX_BLOCK) coulomb_finish_kernel(Lattice L, T*
     const unsigned st = (unsigned)L.Nxh * (unsigned)L.Ny * (unsigned)L.Nz;
     const unsigned hf = s.t == L.Nt - 1 ? h - st * (unsigned)(L.Nt - 1) : h + st;
     cx<T> u[9], g[9], gn[9], t[9];
-    T* blk = native + (size_t)(parity * 4 + 3) * R * L.H;
-    LinkIO<T, R>::load(blk, L.H, h, u, pol);
-    LinkIO<T, 18>::load(G + (size_t)parity * 18 * L.H, L.H, h, g, pol);
-    LinkIO<T, 18>::load(G + (size_t)(1 - parity) * 18 * L.H, L.H, hf, gn, pol);
+    T* blk = native + (size_t)(parity * 4 + 3) * R * L.Hp;
+    LinkIO<T, R>::load(blk, L.Hp, h, u, pol);
+    LinkIO<T, 18>::load(G + (size_t)parity * 18 * L.Hp, L.Hp, h, g, pol);
+    LinkIO<T, 18>::load(G + (size_t)(1 - parity) * 18 * L.Hp, L.Hp, hf, gn, pol);
 #pragma unroll
     for (int r = 0; r < 3; ++r)
 #pragma unroll
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) coulomb_finish_kernel(Lattice L, T*
 #pragma unroll
         for (int c = 0; c < 3; ++c)
             u[3 * r + c] = cmul_cb(t[3 * r], gn[3 * c]) + cmul_cb(t[3 * r + 1], gn[3 * c + 1]) + cmul_cb(t[3 * r + 2], gn[3 * c + 2]);
-    LinkIO<T, R>::store(blk, L.H, h, u, pol);
+    LinkIO<T, R>::store(blk, L.Hp, h, u, pol);
 }
 
 cudaError_t launch_coulomb_init(int prec, const Lattice& L, void* G, cudaStream_t st)
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__(AUX_BLOCK) functional_kernel(Lattice L, int nd
     if (local < Hs) {
         const unsigned h = (unsigned)t * Hs + local;
         for (int mu = 0; mu < nd; ++mu)
-            acc += (double)LinkIO<T, R>::trace_re(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, h, pol);
+            acc += (double)LinkIO<T, R>::trace_re(native + (size_t)(parity * 4 + mu) * R * L.Hp, L.Hp, h, pol);
     }
     block_sum_to(acc, partials + (size_t)blockIdx.y * gridDim.x + blockIdx.x);
 }
@@ -300,8 +301,8 @@ __global__ void __launch_bounds__(AUX_BLOCK) theta_kernel(Lattice L, int nd, con
         for (int mu = 0; mu < 4; ++mu) { // unrolled: the loads of all directions are in flight together
             if (mu >= nd) break;
             cx<T> f[9], b[9];
-            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.H, L.H, s.h, f, pol);
-            LinkIO<T, R>::load(native + (size_t)((1 - parity) * 4 + mu) * R * L.H, L.H, backward_neighbour(L, s, mu), b, pol);
+            LinkIO<T, R>::load(native + (size_t)(parity * 4 + mu) * R * L.Hp, L.Hp, s.h, f, pol);
+            LinkIO<T, R>::load(native + (size_t)((1 - parity) * 4 + mu) * R * L.Hp, L.Hp, backward_neighbour(L, s, mu), b, pol);
 #pragma unroll
             for (int r = 0; r < 3; ++r)
 #pragma unroll

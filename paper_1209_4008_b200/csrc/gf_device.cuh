@@ -3,13 +3,17 @@
 //
 // Native layout ("Data layout in HBM").  H = V/2 sites per parity.  Half-site index of a site
 // (x,y,z,t) of parity p = (x+y+z+t)&1:   h = (x>>1) + (Nx/2) * (y + Ny * (z + Nz * t)).
-// Link U_mu(x) lives in link block  l = p*4 + mu  (parity-split: PAPER.md:124), which holds R*H reals.
-// Inside a block the complex entries e = 3*row + col (e < R/2; R = 12 stores rows 0,1 only) are
-// component-major with the site index fastest, grouped in 128-bit vectors:
-//   fp64: plane e is H double2 (re,im)                          -> real offset  e*2*H + 2*h
-//   fp32: plane q = e/2 is H float4 (re,im of e=2q; re,im of e=2q+1) -> real offset  q*4*H + 4*h
-//         R = 18: the ninth entry (e = 8) is a trailing plane of H float2 at real offset 16*H + 2*h
-// so a warp's load of one plane is one contiguous 512-byte (fp32: 512 or 256) run.
+// Link U_mu(x) lives in link block  l = p*4 + mu  (parity-split: PAPER.md:124), which holds R*Hp reals, Hp = H rounded
+// up to a multiple of 32.  Inside a block the sites are grouped in TILES of 32 consecutive half-sites (one warp's worth);
+// inside a tile the complex entries e = 3*row + col (e < R/2; R = 12 stores rows 0,1 only) are
+// component-major with the site index fastest, in 128-bit vectors:
+//   fp64: tile = R/2 planes of 32 double2 (re,im)                      -> real offset  (h>>5)*R*32 + e*64 + 2*(h&31)
+//   fp32: tile = R/4 planes of 32 float4 (re,im of e=2q; re,im of e=2q+1) -> real offset  (h>>5)*R*32 + q*128 + 4*(h&31)
+//         R = 18: the ninth entry (e = 8) is a trailing plane of 32 float2 at  (h>>5)*R*32 + 512 + 2*(h&31)
+// so a warp's load of one plane is one contiguous 512-byte (fp32 tail: 256-byte) run, as with whole-lattice planes, but
+// all planes of a link sit at CONSTANT offsets from one address per thread: one address computation per link instead
+// of one per plane (the half-sweep spent 15 % of its instructions on 64-bit address arithmetic), and a site's link is
+// one 2.3 KB (fp32 R18) stretch of a DRAM page instead of five pages.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -214,108 +218,119 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 
 template <typename T, int R> struct LinkIO;
 
+constexpr int TILE = 32; // sites per tile of the native layout
+
 template <int R>
 struct LinkIO<double, R> {
     static constexpr int NE = R / 2;
-    // blk: first real of the link block; H: sites per parity; h: half-site index
-    static __device__ __forceinline__ void load(const double* blk, size_t H, size_t h, cx<double> (&u)[9], uint64_t pol)
+    // blk: first real of the link block; Hp: padded sites per block (unused: the tiles carry the layout); h: half-site index
+    static __device__ __forceinline__ const double2* at(const double* blk, size_t h)
     {
-        const double2* p = reinterpret_cast<const double2*>(blk) + h;
+        return reinterpret_cast<const double2*>(blk) + (h >> 5) * (size_t)(NE * TILE) + (h & 31);
+    }
+    static __device__ __forceinline__ void load(const double* blk, size_t, size_t h, cx<double> (&u)[9], uint64_t pol)
+    {
+        const double2* p = at(blk, h);
 #pragma unroll
         for (int e = 0; e < NE; ++e) {
-            double2 v = ldg(p + (size_t)e * H, pol);
+            double2 v = ldg(p + e * TILE, pol);
             u[e] = {v.x, v.y};
         }
         if (R == 12) rebuild_row2(u);
     }
     // Re tr U from the diagonal planes alone (R = 12: rows 0,1 in full, entry (2,2) rebuilt)
-    static __device__ __forceinline__ double trace_re(const double* blk, size_t H, size_t h, uint64_t pol)
+    static __device__ __forceinline__ double trace_re(const double* blk, size_t Hp, size_t h, uint64_t pol)
     {
-        const double2* p = reinterpret_cast<const double2*>(blk) + h;
-        if (R == 18) return ldg(p, pol).x + ldg(p + 4 * H, pol).x + ldg(p + 8 * H, pol).x;
+        const double2* p = at(blk, h);
+        if (R == 18) return ldg(p, pol).x + ldg(p + 4 * TILE, pol).x + ldg(p + 8 * TILE, pol).x;
         cx<double> u[9];
-        load(blk, H, h, u, pol);
+        load(blk, Hp, h, u, pol);
         return u[0].re + u[4].re + u[8].re;
     }
-    static __device__ __forceinline__ void prefetch(const double* blk, size_t H, size_t h)
+    static __device__ __forceinline__ void prefetch(const double* blk, size_t, size_t h)
     {
-        const double2* p = reinterpret_cast<const double2*>(blk) + h;
+        const double2* p = at(blk, h);
 #pragma unroll
-        for (int e = 0; e < NE; ++e) prefetch_l2(p + (size_t)e * H);
+        for (int e = 0; e < NE; ++e) prefetch_l2(p + e * TILE);
     }
-    static __device__ __forceinline__ void store(double* blk, size_t H, size_t h, const cx<double> (&u)[9], uint64_t pol)
+    static __device__ __forceinline__ void store(double* blk, size_t, size_t h, const cx<double> (&u)[9], uint64_t pol)
     {
-        double2* p = reinterpret_cast<double2*>(blk) + h;
+        double2* p = const_cast<double2*>(at(blk, h));
 #pragma unroll
-        for (int e = 0; e < NE; ++e) stg(p + (size_t)e * H, make_double2(u[e].re, u[e].im), pol);
+        for (int e = 0; e < NE; ++e) stg(p + e * TILE, make_double2(u[e].re, u[e].im), pol);
     }
 };
 
 template <int R>
 struct LinkIO<float, R> {
     static constexpr int NQ = R / 4; // float4 planes: 4 (R18) or 3 (R12)
+    static __device__ __forceinline__ const float* tile(const float* blk, size_t h) { return blk + (h >> 5) * (size_t)(R * TILE); }
     // the stored entries only (R = 12: u[6..8] untouched)
-    static __device__ __forceinline__ void load_stored(const float* blk, size_t H, size_t h, cx<float> (&u)[9], uint64_t pol)
+    static __device__ __forceinline__ void load_stored(const float* blk, size_t, size_t h, cx<float> (&u)[9], uint64_t pol)
     {
-        const float4* p = reinterpret_cast<const float4*>(blk) + h;
+        const float* t = tile(blk, h);
+        const float4* p = reinterpret_cast<const float4*>(t) + (h & 31);
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
-            float4 v = ldg(p + (size_t)q * H, pol);
+            float4 v = ldg(p + q * TILE, pol);
             u[2 * q] = {v.x, v.y};
             u[2 * q + 1] = {v.z, v.w};
         }
         if (R == 18) {
-            float2 v = ldg(reinterpret_cast<const float2*>(blk + 16 * H) + h, pol);
+            float2 v = ldg(reinterpret_cast<const float2*>(t + 16 * TILE) + (h & 31), pol);
             u[8] = {v.x, v.y};
         }
     }
-    static __device__ __forceinline__ void load(const float* blk, size_t H, size_t h, cx<float> (&u)[9], uint64_t pol)
+    static __device__ __forceinline__ void load(const float* blk, size_t Hp, size_t h, cx<float> (&u)[9], uint64_t pol)
     {
-        load_stored(blk, H, h, u, pol);
+        load_stored(blk, Hp, h, u, pol);
         if (R == 12) rebuild_row2(u);
     }
     // float storage, double arithmetic (the rare-path fix-up of the fp32 sweep, gf_sweep.cuh): the stored floats are
     // widened exactly; R = 12: row 2 is rebuilt in double
-    static __device__ __forceinline__ void load(const float* blk, size_t H, size_t h, cx<double> (&u)[9], uint64_t pol)
+    static __device__ __forceinline__ void load(const float* blk, size_t Hp, size_t h, cx<double> (&u)[9], uint64_t pol)
     {
         cx<float> v[9];
-        load_stored(blk, H, h, v, pol);
+        load_stored(blk, Hp, h, v, pol);
 #pragma unroll
         for (int e = 0; e < R / 2; ++e) u[e] = {(double)v[e].re, (double)v[e].im};
         if (R == 12) rebuild_row2(u);
     }
-    static __device__ __forceinline__ void store(float* blk, size_t H, size_t h, const cx<double> (&u)[9], uint64_t pol)
+    static __device__ __forceinline__ void store(float* blk, size_t Hp, size_t h, const cx<double> (&u)[9], uint64_t pol)
     {
         cx<float> v[9];
 #pragma unroll
         for (int e = 0; e < 9; ++e) v[e] = {(float)u[e].re, (float)u[e].im};
-        store(blk, H, h, v, pol);
+        store(blk, Hp, h, v, pol);
     }
-    static __device__ __forceinline__ double trace_re(const float* blk, size_t H, size_t h, uint64_t pol)
+    static __device__ __forceinline__ double trace_re(const float* blk, size_t Hp, size_t h, uint64_t pol)
     {
         if (R == 18) {
-            const float4* p = reinterpret_cast<const float4*>(blk) + h;
-            return (double)ldg(p, pol).x + (double)ldg(p + 2 * H, pol).x +
-                   (double)ldg(reinterpret_cast<const float2*>(blk + 16 * H) + h, pol).x;
+            const float* t = tile(blk, h);
+            const float4* p = reinterpret_cast<const float4*>(t) + (h & 31);
+            return (double)ldg(p, pol).x + (double)ldg(p + 2 * TILE, pol).x +
+                   (double)ldg(reinterpret_cast<const float2*>(t + 16 * TILE) + (h & 31), pol).x;
         }
         cx<float> u[9];
-        load(blk, H, h, u, pol);
+        load(blk, Hp, h, u, pol);
         return (double)u[0].re + (double)u[4].re + (double)u[8].re;
     }
-    static __device__ __forceinline__ void prefetch(const float* blk, size_t H, size_t h)
+    static __device__ __forceinline__ void prefetch(const float* blk, size_t, size_t h)
     {
-        const float4* p = reinterpret_cast<const float4*>(blk) + h;
+        const float* t = tile(blk, h);
+        const float4* p = reinterpret_cast<const float4*>(t) + (h & 31);
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) prefetch_l2(p + (size_t)q * H);
-        if (R == 18) prefetch_l2(reinterpret_cast<const float2*>(blk + 16 * H) + h);
+        for (int q = 0; q < NQ; ++q) prefetch_l2(p + q * TILE);
+        if (R == 18) prefetch_l2(reinterpret_cast<const float2*>(t + 16 * TILE) + (h & 31));
     }
-    static __device__ __forceinline__ void store(float* blk, size_t H, size_t h, const cx<float> (&u)[9], uint64_t pol)
+    static __device__ __forceinline__ void store(float* blk, size_t, size_t h, const cx<float> (&u)[9], uint64_t pol)
     {
-        float4* p = reinterpret_cast<float4*>(blk) + h;
+        float* t = const_cast<float*>(tile(blk, h));
+        float4* p = reinterpret_cast<float4*>(t) + (h & 31);
 #pragma unroll
         for (int q = 0; q < NQ; ++q)
-            stg(p + (size_t)q * H, make_float4(u[2 * q].re, u[2 * q].im, u[2 * q + 1].re, u[2 * q + 1].im), pol);
-        if (R == 18) stg(reinterpret_cast<float2*>(blk + 16 * H) + h, make_float2(u[8].re, u[8].im), pol);
+            stg(p + q * TILE, make_float4(u[2 * q].re, u[2 * q].im, u[2 * q + 1].re, u[2 * q + 1].im), pol);
+        if (R == 18) stg(reinterpret_cast<float2*>(t + 16 * TILE) + (h & 31), make_float2(u[8].re, u[8].im), pol);
     }
 };
 
@@ -326,6 +341,7 @@ struct LinkIO<float, R> {
 struct Lattice {
     int Nxh, Ny, Nz, Nt; // Nxh = Nx/2
     unsigned H;          // V/2
+    unsigned Hp;         // H rounded up to whole tiles of 32 sites: sites per link block in memory
 };
 
 struct Site {

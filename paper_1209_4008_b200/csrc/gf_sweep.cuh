@@ -367,7 +367,7 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
     using IO = LinkIO<float, R>;
     using GIO = LinkIO<float, 18>;
     const Site s = decode_site(p.L, h, ph.parity);
-    const size_t H = p.L.H;
+    const size_t Hp = p.L.Hp;
     float* const base = reinterpret_cast<float*>(p.U);
     const uint64_t ld = make_l2_policy(POLICY_NORMAL), st = make_l2_policy(p.st_policy);
     cx<double> K[9];
@@ -375,8 +375,8 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
     for (int e = 0; e < 9; ++e) K[e] = {0.0, 0.0};
     for (int mu = 0; mu < p.nd; ++mu) { // eq. 2.3 (C2), every direction entering K
         cx<double> f[9], b[9];
-        IO::load(base + (size_t)(ph.parity * 4 + mu) * R * H, H, s.h, f, ld);
-        IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, backward_neighbour(p.L, s, mu), b, ld);
+        IO::load(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, s.h, f, ld);
+        IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, backward_neighbour(p.L, s, mu), b, ld);
         if (ph.reunit) { reunitarise(f); reunitarise(b); }
 #pragma unroll
         for (int r = 0; r < 3; ++r)
@@ -393,31 +393,31 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
         const int mu = lane_mu0 + m;
         if (CB && mu == 3) continue;
         cx<double> u[9];
-        float* const fb = base + (size_t)(ph.parity * 4 + mu) * R * H;
-        IO::load(fb, H, s.h, u, ld);
+        float* const fb = base + (size_t)(ph.parity * 4 + mu) * R * Hp;
+        IO::load(fb, Hp, s.h, u, ld);
         if (ph.reunit) reunitarise(u);
         su2_left<0, 1>(a0, b0, u); // U_mu(x) <- G U_mu(x)
         su2_left<0, 2>(a1, b1, u);
         su2_left<1, 2>(a2, b2, u);
-        IO::store(fb, H, s.h, u, st);
-        float* const bb = base + (size_t)((1 - ph.parity) * 4 + mu) * R * H;
+        IO::store(fb, Hp, s.h, u, st);
+        float* const bb = base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp;
         const unsigned hb = backward_neighbour(p.L, s, mu);
-        IO::load(bb, H, hb, u, ld);
+        IO::load(bb, Hp, hb, u, ld);
         if (ph.reunit) reunitarise(u);
         su2_right_dagger<0, 1, 3>(a0, b0, u); // U_mu(x-mu) <- U_mu(x-mu) G^dagger
         su2_right_dagger<0, 2, 3>(a1, b1, u);
         su2_right_dagger<1, 2, 3>(a2, b2, u);
-        IO::store(bb, H, hb, u, st);
+        IO::store(bb, Hp, hb, u, st);
     }
     if (CB && lane_mu0 + NMU - 1 == 3) { // reading B: G(x) <- g G(x)
         cx<double> u[9];
-        float* const gb = reinterpret_cast<float*>(p.G) + (size_t)ph.parity * 18 * H;
-        GIO::load(gb, H, s.h, u, ld);
+        float* const gb = reinterpret_cast<float*>(p.G) + (size_t)ph.parity * 18 * Hp;
+        GIO::load(gb, Hp, s.h, u, ld);
         if (ph.reunit) reunitarise(u);
         su2_left<0, 1>(a0, b0, u);
         su2_left<0, 2>(a1, b1, u);
         su2_left<1, 2>(a2, b2, u);
-        GIO::store(gb, H, s.h, u, st);
+        GIO::store(gb, Hp, s.h, u, st);
     }
     if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
 }
@@ -657,6 +657,7 @@ struct SweepKernel {
     static __device__ __forceinline__ void issue_prefetch(const SweepParams& p, const SweepPhase& ph, const Site& s,
                                                           const unsigned (&hb)[NMU], int lane_mu0, T* base, size_t H)
     {
+        const size_t Hp = p.L.Hp;
         if (p.prefetch) {
             const long long d = ph.reverse ? -(long long)p.prefetch : (long long)p.prefetch;
             const long long hf = (long long)s.h + d;
@@ -666,8 +667,8 @@ struct SweepKernel {
                     const int mu = lane_mu0 + m;
                     const long long hbd = (long long)hb[m] + d;
                     if (CB && mu == 3) continue;
-                    IO::prefetch(base + (size_t)(ph.parity * 4 + mu) * R * H, H, (size_t)hf);
-                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, (size_t)hbd);
+                    IO::prefetch(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, (size_t)hf);
+                    if (hbd >= 0 && hbd < (long long)H) IO::prefetch(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, (size_t)hbd);
                 }
             }
         }
@@ -684,7 +685,7 @@ struct SweepKernel {
                                                        const int* mon_frozen, double (&mon_out)[3])
     {
         const Site s = decode_site(p.L, slot, ph.parity);
-        const size_t H = p.L.H;
+        const size_t H = p.L.H, Hp = p.L.Hp;
         T* const base = reinterpret_cast<T*>(p.U);
 
         const MemPolicy pol = {make_l2_policy(p.ld_policy), make_l2_policy(p.st_policy)};
@@ -718,12 +719,12 @@ struct SweepKernel {
         for (int m = 0; m < NMU; ++m) {
             const int mu = lane_mu0 + m;
             if (CB && mu == 3) continue;
-            IO::load(base + (size_t)(ph.parity * 4 + mu) * R * H, H, s.h, F[m], pol.ld);
-            IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.ld);
+            IO::load(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, s.h, F[m], pol.ld);
+            IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, hb[m], B[m], pol.ld);
         }
         cx<T> Gt[9];
         const bool owns_t = CB && (lane_mu0 + NMU - 1 == 3); // the thread that would hold the temporal links
-        if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)ph.parity * 18 * H, H, s.h, Gt, pol.ld);
+        if (owns_t) GIO::load(reinterpret_cast<const T*>(p.G) + (size_t)ph.parity * 18 * Hp, Hp, s.h, Gt, pol.ld);
         if (MODE == MODE_HEATBATH) issue_prefetch(p, ph, s, hb, lane_mu0, base, H);
         // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
         const uint32_t sc = canonical_index(s) + p.site_offset;
@@ -797,10 +798,10 @@ struct SweepKernel {
         for (int m = 0; m < NMU; ++m) {
             const int mu = lane_mu0 + m;
             if (CB && mu == 3) continue;
-            IO::store(base + (size_t)(ph.parity * 4 + mu) * R * H, H, s.h, F[m], pol.st);
-            IO::store(base + (size_t)((1 - ph.parity) * 4 + mu) * R * H, H, hb[m], B[m], pol.st);
+            IO::store(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, s.h, F[m], pol.st);
+            IO::store(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, hb[m], B[m], pol.st);
         }
-        if (owns_t) GIO::store(reinterpret_cast<T*>(p.G) + (size_t)ph.parity * 18 * H, H, s.h, Gt, pol.st);
+        if (owns_t) GIO::store(reinterpret_cast<T*>(p.G) + (size_t)ph.parity * 18 * Hp, Hp, s.h, Gt, pol.st);
     }
 
     static __device__ __forceinline__ void run(const SweepParams& p)
