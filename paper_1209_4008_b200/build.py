@@ -22,6 +22,7 @@ LIB = os.path.join(HERE, "libgf.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+FLAGS += os.environ.get("GF_NVCC_EXTRA", "").split()  # tuning experiments: extra -D switches (none in a normal build)
 
 # (object name, source, extra defines).  The sweep kernels of one (precision, reals-per-link) are three units
 # (gf_sweep_inst.cu: relaxation + launcher, monitored relaxation, heatbath), twelve in all.

@@ -346,7 +346,7 @@ static cudaError_t launch_sweep(gf_ctx* c, int mode, const SweepParams& p_in, cu
     const int tps = auto_tps(c, mode), block = auto_block(c);
     SweepParams p = p_in;
     p.prefetch = (unsigned)auto_prefetch(c, mode);
-    if (mode == MODE_HEATBATH) p.watch_thr2 = c->chain == CHAIN_FP32 ? 0.0f : c->fix_threshold * c->fix_threshold;
+    if (mode == MODE_HEATBATH) p.watch_thr2 = c->chain == CHAIN_FP32 ? -1.0f : c->fix_threshold * c->fix_threshold;
     if (c->precision == GF_FP32) return c->R == 18 ? launch_sweep_f32_r18(tps, mode, block, p, st) : launch_sweep_f32_r12(tps, mode, block, p, st);
     return c->R == 18 ? launch_sweep_f64_r18(tps, mode, block, p, st) : launch_sweep_f64_r12(tps, mode, block, p, st);
 }

@@ -185,6 +185,22 @@ __device__ __forceinline__ void su2_variant_step(const T (&k)[4], int variant, d
 // Kennedy-Pendleton, hvec uniform on the sphere; g = h (x) conj(khat).
 // Uniforms: u = (2 (x >> 9) + 1) 2^-24, exact in fp32 and fp64.
 // ---------------------------------------------------------------------------------------------------------
+// One Kennedy-Pendleton trial (C14) splits into a part that depends on the random numbers alone,
+//     s = -ln u1 cos^2(2 pi u3) - ln u2,   u4,
+// and the part that needs K:  delta = s / alpha,  accept iff u4^2 <= 1 - delta/2.  The first part of trial 0 and the unit
+// vector of the direction of hvec are computed up front, while the link loads are in flight (EarlyDraw), for the three
+// subgroups at once -- independent chains the scheduler can interleave; behind K only two multiplications and a
+// compare are left on the critical path of a subgroup step.
+template <typename DT> struct TrialPre {
+    DT s;     // l1 c^2 + l2, l = -ln u
+    DT lsum;  // 1 + l1 + l2: scale of the absolute error of the SFU value of s (fp32 draw only)
+    DT u4;
+};
+template <typename DT> struct EarlyDraw {
+    TrialPre<DT> t0;  // trial 0
+    DT e1, e2, e3;    // direction of hvec, from the Philox block with counter word 3 = 0x80000000
+};
+
 template <typename T> struct KPMath;
 // fp64: the draw is evaluated in double like the oracle's, with correctly-rounded-to-1-ulp library functions (log,
 // cospi/sinpi) but without IEEE divisions and square roots (1/|k| by rsqrt, delta as one fused expression times
@@ -193,93 +209,140 @@ template <typename T> struct KPMath;
 // within ~1e-15 of the threshold, i.e. with probability ~1e-15 per trial (tests compare every trial count).
 template <> struct KPMath<double> {
     static __device__ __forceinline__ double uni(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
-    static __device__ __forceinline__ double cos2pi(double u) { return cospi(2.0 * u); }
-    static __device__ __forceinline__ double sin2pi(double u) { return sinpi(2.0 * u); }
     static __device__ __forceinline__ double neglog(double u) { return -log(u); }
     static __device__ __forceinline__ double root(double x) { return x > 0.0 ? x * rsqrt(x) : 0.0; }
-    // one Kennedy-Pendleton trial from its Philox block (C14): delta, accept iff u4^2 <= 1 - delta/2
-    static __device__ __forceinline__ bool trial(const uint32_t (&x)[4], double n2, double Td, double inv_alpha, double& d,
-                                                 double& est)
+    // the angle of a trial (u3) as it enters sincos2pi; cos^2 of it from the cosine
+    static __device__ __forceinline__ double trial_angle(double u3) { return u3; }
+    static __device__ __forceinline__ double cos_squared(double c) { return c * c; }
+    static __device__ __forceinline__ void sincos2pi(double a, double& sn, double& cs) { sincospi(2.0 * a, &sn, &cs); }
+    static __device__ __forceinline__ bool decide(const TrialPre<double>& t, double inv_alpha, double& d, double& est, bool& border)
     {
-        (void)n2; (void)Td;
+        (void)border;
         est = 0.0; // never refined
-        const double c = cos2pi(uni(x[2]));
-        d = fma(neglog(uni(x[0])), c * c, neglog(uni(x[1]))) * inv_alpha;
-        const double u4 = uni(x[3]);
-        return u4 * u4 <= fma(-0.5, d, 1.0);
+        d = t.s * inv_alpha;
+        return t.u4 * t.u4 <= fma(-0.5, d, 1.0);
     }
 };
 
-// delta of one trial in double from the block norm |k|^2, for the fp32 kernel: the accept test of borderline trials
-// and the value of delta where the SFU draw is not accurate enough (small alpha, large -ln u)
-static __device__ __noinline__ double kp_delta_f64(double n2, double Td, uint32_t x0, uint32_t x1, uint32_t x2)
-{
-    using M = KPMath<double>;
-    const double alpha = sqrt(n2) / Td;
-    const double c = M::cos2pi(M::uni(x2));
-    return (M::neglog(M::uni(x0)) / alpha) * (c * c) + (M::neglog(M::uni(x1)) / alpha);
-}
-
-// fp32: the draw runs on the SFU: u from the mantissa trick (exact), -ln u = -ln2 * lg2(u) (MUFU.LG2), cos/sin by
-// MUFU.COS/SIN, one reciprocal of alpha per subgroup instead of two divisions per trial.  The SFU value of
-// delta carries an absolute error of up to ~1e-6 (1 + l1 + l2)/alpha (lg2: 2 ulp, 2^-22 near 1; cos: ~4e-7), which
-// would flip ~1e-6 of the accept decisions against the fp64 oracle.  Two-tier test: a trial whose u4^2 falls inside
-// that error band of the threshold is decided again in double (kp_accept_f64, from the same |k|^2 and Philox block);
-// what is left are the flips caused by the fp32 rounding of K itself (alpha differs from the oracle's at ~1e-7).
+// fp32: the draw runs on the SFU: u from the mantissa trick (exact), -ln u = -ln2 * lg2(u) (MUFU.LG2), cos / sin by
+// MUFU.COS / SIN, one reciprocal of alpha per subgroup instead of two divisions per trial.  The SFU value of delta
+// carries an absolute error of up to ~1e-6 (1 + l1 + l2)/alpha (lg2: 2 ulp, 2^-22 near 1; cos: ~4e-7), which would flip
+// ~1e-6 of the accept decisions against the fp64 oracle.  Two-tier test: a trial whose u4^2 falls inside that error
+// band of the threshold is BORDERLINE: the thread goes on with the fp32 decision, but its site is redone in double at
+// the end (fixup_site_f64: K, the draw with 1-ulp log / cospi and the link products in double, from the stored links,
+// which nobody else touches in this half-sweep, C6).  The hot path holds no double-precision code and no call; what is
+// left are the flips caused by the fp32 rounding of K itself at the sites that are not redone (alpha differs at ~1e-7).
 template <> struct KPMath<float> {
     // (2 (x >> 9) + 1) 2^-24 = [1 + (x >> 9) 2^-23] - (1 - 2^-24): both terms and the result are fp32 numbers
     static __device__ __forceinline__ float uni(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994039535522461f; }
-    static __device__ __forceinline__ float cos2pi(float u) { return __cosf(6.283185307179586f * u); }
-    static __device__ __forceinline__ float sin2pi(float u) { return __sinf(6.283185307179586f * u); }
     static __device__ __forceinline__ float neglog(float u) { return -0.693147180559945f * __log2f(u); }
     static __device__ __forceinline__ float root(float x) { return x > 0.0f ? x * rsqrtf(x) : 0.0f; }
-    // est: inv_alpha (1 + l1 + l2), the scale of the absolute error of the SFU value of delta (in units of ~5e-7)
-    static __device__ __forceinline__ bool trial(const uint32_t (&x)[4], double n2, double Td, float inv_alpha, float& d,
-                                                 float& est)
+    // cos^2(2 pi u3) = (1 + cos(4 pi u3)) / 2, the argument folded exactly into [-pi, pi] (MUFU.COS is specified
+    // there): the absolute error of c^2 is half that of the SFU cosine instead of 2 |c| times it
+    static __device__ __forceinline__ float trial_angle(float u3) { const float v = 2.0f * u3; return v - rintf(v); }
+    static __device__ __forceinline__ float cos_squared(float c) { return fmaf(0.5f, c, 0.5f); }
+    static __device__ __forceinline__ void sincos2pi(float a, float& sn, float& cs)
     {
-        // cos^2(2 pi u3) = (1 + cos(4 pi u3)) / 2, the argument folded exactly into [-pi, pi] (MUFU.COS is specified
-        // there): the absolute error of c^2 is half that of the SFU cosine instead of 2 |c| times it
-        const float v = 2.0f * uni(x[2]);
-        const float c2 = fmaf(0.5f, __cosf(6.283185307179586f * (v - rintf(v))), 0.5f);
-        const float l1 = neglog(uni(x[0])), l2 = neglog(uni(x[1]));
-        d = fmaf(l1, c2, l2) * inv_alpha;
-        const float u4 = uni(x[3]);
-        const float diff = fmaf(u4, u4, fmaf(0.5f, d, -1.0f)); // u4^2 - (1 - delta/2)
-        est = inv_alpha * (1.0f + l1 + l2);
-        if (fabsf(diff) < fmaf(2e-6f, est, 3e-7f)) {
-            const double u4d = KPMath<double>::uni(x[3]);
-            return u4d * u4d <= 1.0 - 0.5 * kp_delta_f64(n2, Td, x[0], x[1], x[2]);
-        }
+        const float x = 6.283185307179586f * a;
+        sn = __sinf(x);
+        cs = __cosf(x);
+    }
+    // est: inv_alpha (1 + l1 + l2), the scale of the absolute error of the SFU value of delta (in units of ~5e-7)
+    static __device__ __forceinline__ bool decide(const TrialPre<float>& t, float inv_alpha, float& d, float& est, bool& border)
+    {
+        d = t.s * inv_alpha;
+        const float diff = fmaf(t.u4, t.u4, fmaf(0.5f, d, -1.0f)); // u4^2 - (1 - delta/2)
+        est = inv_alpha * t.lsum;
+        border = border || fabsf(diff) < fmaf(2e-6f, est, 3e-7f);
         return diff <= 0.0f;
     }
 };
 
-// The Philox counters of a draw hold (site, step, parity, subgroup, trial) and no data, so the block of trial 0
-// and the direction block of each subgroup are generated up front, as six independent chains, while the thread's
-// link loads are in flight (EarlyRandom); only rejected trials call the generator inside the data-dependent loop.
-struct EarlyRandom {
-    uint32_t trial0[4]; // Philox block of trial 0: u1, u2, u3, u4
-    uint32_t dir[2];    // first two words of the direction block (counter word 3 = 0x80000000)
+// the K-independent part of one trial from its Philox block (u1, u2, u3, u4)
+template <typename DT>
+__device__ __forceinline__ TrialPre<DT> kp_trial_pre(const uint32_t (&x)[4])
+{
+    using M = KPMath<DT>;
+    DT sn, cs;
+    M::sincos2pi(M::trial_angle(M::uni(x[2])), sn, cs);
+    (void)sn;
+    const DT l1 = M::neglog(M::uni(x[0])), l2 = M::neglog(M::uni(x[1]));
+    TrialPre<DT> t;
+    t.s = gf_fma(l1, M::cos_squared(cs), l2);
+    t.lsum = DT(1) + l1 + l2;
+    t.u4 = M::uni(x[3]);
+    return t;
+}
+
+// The Philox counters of a draw hold (site, step, parity, subgroup, trial) and no data, so trial 0 and the direction
+// of each subgroup are prepared up front, as independent chains, while the thread's link loads are in flight; only
+// rejected trials call the generator inside the data-dependent loop.
+template <typename DT>
+__device__ __forceinline__ void early_draw(uint32_t key0, uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2, EarlyDraw<DT>& e)
+{
+    using M = KPMath<DT>;
+    uint32_t x[4];
+    philox4x32_10(c0, c1, c2, 0u, key0, key1, x);
+    e.t0 = kp_trial_pre<DT>(x);
+    philox4x32_10(c0, c1, c2, 0x80000000u, key0, key1, x);
+    const DT cos_t = DT(1) - DT(2) * M::uni(x[0]);
+    const DT sin_t = M::root(DT(1) - cos_t * cos_t);
+    DT sn, cs;
+    M::sincos2pi(M::uni(x[1]), sn, cs);
+    e.e1 = sin_t * cs;
+    e.e2 = sin_t * sn;
+    e.e3 = cos_t;
+}
+
+// The same for kernels in which two (or four) threads share a site: the two lanes of a pair (lane, lane ^ 1) run ONE
+// instruction stream on different data and exchange the results -- role 0 generates the Philox block of trial 0, takes
+// -ln u1 and the cosine of the trial; role 1 generates the direction block, takes -ln u2 and sine / cosine of the
+// direction: one generator call, one logarithm and one sincos per thread instead of two, two and two.
+template <typename DT> struct Shfl;
+template <> struct Shfl<float> {
+    static __device__ __forceinline__ float get(unsigned mask, float v, int src) { return __shfl_sync(mask, v, src); }
+};
+template <> struct Shfl<double> {
+    static __device__ __forceinline__ double get(unsigned mask, double v, int src) { return __shfl_sync(mask, v, src); }
 };
 
-__device__ __forceinline__ void early_random(uint32_t key0, uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2,
-                                             EarlyRandom& e)
+template <typename DT>
+__device__ __forceinline__ void early_draw_pair(uint32_t key0, uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2, unsigned mask,
+                                                EarlyDraw<DT>& e)
 {
-    uint32_t x[4];
-    philox4x32_10(c0, c1, c2, 0u, key0, key1, e.trial0);
-    philox4x32_10(c0, c1, c2, 0x80000000u, key0, key1, x);
-    e.dir[0] = x[0];
-    e.dir[1] = x[1];
+    using M = KPMath<DT>;
+    const int lane = (int)(threadIdx.x & 31u), src0 = lane & ~1, src1 = lane | 1;
+    const bool role = (lane & 1) != 0;
+    uint32_t y[4];
+    philox4x32_10(c0, c1, c2, role ? 0x80000000u : 0u, key0, key1, y);
+    const uint32_t x1 = __shfl_sync(mask, y[1], src0); // u2 and u4 of the trial, generated by role 0
+    const uint32_t x3 = __shfl_sync(mask, y[3], src0);
+    const DT l = M::neglog(M::uni(role ? x1 : y[0]));
+    DT sn, cs;
+    M::sincos2pi(role ? M::uni(y[1]) : M::trial_angle(M::uni(y[2])), sn, cs);
+    const DT cos_t = DT(1) - DT(2) * M::uni(y[0]); // meaningful on role 1
+    const DT sin_t = M::root(DT(1) - cos_t * cos_t);
+    const DT l1 = Shfl<DT>::get(mask, l, src0), l2 = Shfl<DT>::get(mask, l, src1);
+    e.t0.s = gf_fma(l1, M::cos_squared(Shfl<DT>::get(mask, cs, src0)), l2);
+    e.t0.lsum = DT(1) + l1 + l2;
+    e.t0.u4 = M::uni(x3);
+    e.e1 = Shfl<DT>::get(mask, sin_t * cs, src1);
+    e.e2 = Shfl<DT>::get(mask, sin_t * sn, src1);
+    e.e3 = Shfl<DT>::get(mask, cos_t, src1);
 }
 
 // returns the number of trials used (0: degenerate block, identity taken; 4097: cap hit); cond = |k|^2 (the
 // conditioning number of g = h (x) conj(khat), see su2_overrelax_step).
 // CT: type of the site chain (k, khat = k/|k|, g -- the ill-conditioned part); DT: type of the draw (alpha, the
 // Kennedy-Pendleton trials, h).  (double, float): fp32 kernels with the chain in double, the draw on the SFU.
-template <typename CT, typename DT>
+// redo (fp32 draw): set where the SFU draw is not good enough for this site -- a borderline accept test (KPMath<float>)
+// or an accepted delta whose SFU error would move the links by more than ~1e-5 -- and the site is to be redone in double.
+// PAIR: the lanes (lane, lane ^ 1) hold the same site (identical K, bit for bit, so identical decisions): the retry
+// loop evaluates two trials per pass, trial t on the even lane and t + 1 on the odd one, and takes the first accepted.
+template <typename CT, typename DT, bool PAIR>
 __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double Td, uint32_t key0,
                                                       uint32_t key1, uint32_t c0, uint32_t c1, uint32_t c2,
-                                                      const EarlyRandom& early, CT (&g)[4], CT& cond)
+                                                      const EarlyDraw<DT>& early, CT (&g)[4], CT& cond, bool& redo)
 {
     using M = KPMath<DT>;
     const CT n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
@@ -289,21 +352,43 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double T
     const CT inv_n = gf_rsqrt<CT>(n2);
     const DT inv_alpha = (DT)((CT)Td * inv_n);
     const CT kc0 = k[0] * inv_n, kc1 = -k[1] * inv_n, kc2 = -k[2] * inv_n, kc3 = -k[3] * inv_n; // conj(khat)
-    // unit vector of the direction of hvec: data independent, computed ahead of the draw
-    const DT cos_t = DT(1) - DT(2) * M::uni(early.dir[0]);
-    const DT up = M::uni(early.dir[1]);
-    const DT sin_t = M::root(DT(1) - cos_t * cos_t);
-    const DT e1 = sin_t * M::cos2pi(up), e2 = sin_t * M::sin2pi(up), e3 = cos_t;
-    // trial 0 from the words generated up front: straight-line code, so that it can be scheduled together with the
+    // trial 0 from the values prepared up front: straight-line code, so that it can be scheduled together with the
     // link updates of the previous subgroup; only rejected lanes enter the loop
     DT d, est;
     unsigned trial = 0;
-    uint32_t x[4] = {early.trial0[0], early.trial0[1], early.trial0[2], early.trial0[3]};
-    bool accepted = M::trial(x, (double)n2, Td, inv_alpha, d, est);
+    bool accepted = M::decide(early.t0, inv_alpha, d, est, redo);
+#ifdef GF_EXP_NOLOOP
+    accepted = true;
+#endif
     if (!accepted) {
-        for (trial = 1; trial < 4096u; ++trial) {
-            philox4x32_10(c0, c1, c2, trial, key0, key1, x);
-            if (M::trial(x, (double)n2, Td, inv_alpha, d, est)) { accepted = true; break; }
+        if (PAIR) {
+            const int lane = (int)(threadIdx.x & 31u), src0 = lane & ~1, src1 = lane | 1;
+            const unsigned pair = 3u << src0;
+            const unsigned role = (unsigned)(lane & 1);
+            for (unsigned t = 1; t < 4096u; t += 2) {
+                uint32_t x[4];
+                philox4x32_10(c0, c1, c2, t + role, key0, key1, x);
+                DT dm, em;
+                bool bm = false;
+                const bool am = M::decide(kp_trial_pre<DT>(x), inv_alpha, dm, em, bm) && (t + role < 4096u);
+                const unsigned acc = __ballot_sync(pair, am) >> src0;      // bit 0: trial t, bit 1: trial t + 1
+                const unsigned bor = __ballot_sync(pair, bm) >> src0;
+                if (bor & (1u | ((acc & 1u) ? 0u : 2u))) redo = true;      // trial t + 1 counts only if trial t was rejected
+                if (acc & 3u) {
+                    const int from = (acc & 1u) ? src0 : src1;
+                    d = Shfl<DT>::get(pair, dm, from);
+                    est = Shfl<DT>::get(pair, em, from);
+                    trial = t + ((acc & 1u) ? 0u : 1u);
+                    accepted = true;
+                    break;
+                }
+            }
+        } else {
+            uint32_t x[4];
+            for (trial = 1; trial < 4096u; ++trial) {
+                philox4x32_10(c0, c1, c2, trial, key0, key1, x);
+                if (M::decide(kp_trial_pre<DT>(x), inv_alpha, d, est, redo)) { accepted = true; break; }
+            }
         }
     }
     if (!accepted) {
@@ -312,13 +397,13 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double T
         return 4097u;
     }
     // fp32 draw: the SFU value of the accepted delta is off by ~5e-7 est, which moves h0 by as much and hvec, of
-    // length r = sqrt(delta (2 - delta)), by that over r.  Where this is too much for the links (small alpha, large
-    // -ln u, h0 near -1: ~1e-3 of the draws at T = 1.4, none once alpha > 10) delta is taken in double
-    if (sizeof(DT) == 4 && est * est > DT(16) * fmin(d * (DT(2) - d), DT(1)))
-        d = (DT)kp_delta_f64((double)n2, Td, x[0], x[1], x[2]);
+    // length r = sqrt(delta (2 - delta)), by that over r.  Where this is too much for the links (est > 16 r: more than
+    // ~8e-6; small alpha, large -ln u, h0 near +-1: ~1e-4 of the draws at T = 1.4, none once alpha > 10) the site is
+    // redone in double
+    if (sizeof(DT) == 4) redo = redo || est * est > DT(256) * fmin(d * (DT(2) - d), DT(1));
     const DT h0d = DT(1) - d;
     const DT r = M::root(d * (DT(2) - d)); // = sqrt(1 - h0^2) without the cancellation at small delta
-    const CT h0 = (CT)h0d, h1 = (CT)(r * e1), h2 = (CT)(r * e2), h3 = (CT)(r * e3);
+    const CT h0 = (CT)h0d, h1 = (CT)(r * early.e1), h2 = (CT)(r * early.e2), h3 = (CT)(r * early.e3);
     // g = h (x) conj(khat):  (pq)_0 = p0 q0 - p.q,  (pq)_vec = p0 qvec + q0 pvec - pvec x qvec   (C13)
     g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3;
     g[1] = h0 * kc1 + kc0 * h1 - (h2 * kc3 - h3 * kc2);
@@ -350,9 +435,10 @@ __device__ __forceinline__ void fixup_subgroup(const SweepParams& p, const Sweep
     } else if (MODE == MODE_VARIANT) {
         su2_variant_step<double>(k, p.variant, p.omega, p.key0, p.key1, site_canon, ph.step, c2, h, cond);
     } else {
-        EarlyRandom early;
-        early_random(p.key0, p.key1, site_canon, ph.step, c2, early);
-        const unsigned ntr = su2_heatbath_step<double, double>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond);
+        EarlyDraw<double> early;
+        early_draw<double>(p.key0, p.key1, site_canon, ph.step, c2, early);
+        bool redo = false; // the double draw has no second tier
+        const unsigned ntr = su2_heatbath_step<double, double, false>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond, redo);
         if (record && p.trials != nullptr) p.trials[3u * (size_t)(site_canon - p.site_offset) + SUB] = ntr;
     }
     a = {h[0], h[3]};
@@ -422,6 +508,15 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
     if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
 }
 
+__device__ __forceinline__ void pin_early(const EarlyDraw<float>& e)
+{
+    asm volatile("" :: "f"(e.t0.s), "f"(e.t0.lsum), "f"(e.t0.u4), "f"(e.e1), "f"(e.e2), "f"(e.e3));
+}
+__device__ __forceinline__ void pin_early(const EarlyDraw<double>& e)
+{
+    asm volatile("" :: "d"(e.t0.s), "d"(e.t0.u4), "d"(e.e1), "d"(e.e2), "d"(e.e3));
+}
+
 __device__ __forceinline__ int tie_bits(float x) { return __float_as_int(x); }
 __device__ __forceinline__ int tie_bits(double x) { return __double2hiint(x); }
 
@@ -455,7 +550,12 @@ struct SweepKernel {
     static constexpr int NMU = 4 / TPS;
     static constexpr bool FP32 = sizeof(T) == 4;
     static constexpr bool HYB = FP32 && MODE != MODE_HEATBATH;        // relaxation sweeps: chain type chosen per launch
-    static constexpr bool FIX = FP32 && MODE == MODE_HEATBATH && !DC; // heatbath: fp32 chain, weak sites redone in double
+#ifdef GF_EXP_NOFIX
+    static constexpr bool FIX = false;
+#else
+    static constexpr bool FIX = FP32 && MODE == MODE_HEATBATH;        // heatbath: weak sites and weak draws redone in double
+#endif
+    static constexpr bool PAIR = MODE == MODE_HEATBATH && TPS >= 2;   // heatbath: two lanes of a site share the work of the draw
     static_assert(!DC || (FP32 && MODE == MODE_HEATBATH), "DC is a variant of the fp32 heatbath kernel");
     static_assert(MON == 0 || MODE != MODE_HEATBATH, "the monitor belongs to the relaxation sweeps");
     using IO = LinkIO<T, R>;
@@ -465,7 +565,7 @@ struct SweepKernel {
     template <typename CT, int I, int J, int SUB>
     static __device__ __forceinline__ void subgroup(const SweepParams& p, const SweepPhase& ph, cx<CT> (&K)[9],
                                                     cx<T> (&F)[NMU][9], cx<T> (&B)[NMU][9], uint32_t site_canon,
-                                                    bool record, const EarlyRandom& early, int lane_mu0,
+                                                    bool record, const EarlyDraw<T>& early, int lane_mu0,
                                                     cx<T> (&Gt)[9], bool& watch)
     {
         CT k[4], h[4], cond;
@@ -477,10 +577,12 @@ struct SweepKernel {
             su2_variant_step<CT>(k, p.variant, p.omega, p.key0, p.key1, site_canon, ph.step, c2, h, cond);
             (void)early;
         } else {
-            unsigned ntr = su2_heatbath_step<CT, T>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond);
+            bool redo = false;
+            unsigned ntr = su2_heatbath_step<CT, T, PAIR>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond, redo);
             if (record && p.trials != nullptr) p.trials[3u * (size_t)(site_canon - p.site_offset) + SUB] = ntr;
+            if (FP32) watch = watch || (redo && p.watch_thr2 >= 0.0f); // a negative threshold: no repairs at all (CHAIN_FP32)
         }
-        if (FP32) watch = watch || ((float)cond < p.watch_thr2);
+        if (FP32 && !DC) watch = watch || ((float)cond < p.watch_thr2);
         const cx<CT> ac = {h[0], h[3]}, bc = {h[2], h[1]}; // C4
         const cx<T> a = {(T)h[0], (T)h[3]}, b = {(T)h[2], (T)h[1]};
 #pragma unroll
@@ -501,7 +603,7 @@ struct SweepKernel {
     template <typename CT>
     static __device__ __forceinline__ bool chain(const SweepParams& p, const SweepPhase& ph, cx<T> (&F)[NMU][9],
                                                  cx<T> (&B)[NMU][9], cx<T> (&Gt)[9], uint32_t sc,
-                                                 const EarlyRandom (&early)[3], int lane_mu0, unsigned mask, bool& watch,
+                                                 const EarlyDraw<T> (&early)[3], int lane_mu0, unsigned mask, bool& watch,
                                                  double& th_pre, double& th_post, int mon_skip)
     {
         // K(x) = sum_{mu < nd} [ U_mu(x) + U_mu(x-mu)^dagger ]   (eq. 2.3; C2)
@@ -728,17 +830,18 @@ struct SweepKernel {
         if (MODE == MODE_HEATBATH) issue_prefetch(p, ph, s, hb, lane_mu0, base, H);
         // heatbath: random numbers of trial 0 and of the direction, generated under the shadow of the loads
         const uint32_t sc = canonical_index(s) + p.site_offset;
-        EarlyRandom early[3];
+        EarlyDraw<T> early[3];
         if (MODE == MODE_HEATBATH) {
 #pragma unroll
-            for (int sub = 0; sub < 3; ++sub)
-                early_random(p.key0, p.key1, sc, ph.step, ((uint32_t)ph.parity << 2) | (uint32_t)sub, early[sub]);
-            // pin the 18 words here, before the first use of a loaded link: volatile asm statements keep their
-            // order, so the generator runs between the issue of the loads and their consumption
+            for (int sub = 0; sub < 3; ++sub) {
+                const uint32_t c2 = ((uint32_t)ph.parity << 2) | (uint32_t)sub;
+                if (PAIR) early_draw_pair<T>(p.key0, p.key1, sc, ph.step, c2, mask, early[sub]);
+                else early_draw<T>(p.key0, p.key1, sc, ph.step, c2, early[sub]);
+            }
+            // pin the values here, before the first use of a loaded link: volatile asm statements keep their order, so
+            // the generator and the logarithms run between the issue of the loads and their consumption
 #pragma unroll
-            for (int sub = 0; sub < 3; ++sub)
-                asm volatile("" :: "r"(early[sub].trial0[0]), "r"(early[sub].trial0[1]), "r"(early[sub].trial0[2]),
-                             "r"(early[sub].trial0[3]), "r"(early[sub].dir[0]), "r"(early[sub].dir[1]));
+            for (int sub = 0; sub < 3; ++sub) pin_early(early[sub]);
         }
         if (ph.reunit) {
 #pragma unroll
@@ -776,8 +879,12 @@ struct SweepKernel {
             if (MON && !updated) return;
             if constexpr (FIX) {
                 if (watch) {
+#ifdef GF_EXP_FIXFLAG
+                    if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
+#else
                     fixup_site_f64<R, TPS, MODE, CB>(p, ph, slot, lane_mu0); // stores the links itself
                     return;
+#endif
                 }
             }
         }
@@ -853,6 +960,9 @@ struct SweepKernel {
 template <typename T, int R, int TPS, int MODE, bool CB>
 constexpr int sweep_max_registers()
 {
+#ifdef GF_EXP_HB_MAXREG
+    if (sizeof(T) == 4 && MODE == MODE_HEATBATH && TPS == 1) return GF_EXP_HB_MAXREG;
+#endif
     if (sizeof(T) == 4 && MODE != MODE_HEATBATH) { // what ptxas gives the same kernel with the fp32 chain alone, rounded up to 8
         const bool var = MODE == MODE_VARIANT;
         if (R == 12) {
