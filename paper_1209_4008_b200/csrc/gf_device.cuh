@@ -395,10 +395,7 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
                                               uint32_t k1, uint32_t (&out)[4])
 {
 #pragma unroll
-#ifndef GF_EXP_PHILOX_ROUNDS
-#define GF_EXP_PHILOX_ROUNDS 10
-#endif
-    for (int round = 0; round < GF_EXP_PHILOX_ROUNDS; ++round) {
+    for (int round = 0; round < 10; ++round) {
         const uint64_t p0 = (uint64_t)0xD2511F53u * c0; // one IMAD.WIDE.U32 gives hi and lo
         const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
         c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;

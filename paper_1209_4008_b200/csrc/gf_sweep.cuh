@@ -247,6 +247,13 @@ template <> struct KPMath<float> {
         sn = __sinf(x);
         cs = __cosf(x);
     }
+    // delta of a trial from its uniforms with the 1-ulp library functions instead of the SFU
+    static __device__ __forceinline__ float accurate_delta(const uint32_t (&x)[4], float inv_alpha)
+    {
+        const float l1 = -logf(uni(x[0])), l2 = -logf(uni(x[1]));
+        const float c = cospif(2.0f * uni(x[2]));
+        return fmaf(l1, c * c, l2) * inv_alpha;
+    }
     // est: inv_alpha (1 + l1 + l2), the scale of the absolute error of the SFU value of delta (in units of ~5e-7)
     static __device__ __forceinline__ bool decide(const TrialPre<float>& t, float inv_alpha, float& d, float& est, bool& border)
     {
@@ -357,9 +364,6 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double T
     DT d, est;
     unsigned trial = 0;
     bool accepted = M::decide(early.t0, inv_alpha, d, est, redo);
-#ifdef GF_EXP_NOLOOP
-    accepted = true;
-#endif
     if (!accepted) {
         if (PAIR) {
             const int lane = (int)(threadIdx.x & 31u), src0 = lane & ~1, src1 = lane | 1;
@@ -398,9 +402,17 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double T
     }
     // fp32 draw: the SFU value of the accepted delta is off by ~5e-7 est, which moves h0 by as much and hvec, of
     // length r = sqrt(delta (2 - delta)), by that over r.  Where this is too much for the links (est > 16 r: more than
-    // ~8e-6; small alpha, large -ln u, h0 near +-1: ~1e-4 of the draws at T = 1.4, none once alpha > 10) the site is
-    // redone in double
-    if (sizeof(DT) == 4) redo = redo || est * est > DT(256) * fmin(d * (DT(2) - d), DT(1));
+    // ~8e-6; small alpha, large -ln u, h0 near +-1: 6e-4 of the draws at T = 1.4, none once alpha > 10) delta is taken
+    // again from the uniforms of the accepted trial with the 1-ulp functions (logf, cospif: ~1.5e-7 est), a few dozen
+    // instructions inline; only where even that is too coarse (est > 64 r, 1e-5 of the draws) the site is redone in double
+    if constexpr (sizeof(DT) == 4) {
+        if (est * est > DT(256) * fmin(d * (DT(2) - d), DT(1))) {
+            uint32_t x[4];
+            philox4x32_10(c0, c1, c2, trial, key0, key1, x);
+            d = M::accurate_delta(x, inv_alpha);
+            redo = redo || est * est > DT(4096) * fmin(d * (DT(2) - d), DT(1));
+        }
+    }
     const DT h0d = DT(1) - d;
     const DT r = M::root(d * (DT(2) - d)); // = sqrt(1 - h0^2) without the cancellation at small delta
     const CT h0 = (CT)h0d, h1 = (CT)(r * early.e1), h2 = (CT)(r * early.e2), h3 = (CT)(r * early.e3);
@@ -417,36 +429,100 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double T
 // g = h (x) conj(khat) with khat = k/|k| is ill-conditioned where the projected block is small: the fp32 rounding of K
 // (~1e-6) then moves the links by ~1e-6/|k|.  (For the heatbath there is no second small factor, and a BLACK site
 // inherits only ~1e-6 from its RED neighbours, so unlike the relaxation sweeps a per-site repair is enough here.)  A
-// thread whose |k|^2 fell below SweepParams::fix_thr2 in any of its three subgroup steps drops its fp32 result and
-// redoes the site here from the stored fp32 links (untouched so far: within a half-sweep only this site writes them,
-// C6): K, the three SU(2) steps, K <- G K and the link products all in double, one rounding to fp32 at the store.
+// thread whose |k|^2 fell below SweepParams::watch_thr2 in one of its three subgroup steps, or whose SFU draw was not
+// good enough (KPMath<float>), drops its fp32 result and redoes the site here from the stored fp32 links (untouched so
+// far: within a half-sweep only this site writes them, C6): K, the three SU(2) steps with the draw in double (same
+// arithmetic as the fp64 kernel's), K <- G K and the link products all in double, one rounding to fp32 at the store.
 // Every thread of a site takes the same decision (K is bit-identical on them) and redoes its own links; no shuffles
 // on this divergent path: each thread builds K for itself.  DESIGN.md sec. 4.
+//
+// This code runs at ~1e-5 of the sites, i.e. a few dozen times per launch of a 7 M-site lattice, and each time it is COLD:
+// its instructions come from L2 or DRAM, ~1 us per 128-byte line (8 instructions), and the block that runs it holds up
+// the end of its launch.  So it is written for size, not speed: rolled loops, run-time subgroup indices on arrays in
+// local memory, one copy of the trial code (trial 0 is the first pass of the loop), the three SU(2) factors accumulated
+// into one 3x3 matrix G = G3 G2 G1 that is applied to the links in a rolled loop (C8: equal to applying them one after
+// the other up to rounding, here in double).  Unrolled like the hot path it was 4600 instructions (74 KB) and cost
+// 48^3x64 fp32 annealing 13 % through launch tails; profiles/r2_heatbath.md.
 // ---------------------------------------------------------------------------------------------------------
-template <int I, int J, int SUB, int MODE>
-__device__ __forceinline__ void fixup_subgroup(const SweepParams& p, const SweepPhase& ph, cx<double> (&K)[9],
-                                               uint32_t site_canon, bool record, cx<double>& a, cx<double>& b)
+// one SU(2) heatbath step in double on the projected block k: the arithmetic of su2_heatbath_step<double, double, false>
+// with trial 0 taken inside the loop (one copy of the generator and of the logarithms)
+static __device__ __noinline__ unsigned fix_heatbath_step(const double (&k)[4], double Td, uint32_t key0, uint32_t key1, uint32_t c0,
+                                                   uint32_t c1, uint32_t c2, double (&g)[4])
 {
-    double k[4], h[4], cond;
-    su2_project<I, J>(K, k);
-    const uint32_t c2 = ((uint32_t)ph.parity << 2) | (uint32_t)SUB;
-    if (MODE == MODE_OVERRELAX) {
-        su2_overrelax_step<double>(k, p.omega, h, cond);
-    } else if (MODE == MODE_VARIANT) {
-        su2_variant_step<double>(k, p.variant, p.omega, p.key0, p.key1, site_canon, ph.step, c2, h, cond);
-    } else {
-        EarlyDraw<double> early;
-        early_draw<double>(p.key0, p.key1, site_canon, ph.step, c2, early);
-        bool redo = false; // the double draw has no second tier
-        const unsigned ntr = su2_heatbath_step<double, double, false>(k, ph.T, p.key0, p.key1, site_canon, ph.step, c2, early, h, cond, redo);
-        if (record && p.trials != nullptr) p.trials[3u * (size_t)(site_canon - p.site_offset) + SUB] = ntr;
+    using M = KPMath<double>;
+    const double n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2] + k[3] * k[3];
+    if (!(n2 >= Tiny<double>::sq)) { g[0] = 1.0; g[1] = g[2] = g[3] = 0.0; return 0u; }
+    const double inv_n = gf_rsqrt<double>(n2);
+    const double inv_alpha = Td * inv_n;
+    const double kc0 = k[0] * inv_n, kc1 = -k[1] * inv_n, kc2 = -k[2] * inv_n, kc3 = -k[3] * inv_n; // conj(khat)
+    uint32_t x[4];
+    double d = 0.0, est;
+    bool accepted = false, border = false;
+    unsigned trial = 0;
+#pragma unroll 1
+    for (; trial < 4096u; ++trial) {
+        philox4x32_10(c0, c1, c2, trial, key0, key1, x);
+        if (M::decide(kp_trial_pre<double>(x), inv_alpha, d, est, border)) { accepted = true; break; }
     }
-    a = {h[0], h[3]};
-    b = {h[2], h[1]}; // C4
-    su2_left<I, J>(a, b, K); // K <- G K  (C8)
+    if (!accepted) { g[0] = kc0; g[1] = kc1; g[2] = kc2; g[3] = kc3; return 4097u; } // h = identity
+    philox4x32_10(c0, c1, c2, 0x80000000u, key0, key1, x);
+    const double cos_t = 1.0 - 2.0 * M::uni(x[0]);
+    const double sin_t = M::root(1.0 - cos_t * cos_t);
+    double sn, cs;
+    M::sincos2pi(M::uni(x[1]), sn, cs);
+    const double r = M::root(d * (2.0 - d));
+    const double h0 = 1.0 - d, h1 = r * (sin_t * cs), h2 = r * (sin_t * sn), h3 = r * cos_t;
+    g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3; // g = h (x) conj(khat)  (C13)
+    g[1] = h0 * kc1 + kc0 * h1 - (h2 * kc3 - h3 * kc2);
+    g[2] = h0 * kc2 + kc0 * h2 - (h3 * kc1 - h1 * kc3);
+    g[3] = h0 * kc3 + kc0 * h3 - (h1 * kc2 - h2 * kc1);
+    return trial + 1u;
 }
 
-template <int R, int TPS, int MODE, bool CB>
+static __device__ __noinline__ void fix_reunit(cx<double> (&u)[9]) { reunitarise(u); }
+
+// stored fp32 entries -> double, third row rebuilt (R = 12), rows re-orthonormalised on a reunitarisation sweep
+template <int R>
+__device__ __forceinline__ void fix_widen(const cx<float> (&v)[9], int reunit, cx<double> (&u)[9])
+{
+#pragma unroll
+    for (int e = 0; e < R / 2; ++e) u[e] = {(double)v[e].re, (double)v[e].im};
+    if (R == 12) rebuild_row2(u);
+    if (reunit) fix_reunit(u);
+}
+
+// w = G u (dagger = false) or w = u G^dagger (dagger = true)
+template <bool DAGGER>
+__device__ __forceinline__ void fix_mul(const cx<double> (&G)[9], const cx<double> (&u)[9], cx<double> (&w)[9])
+{
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            cx<double> acc = {0.0, 0.0};
+#pragma unroll
+            for (int k = 0; k < 3; ++k) acc = acc + (DAGGER ? cmul_cb(u[3 * r + k], G[3 * c + k]) : G[3 * r + k] * u[3 * k + c]);
+            w[3 * r + c] = acc;
+        }
+}
+
+template <int I, int J, int SUB>
+__device__ __forceinline__ void fix_subgroup(const SweepParams& p, const SweepPhase& ph, uint32_t sc, bool record, cx<double> (&K)[9],
+                                             cx<double> (&G)[9])
+{
+    double k[4], g[4];
+    su2_project<I, J>(K, k);
+    const unsigned ntr = fix_heatbath_step(k, ph.T, p.key0, p.key1, sc, ph.step, ((uint32_t)ph.parity << 2) | (uint32_t)SUB, g);
+    if (record && p.trials != nullptr) p.trials[3u * (size_t)(sc - p.site_offset) + SUB] = ntr;
+    const cx<double> a = {g[0], g[3]}, b = {g[2], g[1]}; // C4
+    su2_left<I, J>(a, b, K); // K <- g K  (C8)
+    su2_left<I, J>(a, b, G); // G <- g G
+}
+
+// The links of the site are fetched ONCE, all together (the block runs in a saturated memory system: every dependent
+// round trip costs microseconds), kept as the stored floats, and widened where they are used: for K, then again for the
+// products G U, U G^dagger with the accumulated G = g3 g2 g1.
+template <int R, int TPS, bool CB>
 __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPhase& ph, unsigned h, int lane_mu0)
 {
     constexpr int NMU = 4 / TPS;
@@ -456,58 +532,55 @@ __device__ __noinline__ void fixup_site_f64(const SweepParams& p, const SweepPha
     const size_t Hp = p.L.Hp;
     float* const base = reinterpret_cast<float*>(p.U);
     const uint64_t ld = make_l2_policy(POLICY_NORMAL), st = make_l2_policy(p.st_policy);
-    cx<double> K[9];
+    cx<float> F[4][9], B[4][9], Gs[9];
+    unsigned hb[4];
 #pragma unroll
-    for (int e = 0; e < 9; ++e) K[e] = {0.0, 0.0};
-    for (int mu = 0; mu < p.nd; ++mu) { // eq. 2.3 (C2), every direction entering K
-        cx<double> f[9], b[9];
-        IO::load(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, s.h, f, ld);
-        IO::load(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, backward_neighbour(p.L, s, mu), b, ld);
-        if (ph.reunit) { reunitarise(f); reunitarise(b); }
+    for (int mu = 0; mu < 4; ++mu) {
+        hb[mu] = backward_neighbour(p.L, s, mu);
+        if (CB && mu == 3) continue;
+        IO::load_stored(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, s.h, F[mu], ld);
+        IO::load_stored(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, hb[mu], B[mu], ld);
+    }
+    const bool owns_t = CB && lane_mu0 + NMU - 1 == 3;
+    float* const gb = reinterpret_cast<float*>(p.G) + (size_t)ph.parity * 18 * Hp;
+    if (owns_t) GIO::load_stored(gb, Hp, s.h, Gs, ld);
+    cx<double> K[9], G[9], u[9], w[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { K[e] = {0.0, 0.0}; G[e] = {(e & 3) == 0 ? 1.0 : 0.0, 0.0}; }
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) { // eq. 2.3 (C2), every direction entering K
+        if (mu >= p.nd || (CB && mu == 3)) continue;
+        fix_widen<R>(F[mu], ph.reunit, u);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) K[e] = K[e] + u[e];
+        fix_widen<R>(B[mu], ph.reunit, u);
 #pragma unroll
         for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int c = 0; c < 3; ++c) K[3 * r + c] = K[3 * r + c] + f[3 * r + c] + conj(b[3 * c + r]);
+            for (int c = 0; c < 3; ++c) K[3 * r + c] = K[3 * r + c] + conj(u[3 * c + r]);
     }
     const uint32_t sc = canonical_index(s) + p.site_offset;
     const bool record = lane_mu0 == 0;
-    cx<double> a0, b0, a1, b1, a2, b2;
-    fixup_subgroup<0, 1, 0, MODE>(p, ph, K, sc, record, a0, b0);
-    fixup_subgroup<0, 2, 1, MODE>(p, ph, K, sc, record, a1, b1);
-    fixup_subgroup<1, 2, 2, MODE>(p, ph, K, sc, record, a2, b2);
-    for (int m = 0; m < NMU; ++m) {
-        const int mu = lane_mu0 + m;
-        if (CB && mu == 3) continue;
-        cx<double> u[9];
-        float* const fb = base + (size_t)(ph.parity * 4 + mu) * R * Hp;
-        IO::load(fb, Hp, s.h, u, ld);
-        if (ph.reunit) reunitarise(u);
-        su2_left<0, 1>(a0, b0, u); // U_mu(x) <- G U_mu(x)
-        su2_left<0, 2>(a1, b1, u);
-        su2_left<1, 2>(a2, b2, u);
-        IO::store(fb, Hp, s.h, u, st);
-        float* const bb = base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp;
-        const unsigned hb = backward_neighbour(p.L, s, mu);
-        IO::load(bb, Hp, hb, u, ld);
-        if (ph.reunit) reunitarise(u);
-        su2_right_dagger<0, 1, 3>(a0, b0, u); // U_mu(x-mu) <- U_mu(x-mu) G^dagger
-        su2_right_dagger<0, 2, 3>(a1, b1, u);
-        su2_right_dagger<1, 2, 3>(a2, b2, u);
-        IO::store(bb, Hp, hb, u, st);
+    fix_subgroup<0, 1, 0>(p, ph, sc, record, K, G); // Cabibbo-Marinari subgroups, order of C4
+    fix_subgroup<0, 2, 1>(p, ph, sc, record, K, G);
+    fix_subgroup<1, 2, 2>(p, ph, sc, record, K, G);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        if (mu < lane_mu0 || mu >= lane_mu0 + NMU || (CB && mu == 3)) continue;
+        fix_widen<R>(F[mu], ph.reunit, u);
+        fix_mul<false>(G, u, w); // U_mu(x) <- G U_mu(x)
+        IO::store(base + (size_t)(ph.parity * 4 + mu) * R * Hp, Hp, s.h, w, st);
+        fix_widen<R>(B[mu], ph.reunit, u);
+        fix_mul<true>(G, u, w);  // U_mu(x-mu) <- U_mu(x-mu) G^dagger
+        IO::store(base + (size_t)((1 - ph.parity) * 4 + mu) * R * Hp, Hp, hb[mu], w, st);
     }
-    if (CB && lane_mu0 + NMU - 1 == 3) { // reading B: G(x) <- g G(x)
-        cx<double> u[9];
-        float* const gb = reinterpret_cast<float*>(p.G) + (size_t)ph.parity * 18 * Hp;
-        GIO::load(gb, Hp, s.h, u, ld);
-        if (ph.reunit) reunitarise(u);
-        su2_left<0, 1>(a0, b0, u);
-        su2_left<0, 2>(a1, b1, u);
-        su2_left<1, 2>(a2, b2, u);
-        GIO::store(gb, Hp, s.h, u, st);
+    if (owns_t) { // reading B: G(x) <- g G(x)
+        fix_widen<18>(Gs, ph.reunit, u);
+        fix_mul<false>(G, u, w);
+        GIO::store(gb, Hp, s.h, w, st);
     }
     if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
 }
-
 __device__ __forceinline__ void pin_early(const EarlyDraw<float>& e)
 {
     asm volatile("" :: "f"(e.t0.s), "f"(e.t0.lsum), "f"(e.t0.u4), "f"(e.e1), "f"(e.e2), "f"(e.e3));
@@ -550,11 +623,7 @@ struct SweepKernel {
     static constexpr int NMU = 4 / TPS;
     static constexpr bool FP32 = sizeof(T) == 4;
     static constexpr bool HYB = FP32 && MODE != MODE_HEATBATH;        // relaxation sweeps: chain type chosen per launch
-#ifdef GF_EXP_NOFIX
-    static constexpr bool FIX = false;
-#else
     static constexpr bool FIX = FP32 && MODE == MODE_HEATBATH;        // heatbath: weak sites and weak draws redone in double
-#endif
     static constexpr bool PAIR = MODE == MODE_HEATBATH && TPS >= 2;   // heatbath: two lanes of a site share the work of the draw
     static_assert(!DC || (FP32 && MODE == MODE_HEATBATH), "DC is a variant of the fp32 heatbath kernel");
     static_assert(MON == 0 || MODE != MODE_HEATBATH, "the monitor belongs to the relaxation sweeps");
@@ -879,12 +948,8 @@ struct SweepKernel {
             if (MON && !updated) return;
             if constexpr (FIX) {
                 if (watch) {
-#ifdef GF_EXP_FIXFLAG
-                    if (p.dc_count != nullptr && lane_mu0 == 0) atomicAdd(p.dc_count + 1, 1ull);
-#else
-                    fixup_site_f64<R, TPS, MODE, CB>(p, ph, slot, lane_mu0); // stores the links itself
+                    fixup_site_f64<R, TPS, CB>(p, ph, slot, lane_mu0); // stores the links itself
                     return;
-#endif
                 }
             }
         }
@@ -960,9 +1025,6 @@ struct SweepKernel {
 template <typename T, int R, int TPS, int MODE, bool CB>
 constexpr int sweep_max_registers()
 {
-#ifdef GF_EXP_HB_MAXREG
-    if (sizeof(T) == 4 && MODE == MODE_HEATBATH && TPS == 1) return GF_EXP_HB_MAXREG;
-#endif
     if (sizeof(T) == 4 && MODE != MODE_HEATBATH) { // what ptxas gives the same kernel with the fp32 chain alone, rounded up to 8
         const bool var = MODE == MODE_VARIANT;
         if (R == 12) {
