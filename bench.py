@@ -490,7 +490,7 @@ def main():
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--e2e-configs", type=int, default=6, help="configurations per step of the end-to-end (host buffer) leg")
+    ap.add_argument("--e2e-configs", type=int, default=12, help="configurations per step of the end-to-end (host buffer) leg")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "t"],
                     help="N > 1: independent replicas (default) or one configuration in t-slabs over the ranks")
     ap.add_argument("--traffic-csv", default=os.path.join(ROOT, "profiles", "r2_traffic.csv"),

@@ -278,12 +278,15 @@ int gf_monitor_last(gf_ctx* ctx, int* check_sweep, double* theta_host, double* F
  *     fp64 evaluation; on a nearly fixed field only the first sweep of a call takes the double chain.
  *   chain = 1: always double (about -7 % at 18 reals, -30 % at 12 reals).  chain = 0: always fp32 (a few 1e-5 of the
  *     sites of a random-gauge start miss 5e-5).
- * Annealing sweeps (gf_anneal*): chain = 2 (default): fp32 chain; a site whose projected block has |k| below
- *   fix_threshold (default 0.15) in one of its three steps is redone in double from the stored fp32 links inside the
- *   same kernel (accept decisions: 1e-7 of the draws differ from an fp64 evaluation; links: all within 5e-5 below
- *   T ~ 0.5, about 1e-6 of the sites of a 7 M-site lattice miss it at T = 1.4, where alpha = |k|/T inherits the fp32
- *   rounding of K).  chain = 1: the double chain at every site (every link within 5e-5; about -17 %).  chain = 0: plain
- *   fp32.
+ * Annealing sweeps (gf_anneal*): chain = 2 (default): fp32 chain, draw on the special-function unit, in three tiers:
+ *   (i) the accepted delta is taken again with 1-ulp fp32 functions where its SFU error would move the links by more
+ *   than ~8e-6; (ii) a site is redone in double from the stored fp32 links inside the same kernel (K, the draw, the link
+ *   products; one rounding at the store) where the projected block has |k| below fix_threshold (default 0.15) in one of
+ *   its three steps, where an accept test fell inside the SFU error band of its threshold, or where (i) is still too
+ *   coarse -- 8e-5 of the sites at T = 1.4, none below T ~ 0.1.  Accept decisions: 1e-7 of the draws differ from an fp64
+ *   evaluation; links: all within 5e-5 below T ~ 0.5, about 1e-6 of the sites of a 7 M-site lattice miss it at T = 1.4,
+ *   where alpha = |k|/T inherits the fp32 rounding of K.  chain = 1: the double chain at every site (every link within
+ *   5e-5; about -17 %).  chain = 0: plain fp32, no tiers.
  * A threshold of 0 keeps the current value.  Ignored by fp64 contexts.  GF_EINVAL: chain outside 0..2, a threshold < 0
  * or > 1e3.
  * gf_chain_count (each output may be NULL; synchronises the stream): half-sweep launches that ran the double chain and

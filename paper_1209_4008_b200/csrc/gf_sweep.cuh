@@ -624,6 +624,16 @@ struct SweepKernel {
     static constexpr bool FP32 = sizeof(T) == 4;
     static constexpr bool HYB = FP32 && MODE != MODE_HEATBATH;        // relaxation sweeps: chain type chosen per launch
     static constexpr bool FIX = FP32 && MODE == MODE_HEATBATH;        // heatbath: weak sites and weak draws redone in double
+    // ACC: the three SU(2) factors of a site are accumulated into G = g3 g2 g1 and applied to the links once (C8): 108
+    // multiply-adds per link instead of 144, but nothing independent is left to schedule beside the serial chain of the
+    // next subgroup step.  Measured (profiles/r2_variants.md E): pays for the relaxation kernels (+2..5 %) and the fp32
+    // 12-real heatbath kernel, costs the other heatbath kernels 4..6 %, whose chain is longer.
+#ifdef GF_ACCG
+    static constexpr bool ACC = ((GF_ACCG & 1) && R == 12) || ((GF_ACCG & 2) && MODE == MODE_HEATBATH) || (GF_ACCG & 4);
+#else
+    static constexpr bool ACC = MODE != MODE_HEATBATH || (sizeof(T) == 4 && R == 12);
+#endif
+    static constexpr int OUT_ROWS = (R == 12 && MON == 0) ? 2 : 3; // rows of an updated link that anybody reads
     static constexpr bool PAIR = MODE == MODE_HEATBATH && TPS >= 2;   // heatbath: two lanes of a site share the work of the draw
     static_assert(!DC || (FP32 && MODE == MODE_HEATBATH), "DC is a variant of the fp32 heatbath kernel");
     static_assert(MON == 0 || MODE != MODE_HEATBATH, "the monitor belongs to the relaxation sweeps");
@@ -635,7 +645,7 @@ struct SweepKernel {
     static __device__ __forceinline__ void subgroup(const SweepParams& p, const SweepPhase& ph, cx<CT> (&K)[9],
                                                     cx<T> (&F)[NMU][9], cx<T> (&B)[NMU][9], uint32_t site_canon,
                                                     bool record, const EarlyDraw<T>& early, int lane_mu0,
-                                                    cx<T> (&Gt)[9], bool& watch)
+                                                    cx<T> (&Gt)[9], bool& watch, cx<CT> (&Gacc)[9])
     {
         CT k[4], h[4], cond;
         su2_project<I, J>(K, k);
@@ -654,13 +664,17 @@ struct SweepKernel {
         if (FP32 && !DC) watch = watch || ((float)cond < p.watch_thr2);
         const cx<CT> ac = {h[0], h[3]}, bc = {h[2], h[1]}; // C4
         const cx<T> a = {(T)h[0], (T)h[3]}, b = {(T)h[2], (T)h[1]};
+        if (ACC) {
+            su2_left<I, J>(ac, bc, Gacc);               // G <- g G: applied to the links after the third step
+        } else {
 #pragma unroll
-        for (int m = 0; m < NMU; ++m) {
-            if (CB && lane_mu0 + m == 3) {
-                su2_left<I, J>(a, b, Gt);               // G(x) <- g G(x): the temporal links wait (reading B)
-            } else {
-                su2_left<I, J>(a, b, F[m]);             // U_mu(x)     <- G U_mu(x)
-                su2_right_dagger<I, J, 3>(a, b, B[m]);  // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
+            for (int m = 0; m < NMU; ++m) {
+                if (CB && lane_mu0 + m == 3) {
+                    su2_left<I, J>(a, b, Gt);               // G(x) <- g G(x): the temporal links wait (reading B)
+                } else {
+                    su2_left<I, J>(a, b, F[m]);             // U_mu(x)     <- G U_mu(x)
+                    su2_right_dagger<I, J, 3>(a, b, B[m]);  // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
+                }
             }
         }
         su2_left<I, J>(ac, bc, K);                      // K <- G K  (C8)
@@ -711,9 +725,26 @@ struct SweepKernel {
         }
         const bool record = lane_mu0 == 0;
         if (MON == 2 && p.mon.pre_part != nullptr) th_pre = record ? site_theta(K) : 0.0;
-        subgroup<CT, 0, 1, 0>(p, ph, K, F, B, sc, record, early[0], lane_mu0, Gt, watch); // Cabibbo-Marinari subgroups, order of C4
-        subgroup<CT, 0, 2, 1>(p, ph, K, F, B, sc, record, early[1], lane_mu0, Gt, watch);
-        subgroup<CT, 1, 2, 2>(p, ph, K, F, B, sc, record, early[2], lane_mu0, Gt, watch);
+        cx<CT> Gacc[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) Gacc[e] = {(e & 3) == 0 ? CT(1) : CT(0), CT(0)};
+        subgroup<CT, 0, 1, 0>(p, ph, K, F, B, sc, record, early[0], lane_mu0, Gt, watch, Gacc); // Cabibbo-Marinari subgroups, order of C4
+        subgroup<CT, 0, 2, 1>(p, ph, K, F, B, sc, record, early[1], lane_mu0, Gt, watch, Gacc);
+        subgroup<CT, 1, 2, 2>(p, ph, K, F, B, sc, record, early[2], lane_mu0, Gt, watch, Gacc);
+        if (ACC) {
+            cx<T> G[9]; // rounded to the type of the links once
+#pragma unroll
+            for (int e = 0; e < 9; ++e) G[e] = {(T)Gacc[e].re, (T)Gacc[e].im};
+#pragma unroll
+            for (int m = 0; m < NMU; ++m) {
+                if (CB && lane_mu0 + m == 3) {
+                    mat_left<3>(G, Gt);                       // G(x) <- G G(x)  (reading B)
+                } else {
+                    mat_left<OUT_ROWS>(G, F[m]);              // U_mu(x)     <- G U_mu(x)
+                    mat_right_dagger<OUT_ROWS>(G, B[m]);      // U_mu(x-mu)  <- U_mu(x-mu) G^dagger
+                }
+            }
+        }
         if (MON == 2 && p.mon.post_part != nullptr) th_post = record ? site_theta(K) : 0.0;
         return true;
     }
