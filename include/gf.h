@@ -298,7 +298,13 @@ int gf_chain_count(gf_ctx* ctx, unsigned long long* double_launches_host, unsign
 int gf_set_trial_buffer(gf_ctx* ctx, unsigned* d_trials);
 /* Number of kernels this ctx has launched so far. */
 unsigned long long gf_launch_count(const gf_ctx* ctx);
-/* Registers per thread and local-memory (spill) bytes per thread of the sweep kernel that the current
+/* Diagnostic: the double-precision functions of the fp64 annealing draw (C14) evaluated on n given Philox words x_i
+ * (device): neglog_dev[i] = -ln u_i, sin_dev[i] = sin(2 pi u_i), cos_dev[i] = cos(2 pi u_i), u_i = (2 (x_i >> 9) + 1) 2^-24.
+ * The kernels use their own branch-free versions of these functions (24-bit arguments); this call lets
+ * a test check them over the whole domain.  Each output may be NULL.  Asynchronous on `stream`.  GF_EINVAL: NULL words, n < 0. */
+int gf_debug_kp_math(const unsigned* words_dev, int n, double* neglog_dev, double* sin_dev, double* cos_dev, void* stream);
+/* Registers per thread and local-memory bytes per thread (spills; for the fp32 annealing kernels also the stack frame of
+ * their rare double-precision redo path, 200-300 bytes that the hot path never touches) of the sweep kernel that the current
  * (precision, storage, gauge reading, tuning) selects; mode 0 = overrelaxation, 1 = heatbath, 2 = gf_relax variants. */
 int gf_kernel_info(gf_ctx* ctx, int mode, int* regs_per_thread, int* local_bytes_per_thread);
 

@@ -72,6 +72,7 @@ SIGNATURES = {
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
     "gf_launch_count": (_ull, [_vp]),
     "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
+    "gf_debug_kp_math": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
 }
 
 _lib = None
@@ -348,6 +349,15 @@ def gf_chain_count(ctx):
 
 def gf_set_trial_buffer(ctx, d_trials) -> None:
     _check(ctx, load_library().gf_set_trial_buffer(ctx, _ptr(d_trials)))
+
+
+def gf_debug_kp_math(words_dev, neglog_dev=None, sin_dev=None, cos_dev=None, stream=None) -> None:
+    """-ln u, sin(2 pi u), cos(2 pi u) of the uniforms of the given Philox words (device uint32 / float64 tensors)"""
+    rc = load_library().gf_debug_kp_math(_ptr(words_dev), int(words_dev.numel()), _ptr(neglog_dev) if neglog_dev is not None else None,
+                                         _ptr(sin_dev) if sin_dev is not None else None,
+                                         _ptr(cos_dev) if cos_dev is not None else None, _stream(stream))
+    if rc != GF_OK:
+        raise GFError(rc, "gf_debug_kp_math")
 
 
 def gf_launch_count(ctx) -> int:

@@ -396,3 +396,31 @@ cudaError_t launch_theta(int prec, int R, const Lattice& L, int nt, int nd, cons
 }
 
 } // namespace gf
+
+// ---------------------------------------------------------------------------------------------------------
+// gf_debug_kp_math: the double-precision functions of the Kennedy-Pendleton draw (kp_neglog_word, kp_sincos2pi_word,
+// gf_device.cuh) on given Philox words, so that a test can check them over their whole domain (2^23 uniforms)
+// ---------------------------------------------------------------------------------------------------------
+__global__ void kp_math_kernel(const unsigned* __restrict__ words, int n, double* __restrict__ nl, double* __restrict__ sn,
+                               double* __restrict__ cs)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t x = words[i];
+    if (nl != nullptr) nl[i] = gf::kp_neglog_word(x);
+    if (sn != nullptr || cs != nullptr) {
+        double s, c;
+        gf::kp_sincos2pi_word(x, s, c);
+        if (sn != nullptr) sn[i] = s;
+        if (cs != nullptr) cs[i] = c;
+    }
+}
+
+extern "C" int gf_debug_kp_math(const unsigned* words_dev, int n, double* neglog_dev, double* sin_dev, double* cos_dev, void* stream)
+{
+    if (words_dev == nullptr || n < 0) return -1; // GF_EINVAL
+    if (n == 0) return 0;
+    kp_math_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(words_dev, n, neglog_dev, sin_dev, cos_dev);
+    return cudaGetLastError() == cudaSuccess ? 0 : -2; // GF_ECUDA
+}
+

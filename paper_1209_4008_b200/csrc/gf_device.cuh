@@ -447,4 +447,61 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Double-precision functions of the Kennedy-Pendleton draw (C14), written for their actual arguments: the
+// uniforms are u = (2 (x >> 9) + 1) 2^-24, 24-bit numbers.  The library's log / sincospi are general (special
+// cases behind branches, 64-bit immediates moved through uniform registers: ~80 / ~75 instructions each),
+// and the fp64 annealing kernel is bound by instruction issue and instruction fetch, not by memory
+// (profiles/r2_ncu_heatbath.md).  Here: branch-free, coefficients as constant-bank operands, ~30 instructions
+// each, errors of a few 1e-16 (checked over all 2^23 arguments by tests/test_gpu_variants.py through
+// gf_debug_kp_math).  Tables: gf_kp_tables.inc, written by gen_kp_tables.py.
+// ---------------------------------------------------------------------------------------------------------
+#include "gf_kp_tables.inc"
+
+// -ln u, u the uniform of the Philox word x.  u = m 2^(e-24), m in [1,2) from the leading one of w = 2 (x >> 9) + 1;
+// bin j = top 7 bits of m; f = m r_j - 1 (exact), ln m = T_j + log1p(f); for j >= 64 the table holds T_j - ln 2 and the
+// exponent counts one more, so that nothing cancels as u -> 1.
+__device__ __forceinline__ double kp_neglog_word(uint32_t x)
+{
+    const uint32_t w = 2u * (x >> 9) + 1u; // odd, < 2^24
+    const int lz = __clz((int)w);          // >= 8
+    const uint32_t mi = w << (lz - 8);     // 24 bits, leading one at bit 23: m = mi 2^-23
+    const int j = (int)((mi >> 16) & 127u);
+    const double2 t = GF_KP_LOG_TAB[j];
+    const double m = __hiloint2double((int)(0x3FF00000u | ((mi >> 3) & 0xFFFFFu)), (int)(mi << 29));
+    const double f = fma(m, t.x, -1.0);
+    double p = 1.0 / 7.0;
+    p = fma(p, f, -1.0 / 6.0);
+    p = fma(p, f, 1.0 / 5.0);
+    p = fma(p, f, -1.0 / 4.0);
+    p = fma(p, f, 1.0 / 3.0);
+    p = fma(p, f, -1.0 / 2.0);
+    p = fma(p, f, 1.0);
+    p *= f; // log1p(f), |f| < 0.006
+    const double n = (double)(lz - (j < 64 ? 7 : 8)); // 24 - e, e = 31 - lz; one less where the table took ln 2
+    return fma(n, GF_KP_LN2_HI, fma(n, GF_KP_LN2_LO, -p) - t.y);
+}
+
+// sin(2 pi u), cos(2 pi u), u the uniform of the Philox word x: 4u = q + r exactly, q = 0..4, |r| <= 1/2;
+// sin / cos(pi r / 2) by their series in r^2, then the quadrant
+__device__ __forceinline__ void kp_sincos2pi_word(uint32_t x, double& sn, double& cs)
+{
+    const uint32_t w = 2u * (x >> 9) + 1u;             // 4u = w 2^-22
+    const uint32_t q = (w + (1u << 21)) >> 22;         // nearest integer (w is odd: no ties)
+    const double r = (double)((int)w - (int)(q << 22)) * (1.0 / 4194304.0);
+    const double z = r * r;
+    double s = GF_KP_S7;
+    s = fma(s, z, GF_KP_S6); s = fma(s, z, GF_KP_S5); s = fma(s, z, GF_KP_S4); s = fma(s, z, GF_KP_S3);
+    s = fma(s, z, GF_KP_S2); s = fma(s, z, GF_KP_S1); s = fma(s, z, GF_KP_S0);
+    s *= r;
+    double c = GF_KP_C8;
+    c = fma(c, z, GF_KP_C7); c = fma(c, z, GF_KP_C6); c = fma(c, z, GF_KP_C5); c = fma(c, z, GF_KP_C4);
+    c = fma(c, z, GF_KP_C3); c = fma(c, z, GF_KP_C2); c = fma(c, z, GF_KP_C1); c = fma(c, z, GF_KP_C0);
+    // angle = (pi/2)(q + r): q = 0: (s, c); 1: (c, -s); 2: (-s, -c); 3: (-c, s); 4 = 0
+    const bool swap = (q & 1u) != 0u;
+    const double a = swap ? c : s, b = swap ? s : c;
+    sn = (q & 2u) ? -a : a;
+    cs = (((q + 1u) & 2u) != 0u) ? -b : b;
+}
+
 } // namespace gf

@@ -209,12 +209,13 @@ template <typename T> struct KPMath;
 // within ~1e-15 of the threshold, i.e. with probability ~1e-15 per trial (tests compare every trial count).
 template <> struct KPMath<double> {
     static __device__ __forceinline__ double uni(uint32_t x) { return (double)(2u * (x >> 9) + 1u) * (1.0 / 16777216.0); }
-    static __device__ __forceinline__ double neglog(double u) { return -log(u); }
+    static __device__ __forceinline__ double neglog_w(uint32_t x) { return kp_neglog_word(x); } // -ln uni(x), gf_device.cuh
     static __device__ __forceinline__ double root(double x) { return x > 0.0 ? x * rsqrt(x) : 0.0; }
     // the angle of a trial (u3) as it enters sincos2pi; cos^2 of it from the cosine
     static __device__ __forceinline__ double trial_angle(double u3) { return u3; }
     static __device__ __forceinline__ double cos_squared(double c) { return c * c; }
-    static __device__ __forceinline__ void sincos2pi(double a, double& sn, double& cs) { sincospi(2.0 * a, &sn, &cs); }
+    // sine and cosine of 2 pi uni(x): of the trial's angle (pair = false) and of the direction's (pair = true) alike
+    static __device__ __forceinline__ void sincos_w(uint32_t x, bool dir, double& sn, double& cs) { (void)dir; kp_sincos2pi_word(x, sn, cs); }
     static __device__ __forceinline__ bool decide(const TrialPre<double>& t, double inv_alpha, double& d, double& est, bool& border)
     {
         (void)border;
@@ -236,6 +237,7 @@ template <> struct KPMath<float> {
     // (2 (x >> 9) + 1) 2^-24 = [1 + (x >> 9) 2^-23] - (1 - 2^-24): both terms and the result are fp32 numbers
     static __device__ __forceinline__ float uni(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)) - 0.99999994039535522461f; }
     static __device__ __forceinline__ float neglog(float u) { return -0.693147180559945f * __log2f(u); }
+    static __device__ __forceinline__ float neglog_w(uint32_t x) { return neglog(uni(x)); }
     static __device__ __forceinline__ float root(float x) { return x > 0.0f ? x * rsqrtf(x) : 0.0f; }
     // cos^2(2 pi u3) = (1 + cos(4 pi u3)) / 2, the argument folded exactly into [-pi, pi] (MUFU.COS is specified
     // there): the absolute error of c^2 is half that of the SFU cosine instead of 2 |c| times it
@@ -246,6 +248,12 @@ template <> struct KPMath<float> {
         const float x = 6.283185307179586f * a;
         sn = __sinf(x);
         cs = __cosf(x);
+    }
+    // sine and cosine of the direction's angle 2 pi uni(x) (dir) or of the trial's folded angle (cos_squared takes that cosine)
+    static __device__ __forceinline__ void sincos_w(uint32_t x, bool dir, float& sn, float& cs)
+    {
+        const float u = uni(x);
+        sincos2pi(dir ? u : trial_angle(u), sn, cs);
     }
     // delta of a trial from its uniforms with the 1-ulp library functions instead of the SFU
     static __device__ __forceinline__ float accurate_delta(const uint32_t (&x)[4], float inv_alpha)
@@ -271,9 +279,9 @@ __device__ __forceinline__ TrialPre<DT> kp_trial_pre(const uint32_t (&x)[4])
 {
     using M = KPMath<DT>;
     DT sn, cs;
-    M::sincos2pi(M::trial_angle(M::uni(x[2])), sn, cs);
+    M::sincos_w(x[2], false, sn, cs);
     (void)sn;
-    const DT l1 = M::neglog(M::uni(x[0])), l2 = M::neglog(M::uni(x[1]));
+    const DT l1 = M::neglog_w(x[0]), l2 = M::neglog_w(x[1]);
     TrialPre<DT> t;
     t.s = gf_fma(l1, M::cos_squared(cs), l2);
     t.lsum = DT(1) + l1 + l2;
@@ -295,7 +303,7 @@ __device__ __forceinline__ void early_draw(uint32_t key0, uint32_t key1, uint32_
     const DT cos_t = DT(1) - DT(2) * M::uni(x[0]);
     const DT sin_t = M::root(DT(1) - cos_t * cos_t);
     DT sn, cs;
-    M::sincos2pi(M::uni(x[1]), sn, cs);
+    M::sincos_w(x[1], true, sn, cs);
     e.e1 = sin_t * cs;
     e.e2 = sin_t * sn;
     e.e3 = cos_t;
@@ -324,9 +332,9 @@ __device__ __forceinline__ void early_draw_pair(uint32_t key0, uint32_t key1, ui
     philox4x32_10(c0, c1, c2, role ? 0x80000000u : 0u, key0, key1, y);
     const uint32_t x1 = __shfl_sync(mask, y[1], src0); // u2 and u4 of the trial, generated by role 0
     const uint32_t x3 = __shfl_sync(mask, y[3], src0);
-    const DT l = M::neglog(M::uni(role ? x1 : y[0]));
+    const DT l = M::neglog_w(role ? x1 : y[0]);
     DT sn, cs;
-    M::sincos2pi(role ? M::uni(y[1]) : M::trial_angle(M::uni(y[2])), sn, cs);
+    M::sincos_w(role ? y[1] : y[2], role, sn, cs);
     const DT cos_t = DT(1) - DT(2) * M::uni(y[0]); // meaningful on role 1
     const DT sin_t = M::root(DT(1) - cos_t * cos_t);
     const DT l1 = Shfl<DT>::get(mask, l, src0), l2 = Shfl<DT>::get(mask, l, src1);
@@ -469,7 +477,7 @@ static __device__ __noinline__ unsigned fix_heatbath_step(const double (&k)[4], 
     const double cos_t = 1.0 - 2.0 * M::uni(x[0]);
     const double sin_t = M::root(1.0 - cos_t * cos_t);
     double sn, cs;
-    M::sincos2pi(M::uni(x[1]), sn, cs);
+    M::sincos_w(x[1], true, sn, cs);
     const double r = M::root(d * (2.0 - d));
     const double h0 = 1.0 - d, h1 = r * (sin_t * cs), h2 = r * (sin_t * sn), h3 = r * cos_t;
     g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3; // g = h (x) conj(khat)  (C13)

@@ -532,3 +532,38 @@ def test_fused_monitor_stochastic_and_fallback(gfm):
     with pytest.raises(gfm.GFError):
         gfm.gf_monitor_last(fx.ctx, 4)
     fx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the fp64 annealing draw's own log / sin / cos (branch-free, for 24-bit uniforms) over their WHOLE domain
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.gpu
+def test_kp_double_math_over_all_uniforms(gfm):
+    """kp_neglog_word / kp_sincos2pi_word (gf_device.cuh) against numpy on every one of the 2^23 uniforms
+    u = (2m + 1) 2^-24: -ln u to 4e-16 relative (also as u -> 1, where it falls to 6e-8), sine and cosine to 5e-16
+    absolute.  The reference reduces the angle exactly (4u = q + r) before it calls numpy, so that it carries no
+    argument-rounding error of its own."""
+    import torch
+
+    m = np.arange(2**23, dtype=np.uint64)
+    words = torch.from_numpy((m << 9).astype(np.uint32).view(np.int32)).cuda()  # x >> 9 = m
+    nl = torch.empty(m.size, dtype=torch.float64, device="cuda")
+    sn, cs = torch.empty_like(nl), torch.empty_like(nl)
+    gfm.gf_debug_kp_math(words, nl, sn, cs)
+    torch.cuda.synchronize()
+    w = 2 * m + 1
+    u = w.astype(np.float64) / 2.0**24
+    # -ln u: log1p(u - 1) is the accurate form near 1 (u - 1 is exact)
+    ref = np.where(u > 0.5, -np.log1p(u - 1.0), -np.log(u))
+    rel = np.abs(nl.cpu().numpy() - ref) / ref
+    assert rel.max() <= 4e-16, (rel.max(), int(rel.argmax()))
+    q = (w + 2**21) >> 22
+    r = (w.astype(np.int64) - (q.astype(np.int64) << 22)).astype(np.float64) / 2.0**22
+    s0, c0 = np.sin(0.5 * np.pi * r), np.cos(0.5 * np.pi * r)
+    qq = (q & 3).astype(np.int64)
+    ref_s = np.choose(qq, [s0, c0, -s0, -c0])
+    ref_c = np.choose(qq, [c0, -s0, -c0, s0])
+    assert np.abs(sn.cpu().numpy() - ref_s).max() <= 5e-16
+    assert np.abs(cs.cpu().numpy() - ref_c).max() <= 5e-16
+    # a spot check against the plain definition, argument rounding included
+    assert np.abs(cs.cpu().numpy()[::4097] - np.cos(2 * np.pi * u[::4097])).max() <= 2e-15
