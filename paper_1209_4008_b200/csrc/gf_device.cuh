@@ -452,9 +452,10 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 // uniforms are u = (2 (x >> 9) + 1) 2^-24, 24-bit numbers.  The library's log / sincospi are general (special
 // cases behind branches, 64-bit immediates moved through uniform registers: ~80 / ~75 instructions each),
 // and the fp64 annealing kernel is bound by instruction issue and instruction fetch, not by memory
-// (profiles/r2_ncu_heatbath.md).  Here: branch-free, coefficients as constant-bank operands, ~30 instructions
-// each, errors of a few 1e-16 (checked over all 2^23 arguments by tests/test_gpu_variants.py through
-// gf_debug_kp_math).  Tables: gf_kp_tables.inc, written by gen_kp_tables.py.
+// (profiles/r2_ncu_heatbath.md).  Here: branch-free, ~35 instructions each, errors of a few 1e-16 (checked over
+// all 2^23 arguments by tests/test_gpu_variants.py through gf_debug_kp_math).  Tables: gf_kp_tables.inc, written
+// by gen_kp_tables.py.  (The coefficients stay literals: read from a __constant__ array instead, ptxas keeps
+// them in registers across the three subgroup steps and the kernel spills 248 bytes -- 219 -> 247 us.)
 // ---------------------------------------------------------------------------------------------------------
 #include "gf_kp_tables.inc"
 
