@@ -194,11 +194,12 @@ __device__ __forceinline__ void su2_variant_step(const T (&k)[4], int variant, d
 template <typename DT> struct TrialPre {
     DT s;     // l1 c^2 + l2, l = -ln u
     DT lsum;  // 1 + l1 + l2: scale of the absolute error of the SFU value of s (fp32 draw only)
-    DT u4;
+    float u4; // a 24-bit number: exact as a float also in the fp64 draw (one register instead of two)
 };
 template <typename DT> struct EarlyDraw {
     TrialPre<DT> t0;  // trial 0
-    DT e1, e2, e3;    // direction of hvec, from the Philox block with counter word 3 = 0x80000000
+    DT e1, e2;        // direction of hvec, from the Philox block with counter word 3 = 0x80000000
+    float e3;         // = cos(polar angle) = 1 - 2u, a 24-bit number
 };
 
 template <typename T> struct KPMath;
@@ -221,7 +222,8 @@ template <> struct KPMath<double> {
         (void)border;
         est = 0.0; // never refined
         d = t.s * inv_alpha;
-        return t.u4 * t.u4 <= fma(-0.5, d, 1.0);
+        const double u4 = (double)t.u4;
+        return u4 * u4 <= fma(-0.5, d, 1.0);
     }
 };
 
@@ -285,7 +287,7 @@ __device__ __forceinline__ TrialPre<DT> kp_trial_pre(const uint32_t (&x)[4])
     TrialPre<DT> t;
     t.s = gf_fma(l1, M::cos_squared(cs), l2);
     t.lsum = DT(1) + l1 + l2;
-    t.u4 = M::uni(x[3]);
+    t.u4 = KPMath<float>::uni(x[3]);
     return t;
 }
 
@@ -306,7 +308,7 @@ __device__ __forceinline__ void early_draw(uint32_t key0, uint32_t key1, uint32_
     M::sincos_w(x[1], true, sn, cs);
     e.e1 = sin_t * cs;
     e.e2 = sin_t * sn;
-    e.e3 = cos_t;
+    e.e3 = (float)cos_t;
 }
 
 // The same for kernels in which two (or four) threads share a site: the two lanes of a pair (lane, lane ^ 1) run ONE
@@ -340,10 +342,10 @@ __device__ __forceinline__ void early_draw_pair(uint32_t key0, uint32_t key1, ui
     const DT l1 = Shfl<DT>::get(mask, l, src0), l2 = Shfl<DT>::get(mask, l, src1);
     e.t0.s = gf_fma(l1, M::cos_squared(Shfl<DT>::get(mask, cs, src0)), l2);
     e.t0.lsum = DT(1) + l1 + l2;
-    e.t0.u4 = M::uni(x3);
+    e.t0.u4 = KPMath<float>::uni(x3);
     e.e1 = Shfl<DT>::get(mask, sin_t * cs, src1);
     e.e2 = Shfl<DT>::get(mask, sin_t * sn, src1);
-    e.e3 = Shfl<DT>::get(mask, cos_t, src1);
+    e.e3 = Shfl<float>::get(mask, (float)cos_t, src1);
 }
 
 // returns the number of trials used (0: degenerate block, identity taken; 4097: cap hit); cond = |k|^2 (the
@@ -423,7 +425,7 @@ __device__ __forceinline__ unsigned su2_heatbath_step(const CT (&k)[4], double T
     }
     const DT h0d = DT(1) - d;
     const DT r = M::root(d * (DT(2) - d)); // = sqrt(1 - h0^2) without the cancellation at small delta
-    const CT h0 = (CT)h0d, h1 = (CT)(r * early.e1), h2 = (CT)(r * early.e2), h3 = (CT)(r * early.e3);
+    const CT h0 = (CT)h0d, h1 = (CT)(r * early.e1), h2 = (CT)(r * early.e2), h3 = (CT)(r * (DT)early.e3);
     // g = h (x) conj(khat):  (pq)_0 = p0 q0 - p.q,  (pq)_vec = p0 qvec + q0 pvec - pvec x qvec   (C13)
     g[0] = h0 * kc0 - h1 * kc1 - h2 * kc2 - h3 * kc3;
     g[1] = h0 * kc1 + kc0 * h1 - (h2 * kc3 - h3 * kc2);
@@ -595,7 +597,7 @@ __device__ __forceinline__ void pin_early(const EarlyDraw<float>& e)
 }
 __device__ __forceinline__ void pin_early(const EarlyDraw<double>& e)
 {
-    asm volatile("" :: "d"(e.t0.s), "d"(e.t0.u4), "d"(e.e1), "d"(e.e2), "d"(e.e3));
+    asm volatile("" :: "d"(e.t0.s), "f"(e.t0.u4), "d"(e.e1), "d"(e.e2), "f"(e.e3));
 }
 
 __device__ __forceinline__ int tie_bits(float x) { return __float_as_int(x); }
