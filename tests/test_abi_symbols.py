@@ -70,3 +70,28 @@ def test_product_does_not_import_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src, f
                 assert "gf_oracle" not in src and "liborc" not in src, f
+
+
+def test_kp_tables_are_what_their_generator_writes():
+    """csrc/gf_kp_tables.inc (constants of the fp64 annealing draw's -ln u / sin / cos) is the output of the committed
+    generator, and its table obeys what the kernel relies on: r_j has at most 10 significant bits (m r_j - 1 exact),
+    |m r_j - 1| < 0.006 over the bin, T_j = -ln r_j (minus ln 2 in the upper half), last bin exactly (1/2, 0)."""
+    import math
+    import re
+    import subprocess
+    import sys
+
+    here = os.path.join(ROOT, "paper_1209_4008_b200", "csrc")
+    out = subprocess.run([sys.executable, os.path.join(here, "gen_kp_tables.py")], capture_output=True, text=True, check=True).stdout
+    with open(os.path.join(here, "gf_kp_tables.inc")) as fh:
+        assert fh.read() == out
+    rows = re.findall(r"\{(0x[0-9a-fp.+-]+), (-?0x[0-9a-fp.+-]+)\}", out)
+    assert len(rows) == 128
+    for j, (r, t) in enumerate(rows):
+        r, t = float.fromhex(r), float.fromhex(t)
+        assert (r * 1024).is_integer() and 0.5 <= r <= 1.0
+        lo, hi = 1 + j / 128, 1 + (j + 1) / 128
+        assert max(abs(lo * r - 1), abs(hi * r - 1)) < 0.006
+        want = -math.log(r) - (math.log(2) if j >= 64 else 0.0)
+        assert abs(t - want) <= 2e-16
+    assert rows[127] == ("0x1.0000000000000p-1", "0x0.0p+0")
