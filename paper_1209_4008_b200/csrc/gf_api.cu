@@ -31,6 +31,7 @@ struct gf_ctx {
     float fix_threshold;              // heatbath: |k| below which a site update is redone in double
     int* d_rough;                     // hybrid chain: ring of ROUGH_RING flags + 4 words for two diagnostic counters
     unsigned long long call_sweeps;   // sweeps since the start of the current API call (cadence of the reunitarisation)
+    int force_rough;                  // hybrid chain: run the double chain regardless of the flags (relaxation sweeps inside an annealing)
     unsigned long long half_sweeps;   // half-sweeps of any kind since creation (alternates the traversal direction)
     unsigned long long launches;
     unsigned* d_trials;
@@ -118,7 +119,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precisi
     c->prefetch = -1; // automatic
     c->chain = CHAIN_HYBRID; c->watch_threshold = 1.0f; c->fix_threshold = 0.15f; c->d_rough = nullptr;
     c->coulomb_b = -1; c->d_gfield = nullptr; // automatic: reading B in fp32, A in fp64 (uses_reading_b)
-    c->call_sweeps = 0; c->half_sweeps = 0; c->launches = 0;
+    c->call_sweeps = 0; c->half_sweeps = 0; c->launches = 0; c->force_rough = 0;
     c->d_trials = nullptr; c->last_stream = nullptr;
     c->d_canon = nullptr; c->d_native = nullptr;
     memset(c->slot, 0, sizeof c->slot);
@@ -449,7 +450,7 @@ static void set_phase(gf_ctx* c, SweepParams& p, int parity, bool reunit)
     p.ph.reverse = c->l2_reversal ? (int)(c->half_sweeps & 1ull) : 0;
     // hybrid chain (fp32): the ring position counts the half-sweeps of the call; its first sweep runs the double chain
     p.ph.rough_slot = (int)((2ull * c->call_sweeps + (unsigned)parity) % ROUGH_RING);
-    p.ph.rough_force = c->call_sweeps == 0 ? 1 : 0;
+    p.ph.rough_force = (c->call_sweeps == 0 || c->force_rough) ? 1 : 0;
 }
 
 // start of an API call that sweeps: the sweep counter of the call and, for the hybrid chain, a clean flag ring
@@ -654,9 +655,14 @@ extern "C" int gf_anneal_micro(gf_ctx* c, void* U, double T_start, double T_end,
         if (rc != GF_OK) break;
         c->call_sweeps += 1;
         // microcanonical sweeps g -> g^2 (C19): stochastic relaxation with p = 2 > u, i.e. always
-        if (n_micro > 0)
+        if (n_micro > 0) {
+            // the field between heatbath sweeps is rough by construction and the heatbath kernel keeps no roughness flags:
+            // fp32 contexts run the site chain of these sweeps in double (hybrid chain forced)
+            c->force_rough = 1;
             rc = run_sweeps_core(c, U, MODE_VARIANT, VARIANT_STOCHASTIC, 2.0, n_micro, 0, seed, st,
                                  "gf_anneal_micro: kernel launch", nullptr, gfield, &launched);
+            c->force_rough = 0;
+        }
     }
     // after a failed launch the temporal links are still transformed with the g(x) accumulated so far (reading B)
     if (rc == GF_OK || launched > 0) {
