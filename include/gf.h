@@ -122,6 +122,45 @@ int gf_theta(gf_ctx* ctx, const void* U_native_dev, double* theta_host);
 /* per-timeslice theta_t = (1 / (V_s N_c)) sum_{x in slice t} tr[Delta Delta^dagger]; theta_host_Nt: Nt doubles */
 int gf_theta_slices(gf_ctx* ctx, const void* U_native_dev, double* theta_host_Nt);
 
+/* ---- theta without any allocation ---------------------------------------------------------------------------- */
+
+/* The same theta reduction as gf_theta / gf_theta_slices (same kernels, same summation order), for callers that are
+ * not allowed to allocate GPU memory: a host program that claimed the whole GPU for its own memory pool at start-up,
+ * or one that runs under a fixed memory budget next to other jobs, cannot let a library call cudaMalloc behind its
+ * back (it fails, or eats memory already promised elsewhere), and a measurement loop that checks theta every few
+ * sweeps cannot afford the device-wide stall of a cudaMalloc / cudaFree.  Every other reduction here needs a gf_ctx,
+ * and gf_create allocates.  This call needs no context and calls no cudaMalloc, cudaFree, cudaMallocHost or any other
+ * allocating routine: the field and the output are the caller's, and the only scratch the reduction needs (one partial
+ * sum per thread block) is a fixed array compiled into libgf.so.
+ *
+ *   Nx..Nt, precision, gauge, reals_per_link: as for gf_create / gf_set_storage (no slabs).
+ *   U_native_dev: device, the field in the native layout (gf_field_bytes bytes), read only.
+ *   out_dev:      device, Nt + 2 doubles owned by the caller, fully overwritten: out[0] = theta of the whole lattice
+ *                 (eq. 2.5; what gf_theta returns in Landau gauge), out[1] = max_t theta_t (what gf_theta returns in
+ *                 Coulomb gauge), out[2 + t] = theta_t (gf_theta_slices).
+ *   stream:       the work is only enqueued; out_dev is valid once the stream has reached this point.
+ *   err, err_len: optional host buffer for the message of a failing call (NULL / 0: no message).
+ *
+ * Limit: the built-in scratch holds gf_theta_static_max_partials() = 131072 doubles (1 MiB).  A lattice needs
+ * 2 * Nt * ceil(Nx/2 * Ny * Nz / 256) of them -- 65536 at 64^4, 27648 at 48^3 x 64 -- and a larger one is refused with
+ * GF_EINVAL and a message naming both numbers; nothing is launched.  The price of the array: that 1 MiB is held on
+ * every GPU a process has loaded libgf.so on, until the process exits, used or not.
+ *
+ * First call on each device: it looks up where the array lives on that device (once; the device must be current, as
+ * for every call here) and remembers it.  That look-up is set-up work, not stream work: make the first call on a device
+ * during initialisation, before any stream capture is open.  Later calls only launch the two reduction kernels.
+ *
+ * Sharing: all calls on one GPU use the same array, and it keeps whatever the last call wrote.  That is harmless --
+ * nothing in it has to start at zero, every launch writes each slot before reading it -- but two calls that run on the
+ * GPU at the same time (two streams, two host threads) overwrite each other's partial sums and both results are
+ * garbage.  Order them: one stream, or an event between them.  gf_theta on a context does not touch this array.
+ *
+ * GF_EINVAL: extents (odd, < 2, V >= 2^31), unknown precision / gauge / storage, NULL field or output, lattice beyond
+ * the limit.  GF_ECUDA: the array's address cannot be resolved, or a launch fails. */
+int gf_theta_static(int Nx, int Ny, int Nz, int Nt, int precision, int gauge, int reals_per_link,
+                    const void* U_native_dev, double* out_dev, void* stream, char* err, size_t err_len);
+size_t gf_theta_static_max_partials(void);
+
 /* ---- Alg. 1 with its stop rule -------------------------------------------------------------------------------- */
 
 /* "while precision theta not reached do" with the check after every `check_every`-th sweep

@@ -73,6 +73,8 @@ SIGNATURES = {
     "gf_launch_count": (_ull, [_vp]),
     "gf_kernel_info": (_i, [_vp, _i, _pi, _pi]),
     "gf_debug_kp_math": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
+    "gf_theta_static": (_i, [_i, _i, _i, _i, _i, _i, _i, _vp, _vp, _vp, ctypes.c_char_p, _sz]),
+    "gf_theta_static_max_partials": (_sz, []),
 }
 
 _lib = None
@@ -260,6 +262,24 @@ def gf_theta_slices(ctx, U, Nt: int):
     out = (ctypes.c_double * Nt)()
     _check(ctx, load_library().gf_theta_slices(ctx, _ptr(U), out))
     return list(out)
+
+
+def gf_theta_static(dims, precision: int, gauge: int, reals_per_link: int, U, out_dev, stream=None) -> None:
+    """theta without a context and without any allocation inside the library (include/gf.h, gf_theta_static): for host
+    programs that own all of the GPU's memory themselves or must not stall the device on an allocation.  ``U``: native
+    field (device), ``out_dev``: Nt + 2 doubles on the device, written asynchronously on ``stream``: [0] theta of the
+    lattice, [1] max over timeslices, [2 + t] theta_t.  The scratch is one fixed 1 MiB array per GPU shared by all
+    calls: lattices needing more than ``gf_theta_static_max_partials()`` block partials raise GFError(GF_EINVAL), and
+    calls that overlap on the GPU race.  Make the first call on a device at set-up, before any stream capture."""
+    err = ctypes.create_string_buffer(512)
+    rc = load_library().gf_theta_static(int(dims[0]), int(dims[1]), int(dims[2]), int(dims[3]), int(precision), int(gauge),
+                                        int(reals_per_link), _ptr(U), _ptr(out_dev), _stream(stream), err, len(err))
+    if rc != GF_OK:
+        raise GFError(rc, err.value.decode())
+
+
+def gf_theta_static_max_partials() -> int:
+    return int(load_library().gf_theta_static_max_partials())
 
 
 def gf_overrelax_host(ctx, U_canon_host, omega: float, nsweeps: int):

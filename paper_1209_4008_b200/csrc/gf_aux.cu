@@ -2,6 +2,9 @@
 // kernel: "checks the current value of the gauge fixing functional F_g[U] and the gauge precision
 // theta").  Reductions: fp64 arithmetic on the stored links, warp shuffles inside a block, one partial per block,
 // then a single-block final pass that adds the partials in a fixed order (deterministic, no atomics).
+#include <cstdarg>
+#include <cstdio>
+
 #include "gf_internal.h"
 #include "gf_device.cuh"
 
@@ -424,3 +427,108 @@ extern "C" int gf_debug_kp_math(const unsigned* words_dev, int n, double* neglog
     return cudaGetLastError() == cudaSuccess ? 0 : -2; // GF_ECUDA
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// gf_theta_static (include/gf.h): the theta reduction for callers that must not allocate.
+//
+// Who that is.  A gauge-fixing step usually sits inside somebody else's program: a Monte Carlo or measurement code that
+// took (nearly) all of the GPU's memory into its own pool when it started, or a job that shares the GPU under a fixed
+// memory budget.  From there a cudaMalloc inside this library either fails outright or takes memory the host program
+// has already promised elsewhere; and every cudaMalloc / cudaFree stalls the whole device while the driver maps memory,
+// which is poison for a loop that checks theta every few sweeps.  gf_theta goes through a gf_ctx, and gf_create
+// allocates.  This entry point needs no context and asks the driver for nothing: its inputs and outputs are the
+// caller's, and the one piece of scratch the reduction needs -- one partial sum per thread block -- is the fixed array
+// below, which is part of the library image itself.
+//
+// What it costs.  kStaticPartials doubles (1 MiB) of device memory on every GPU on which a process has loaded
+// libgf.so, from the load until the process exits, whether or not this call is ever used.  A lattice that needs more
+// block partials than that is refused (GF_EINVAL), not truncated.
+//
+// Sharing.  There is one array per GPU and every call on that GPU uses it.  Nothing in it has to start at zero: a launch
+// writes every slot it later reads (one per block of the grid) before the final pass reads them, so the values a
+// previous call left behind are never seen and no clearing pass is launched.  Two calls that are on the GPU at the
+// same time (different streams, different host threads) write the same slots and read each other's sums: the caller
+// must order them (same stream, or an event between them).
+// ---------------------------------------------------------------------------------------------------------
+namespace gf {
+
+constexpr size_t kStaticPartials = 131072; // 64^4 needs 65536, 48^3 x 64 needs 27648, 64^3 x 128 exactly this many
+constexpr int kStaticMaxDevices = 64;
+
+// In device code this name IS the array.  In host code it is only a handle for the runtime's symbol calls -- never a
+// device address: handing `static_partials` itself to a kernel from the host would give it a host address.
+static __device__ __align__(256) double static_partials[kStaticPartials];
+
+static double* g_static_partials_addr[kStaticMaxDevices]; // device address of the array on device i, once resolved
+static int g_static_lock;                                  // spin flag guarding the table (no mutex header needed)
+
+// Resolve, once per device and with that device current, where the array lives on it.
+static cudaError_t static_partials_address(double** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    while (__atomic_exchange_n(&g_static_lock, 1, __ATOMIC_ACQUIRE)) { }
+    double* p = g_static_partials_addr[dev];
+    if (p == nullptr) {
+        e = cudaGetSymbolAddress((void**)&p, static_partials);
+        if (e == cudaSuccess && p == nullptr) e = cudaErrorInvalidSymbol;
+        if (e == cudaSuccess) g_static_partials_addr[dev] = p;
+    }
+    __atomic_store_n(&g_static_lock, 0, __ATOMIC_RELEASE);
+    if (e == cudaSuccess) *out = p;
+    return e;
+}
+
+static int static_fail(char* err, size_t err_len, int code, const char* fmt, ...)
+{
+    if (err != nullptr && err_len > 0) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(err, err_len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+} // namespace gf
+
+extern "C" size_t gf_theta_static_max_partials(void) { return gf::kStaticPartials; }
+
+extern "C" int gf_theta_static(int Nx, int Ny, int Nz, int Nt, int precision, int gauge, int reals_per_link,
+                               const void* U_native_dev, double* out_dev, void* stream, char* err, size_t err_len)
+{
+    using namespace gf;
+    const char* who = "gf_theta_static";
+    if (err != nullptr && err_len > 0) err[0] = 0;
+    const int N[4] = {Nx, Ny, Nz, Nt};
+    for (int d = 0; d < 4; ++d)
+        if (N[d] < 2 || (N[d] & 1))
+            return static_fail(err, err_len, -1, "%s: extent %d is %d; every extent must be even and >= 2", who, d, N[d]);
+    const unsigned long long V = (unsigned long long)Nx * Ny * Nz * Nt;
+    if (V >= (1ull << 31)) return static_fail(err, err_len, -1, "%s: volume %llu >= 2^31", who, V);
+    if (precision != 0 && precision != 1) return static_fail(err, err_len, -1, "%s: unknown precision %d", who, precision);
+    if (gauge != 0 && gauge != 1) return static_fail(err, err_len, -1, "%s: unknown gauge %d", who, gauge);
+    if (reals_per_link != 12 && reals_per_link != 18)
+        return static_fail(err, err_len, -1, "%s: reals_per_link must be 12 or 18, got %d", who, reals_per_link);
+    if (U_native_dev == nullptr || out_dev == nullptr) return static_fail(err, err_len, -1, "%s: NULL field or output", who);
+
+    Lattice L;
+    L.Nxh = Nx / 2; L.Ny = Ny; L.Nz = Nz; L.Nt = Nt; L.H = (unsigned)(V / 2);
+    L.Hp = (L.H + 31u) & ~31u;
+    const unsigned long long need = (unsigned long long)reduce_blocks_per_slice(L) * 2ull * (unsigned long long)Nt;
+    if (need > kStaticPartials)
+        return static_fail(err, err_len, -1,
+                           "%s: a %dx%dx%dx%d lattice needs %llu block partials, the built-in scratch holds %zu (%zu KiB); "
+                           "use gf_theta on a context for lattices this large",
+                           who, Nx, Ny, Nz, Nt, need, (size_t)kStaticPartials, (size_t)(kStaticPartials * sizeof(double) / 1024));
+
+    double* partials = nullptr;
+    cudaError_t e = static_partials_address(&partials);
+    if (e != cudaSuccess)
+        return static_fail(err, err_len, -2, "%s: address of the built-in scratch: %s", who, cudaGetErrorString(e));
+    e = launch_theta(precision, reals_per_link, L, Nt, gauge == 1 ? 3 : 4, U_native_dev, partials, out_dev, (cudaStream_t)stream);
+    if (e != cudaSuccess) return static_fail(err, err_len, -2, "%s: launch: %s", who, cudaGetErrorString(e));
+    return 0;
+}

@@ -95,3 +95,17 @@ def test_kp_tables_are_what_their_generator_writes():
         want = -math.log(r) - (math.log(2) if j >= 64 else 0.0)
         assert abs(t - want) <= 2e-16
     assert rows[127] == ("0x1.0000000000000p-1", "0x0.0p+0")
+
+
+def test_theta_static_refuses_oversized_lattices_before_touching_the_device(lib):
+    """gf_theta_static (no allocation, fixed 1 MiB scratch inside the library): the size check is host arithmetic and
+    comes before any CUDA call, so it can be checked without a GPU."""
+    assert lib.gf_theta_static_max_partials() == 131072
+    with pytest.raises(lib.GFError) as err:
+        lib.gf_theta_static((64, 64, 64, 130), lib.GF_FP32, lib.GF_LANDAU, 12, 256, 256, stream=0)
+    assert err.value.code == lib.GF_EINVAL
+    assert "133120" in str(err.value) and "131072" in str(err.value)
+    for dims in [(3, 4, 4, 4), (4, 4, 4, 0)]:
+        with pytest.raises(lib.GFError) as err:
+            lib.gf_theta_static(dims, lib.GF_FP64, lib.GF_LANDAU, 18, 256, 256, stream=0)
+        assert err.value.code == lib.GF_EINVAL
