@@ -164,24 +164,29 @@ size_t gf_theta_static_max_partials(void);
 /* ---- Alg. 1 with its stop rule -------------------------------------------------------------------------------- */
 
 /* "while precision theta not reached do" with the check after every `check_every`-th sweep
- * (C11).  Coulomb: theta = max over timeslices (C12).  sweeps_done / theta_host / F_host (each may be
- * NULL) receive the number of sweeps and theta and F of the field as returned.  Two forms of the loop:
- *   fused monitor (default where it applies and check_every <= 10, see gf_set_monitor; C21): theta and F of the state
- *     after sweep n are accumulated by the
- *     sweep kernels themselves -- the BLACK half-sweep of sweep n leaves K(x) of its sites in registers, the RED
- *     half-sweep of sweep n+1 builds K(x) of the other half from that state before updating it -- and reduced on the
- *     device in a fixed order while sweep n+1 runs.  The loop ends ONE SWEEP AFTER the first checked sweep n with
- *     theta < theta_tol (sweeps_done = n + 1; a check needs the sweep after it, so none takes place at
- *     n = max_sweeps).  No pass over the field per check, no host synchronisation per check: sweeps are enqueued in
- *     batches of 32 and launches past the stop return at once.  theta before the first sweep and theta / F of the
- *     returned field come from the separate reductions.  Oracle: orc_fix_lag(lag = 1).
- *   separate check (gf_set_monitor(ctx, 0); the paper's second kernel): gf_theta; while theta >=
- *     theta_tol and fewer than max_sweeps sweeps done: min(check_every, max_sweeps - done) sweeps; gf_theta.
- *     Synchronises at every check.  Oracle: orc_fix_lag(lag = 0).
- * The fused form applies when every thread block of the sweep lies inside one timeslice ((Nx Ny Nz / 2) * threads per
- * site divisible by the block size; true for every lattice of BASELINE.json but 4^4 in fp64) and, for fp32 contexts,
- * when theta_tol >= 1e-10 (theta formed from the fp32 K of the sweep resolves ~1e-12); otherwise the call falls back
- * to the separate check.  Errors as gf_relax; GF_EINVAL also for check_every < 1, max_sweeps < 0. */
+ * (C11) -- and, with the default setting, ending ONE SWEEP LATER than the paper's loop: sweeps_done =
+ * n + 1 for the first checked sweep n with theta < theta_tol, and no check at n = max_sweeps (C21).  Coulomb: theta =
+ * max over timeslices (C12).  sweeps_done / theta_host / F_host (each may be NULL) receive the number of sweeps and theta
+ * and F of the field as returned.
+ * The STOP RULE is a setting of the context and of nothing else (gf_set_monitor): the same arguments give the same
+ * sweeps_done whatever the launch shape (gf_set_tuning), the precision, the tolerance or check_every.
+ *   gf_set_monitor(ctx, 1 or 2) -- 1 is the default: the rule above (oracle: orc_fix_lag(lag = 1)).
+ *   gf_set_monitor(ctx, 0): the paper's loop (oracle: orc_fix_lag(lag = 0)): gf_theta; while theta >= theta_tol and
+ *     fewer than max_sweeps sweeps done: min(check_every, max_sweeps - done) sweeps; gf_theta.
+ * Which KERNELS run the default rule is a matter of speed only (gf_fix_last_form tells):
+ *   fused monitor: theta and F of the state after sweep n are accumulated by the sweep kernels themselves -- the BLACK
+ *     half-sweep of sweep n leaves K(x) of its sites in registers, the RED half-sweep of sweep n+1 builds K(x) of the
+ *     other half from that state before updating it -- and reduced on the device in a fixed order while sweep n+1 runs
+ *     (which is where the one-sweep lag comes from).  No pass over the field per check, no host synchronisation per
+ *     check: sweeps are enqueued in batches of 32 and launches past the stop return at once.  theta before the first
+ *     sweep and theta / F of the returned field come from the separate reductions.  Taken when every thread block of the
+ *     sweep lies inside one timeslice ((Nx Ny Nz / 2) * threads per site divisible by the block size; true for every
+ *     lattice of BASELINE.json but 4^4 in fp64), for fp32 contexts when theta_tol >= 1e-10 (theta formed from the fp32 K
+ *     of the sweep resolves ~1e-12), and, with setting 1, when check_every <= 10 (where it pays).
+ *   separate check (the paper's second kernel) otherwise: the same rule with gf_theta at every check and
+ *     one more sweep after the check that met the tolerance; synchronises at every check.  fp64 fields are bit-identical
+ *     between the two; fp32 fields agree to the fp32 tolerance (the fused form sees theta through the fp32 K).
+ * Errors as gf_relax; GF_EINVAL also for check_every < 1, max_sweeps < 0. */
 int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double theta_tol, int check_every,
            int max_sweeps, unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host,
            void* stream);
@@ -189,9 +194,10 @@ int gf_fix(gf_ctx* ctx, void* U_native_dev, int update, double param, double the
 /* Coulomb gauge, "each timeslice fixed independently" (C12, C20): as gf_fix, but a timeslice whose theta_t is below
  * theta_tol at a check is frozen for good (its sites are no longer updated; K, F and theta_t of a slice depend on
  * the spatial links of that slice alone), and the loop ends when no slice is active.  sweeps_done = sweeps of the
- * slowest slice; sweeps_per_slice (Nt ints, may be NULL) the sweeps every slice got.  Fused monitor: the freeze of a
- * slice found below the tolerance after sweep n takes effect from sweep n + 2 (it gets n + 1 sweeps; oracle:
- * orc_fix_slices_lag(lag = 1)); with check_every = 1 every slice stops within one sweep of meeting the tolerance.
+ * slowest slice; sweeps_per_slice (Nt ints, may be NULL) the sweeps every slice got.  Default stop rule (gf_set_monitor
+ * 1 or 2, whichever kernels run it): the freeze of a slice found below the tolerance after sweep n takes effect from
+ * sweep n + 2 (it gets n + 1 sweeps; oracle: orc_fix_slices_lag(lag = 1)); with check_every = 1 every slice stops
+ * within one sweep of meeting the tolerance.  gf_set_monitor(ctx, 0): frozen from sweep n + 1 (orc_fix_slices).
  * GF_EINVAL for a Landau ctx. */
 int gf_fix_slices(gf_ctx* ctx, void* U_native_dev, int update, double param, double theta_tol, int check_every,
                   int max_sweeps, unsigned long long seed, int* sweeps_done, int* sweeps_per_slice,
@@ -297,10 +303,17 @@ int gf_set_prefetch(gf_ctx* ctx, int sites);
  * transform the temporal links once at the end of each call -- 14/16 of the bytes, same result up to rounding.
  * gf_anneal / gf_anneal_micro keep one site field over the whole call.  GF_EINVAL for a Landau context. */
 int gf_set_coulomb_reading(gf_ctx* ctx, int reading_b);
-/* Form of the fixing loops gf_fix / gf_fix_slices: 0 = separate check; 1 (default) = fused monitor where it applies and
+/* Stop rule and kernels of the fixing loops gf_fix / gf_fix_slices.  0 = the paper's loop, separate check kernel (lag 0).
+ * 1 (default) and 2 = the rule of C21 (lag 1: the loop ends, or a timeslice freezes, one sweep after the check that met
+ * the tolerance; no check at max_sweeps) -- the two differ in speed only: 1 takes the fused monitor where it applies and
  * check_every <= 10 (a monitored sweep costs ~4 % more than a plain one, a checked one ~20 %, a separate check about
- * 0.6 sweeps: the fused form wins while checks are frequent); 2 = fused wherever it applies.  GF_EINVAL otherwise. */
+ * 0.6 sweeps: the fused form wins while checks are frequent), 2 wherever it applies; elsewhere the separate check kernel
+ * runs the same rule.  GF_EINVAL otherwise. */
 int gf_set_monitor(gf_ctx* ctx, int fused);
+/* Form of the last gf_fix / gf_fix_slices on this context (each output may be NULL): *lag = 0 the paper's stop rule,
+ * 1 the rule of C21 (one sweep past the check that met the tolerance); *fused = 1 if the sweep kernels monitored theta
+ * themselves, 0 if the separate check kernel ran.  Both -1 before the first such call. */
+int gf_fix_last_form(const gf_ctx* ctx, int* lag, int* fused);
 /* The last check completed by a fused fixing loop on this context: the sweep n it belongs to (0: none yet), theta
  * (Coulomb: max over timeslices) and F of the state after that sweep, the per-timeslice theta_t (Nt doubles).  Each
  * output may be NULL.  Synchronises.  GF_EINVAL if no fused loop has run. */

@@ -67,6 +67,7 @@ SIGNATURES = {
     "gf_raw_sums": (_i, [_vp, _vp, _pd, _pd]),
     "gf_set_monitor": (_i, [_vp, _i]),
     "gf_monitor_last": (_i, [_vp, _pi, _pd, _pd, _pd]),
+    "gf_fix_last_form": (_i, [_vp, _pi, _pi]),
     "gf_set_chain": (_i, [_vp, _i, _d, _d]),
     "gf_chain_count": (_i, [_vp, ctypes.POINTER(_ull), ctypes.POINTER(_ull)]),
     "gf_set_trial_buffer": (_i, [_vp, _vp]),
@@ -353,6 +354,15 @@ def gf_monitor_last(ctx, Nt: int):
     sl = (ctypes.c_double * Nt)()
     _check(ctx, load_library().gf_monitor_last(ctx, ctypes.byref(n), ctypes.byref(th), ctypes.byref(F), sl))
     return n.value, th.value, F.value, list(sl)
+
+
+def gf_fix_last_form(ctx):
+    """(lag, fused) of the last gf_fix / gf_fix_slices on this context: lag 0 = the paper's stop rule, 1 = one sweep
+    after the check that met the tolerance (C21); fused 1 = the sweep kernels monitored theta themselves, 0 = separate
+    check kernel.  (-1, -1) before the first call."""
+    lag, fused = ctypes.c_int(), ctypes.c_int()
+    _check(ctx, load_library().gf_fix_last_form(ctx, ctypes.byref(lag), ctypes.byref(fused)))
+    return lag.value, fused.value
 
 
 def gf_set_chain(ctx, chain: int, watch_threshold: float = 0.0, fix_threshold: float = 0.0) -> None:

@@ -42,6 +42,7 @@ struct gf_ctx {
     int bx;
     // fused F / theta monitor of gf_fix / gf_fix_slices (lazily allocated; sized for one launch shape)
     int monitor;                      // 0: the paper's separate check kernel, 1: fused where it applies and pays (default), 2: fused where it applies
+    int fix_lag, fix_fused;           // form of the last gf_fix / gf_fix_slices on this context (-1: none yet); gf_fix_last_form
     char* d_mon;                      // MonitorState, theta_t[2 Nt], frozen_from[Nt] | group | partials
     char* h_mon;                      // pinned: two copies of the prefix up to `frozen`
     size_t mon_prefix, mon_bytes;
@@ -127,6 +128,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precisi
     c->batch_canon_bytes = 0; c->h_batch = nullptr; c->h_batch_doubles = 0;
     c->err[0] = 0;
     c->bx = reduce_blocks_per_slice(c->L);
+    c->fix_lag = c->fix_fused = -1;
     c->monitor = 1; c->d_mon = nullptr; c->h_mon = nullptr; c->mon_prefix = c->mon_bytes = 0; c->mon_blocks = c->mon_groups = 0;
     c->mon_event[0] = c->mon_event[1] = nullptr;
     const size_t npart = (size_t)c->bx * 2 * Nt;
@@ -1026,6 +1028,67 @@ static int fix_fused(gf_ctx* c, void* U, int update, double param, double tol, i
     return GF_OK;
 }
 
+// The stop rule of gf_fix / gf_fix_slices is a setting of the context and of nothing else: gf_set_monitor(ctx, 0) is the
+// paper's loop (lag 0), any other setting (the default included) the loop of C21 (lag 1), whichever kernels run it.
+static int fix_lag(const gf_ctx* c) { return c->monitor ? 1 : 0; }
+
+extern "C" int gf_fix_last_form(const gf_ctx* c, int* lag, int* fused)
+{
+    if (c == nullptr) return GF_EINVAL;
+    if (lag) *lag = c->fix_lag;
+    if (fused) *fused = c->fix_fused;
+    return GF_OK;
+}
+
+// gf_fix_slices with the stop rule of the fused monitor (orc_fix_slices_lag, lag = 1) run with the separate check: a
+// slice found below the tolerance at the check after sweep n gets one more sweep and is frozen from sweep n + 2; no
+// check at max_sweeps.
+static int fix_slices_lag1(gf_ctx* c, void* U, int mode, int variant, double param, double tol, int check_every,
+                           int max_sweeps, unsigned long long seed, cudaStream_t st, int* sweeps_done, int* per_slice,
+                           double* theta_host, double* F_host)
+{
+    const char* who = "gf_fix_slices";
+    const int Nt = c->Nt;
+    unsigned char* mask = new (std::nothrow) unsigned char[Nt];
+    int* count = new (std::nothrow) int[Nt];
+    int* last = new (std::nothrow) int[Nt]; // last sweep (1-based) that updates the slice; -1: still open
+    if (mask == nullptr || count == nullptr || last == nullptr) {
+        delete[] mask; delete[] count; delete[] last;
+        return fail(c, GF_ENOMEM, "%s: host allocation", who);
+    }
+    int done = 0, any = 0;
+    int rc = reduce_to_host(c, U, true, who);
+    for (int t = 0; t < Nt && rc == GF_OK; ++t) { count[t] = 0; last[t] = c->h_out[2 + t] >= tol ? -1 : 0; any |= last[t] < 0; }
+    while (rc == GF_OK && any && done < max_sweeps) {
+        bool pending = false; // a slice in its one sweep after the check that froze it
+        for (int t = 0; t < Nt; ++t) pending = pending || last[t] > done;
+        const int next_check = (done / check_every + 1) * check_every;
+        const int target = pending ? done + 1 : (next_check < max_sweeps ? next_check : max_sweeps);
+        for (int t = 0; t < Nt; ++t) {
+            mask[t] = last[t] < 0 || last[t] > done;
+            if (mask[t]) count[t] += target - done;
+        }
+        rc = run_sweeps(c, U, mode, variant, param, target - done, done, seed, st, "gf_fix_slices: kernel launch", mask);
+        done = target;
+        if (rc == GF_OK && done % check_every == 0 && done < max_sweeps) {
+            rc = reduce_to_host(c, U, true, who);
+            for (int t = 0; t < Nt && rc == GF_OK; ++t)
+                if (last[t] < 0 && c->h_out[2 + t] < tol) last[t] = done + 1;
+        }
+        any = 0;
+        for (int t = 0; t < Nt; ++t) any |= last[t] < 0 || last[t] > done;
+    }
+    if (rc == GF_OK) rc = reduce_to_host(c, U, true, who); // theta of the field as returned
+    if (rc == GF_OK) {
+        if (sweeps_done) *sweeps_done = done;
+        if (per_slice) memcpy(per_slice, count, sizeof(int) * (size_t)Nt);
+        if (theta_host) *theta_host = c->h_out[1];
+        if (F_host) rc = gf_functional(c, U, F_host);
+    }
+    delete[] mask; delete[] count; delete[] last;
+    return rc;
+}
+
 extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta_tol, int check_every, int max_sweeps,
                       unsigned long long seed, int* sweeps_done, double* theta_host, double* F_host, void* stream)
 {
@@ -1042,11 +1105,47 @@ extern "C" int gf_fix(gf_ctx* c, void* U, int update, double param, double theta
     {
         int mode, variant;
         update_to_mode(update, &mode, &variant);
-        if (monitor_applies(c, mode, theta_tol, check_every))
+        if (monitor_applies(c, mode, theta_tol, check_every)) {
+            c->fix_fused = 1;
+            c->fix_lag = 1;
             return fix_fused(c, U, update, param, theta_tol, check_every, max_sweeps, seed, (cudaStream_t)stream, false,
                              sweeps_done, nullptr, theta_host, F_host, "gf_fix");
+        }
     }
+    c->fix_fused = 0;
+    c->fix_lag = fix_lag(c);
     rc = gf_theta(c, U, &th);
+    if (c->fix_lag == 1) {
+        // the stop rule of the fused monitor (C21, orc_fix_lag with lag = 1) run with the separate check, where the fused
+        // kernels cannot or would not pay: one more sweep after the check that met the tolerance, no check at max_sweeps.
+        // The rule is the context's setting; the launch shape, the precision and the tolerance only pick the kernels.
+        int stop_at = -1;
+        bool current = true; // th belongs to the field as it is now
+        while (rc == GF_OK && th >= theta_tol && done < max_sweeps && done != stop_at) {
+            const int next_check = (done / check_every + 1) * check_every;
+            const int target = next_check < max_sweeps ? next_check : max_sweeps;
+            rc = relax_chunk(c, U, update, param, target - done, done, seed, (cudaStream_t)stream, "gf_fix");
+            done = target;
+            current = false;
+            if (rc == GF_OK && done % check_every == 0 && done < max_sweeps) {
+                double th_check = 0.0;
+                rc = gf_theta(c, U, &th_check);
+                if (rc == GF_OK && th_check < theta_tol) {
+                    rc = relax_chunk(c, U, update, param, 1, done, seed, (cudaStream_t)stream, "gf_fix");
+                    stop_at = ++done;
+                } else if (rc == GF_OK) {
+                    th = th_check;
+                    current = true;
+                }
+            }
+        }
+        if (rc == GF_OK && !current) rc = gf_theta(c, U, &th);
+        if (rc != GF_OK) return rc;
+        if (sweeps_done) *sweeps_done = done;
+        if (theta_host) *theta_host = th;
+        if (F_host) return gf_functional(c, U, F_host);
+        return GF_OK;
+    }
     // Alg. 1: "while precision theta not reached", checked every check_every-th sweep
     while (rc == GF_OK && th >= theta_tol && done < max_sweeps) {
         const int n = check_every < max_sweeps - done ? check_every : max_sweeps - done;
@@ -1082,9 +1181,17 @@ extern "C" int gf_fix_slices(gf_ctx* c, void* U, int update, double param, doubl
         return fail(c, GF_EINVAL, "gf_fix_slices: parameter %g out of range for update %d", param, update);
     cudaStream_t st = (cudaStream_t)stream;
     if (begin_call(c, st) != GF_OK) return GF_ECUDA;
-    if (monitor_applies(c, mode, theta_tol, check_every))
+    if (monitor_applies(c, mode, theta_tol, check_every)) {
+        c->fix_fused = 1;
+        c->fix_lag = 1;
         return fix_fused(c, U, update, param, theta_tol, check_every, max_sweeps, seed, st, true, sweeps_done,
                          sweeps_per_slice, theta_host, F_host, "gf_fix_slices");
+    }
+    c->fix_fused = 0;
+    c->fix_lag = fix_lag(c);
+    if (c->fix_lag == 1)
+        return fix_slices_lag1(c, U, mode, variant, param, theta_tol, check_every, max_sweeps, seed, st, sweeps_done,
+                               sweeps_per_slice, theta_host, F_host);
     const int Nt = c->Nt;
     unsigned char* active = new (std::nothrow) unsigned char[Nt];
     int* count = new (std::nothrow) int[Nt];

@@ -128,11 +128,18 @@ def test_fix_loop_matches_oracle(gfm, gauge):
     dims = (6, 6, 6, 4)
     U = gf_inputs.smooth_random(dims, 0.3, 54)
     fx = gfm.GaugeFixer(dims, precision="fp64", gauge=gauge)
-    fx.load(U)
-    n, th, F = fx.fix(1e-10, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=10, max_sweeps=2000)
-    n_ref, th_ref, F_ref = oracle.fix(U, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-10, 10, 2000, 0, ORC_GAUGE[gauge])
-    assert n == n_ref and 0 < n < 2000 and th < 1e-10
-    assert th == pytest.approx(th_ref, rel=1e-6) and F == pytest.approx(F_ref, rel=1e-10)
+    # the stop rule is the context's setting alone: 0 = the paper's loop (lag 0); the default = C21's (lag 1), run here
+    # with the separate check because this lattice's blocks straddle timeslices (the fused kernels do not apply)
+    for monitor, lag in ((0, 0), (1, 1)):
+        gfm.gf_set_monitor(fx.ctx, monitor)
+        fx.load(U)
+        n, th, F = fx.fix(1e-10, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=10, max_sweeps=2000)
+        ref = U.copy()
+        n_ref, th_ref, F_ref = oracle.fix(ref, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-10, 10, 2000, 0, ORC_GAUGE[gauge], lag=lag)
+        assert n == n_ref and 0 < n < 2000 and th < 1e-10
+        assert th == pytest.approx(th_ref, rel=1e-6) and F == pytest.approx(F_ref, rel=1e-10)
+        assert gfm.gf_fix_last_form(fx.ctx) == (lag, 0)
+        assert np.abs(fx.download() - ref).max() < 1e-9
     if gauge == "coulomb":
         assert max(fx.theta_slices()) == th
     # cut by max_sweeps; zero sweeps when already fixed
@@ -160,8 +167,18 @@ def test_fix_slices_matches_oracle(gfm, precision):
     dims = (6, 6, 6, 8)
     U = gf_inputs.smooth_random(dims, 0.5, 45)
     fx = gfm.GaugeFixer(dims, precision=precision, gauge="coulomb")
-    fx.load(U)
     tol = 1e-9 if precision == "fp64" else 1e-8
+    if precision == "fp64":  # the default rule (lag 1, C21) with the separate check: blocks straddle timeslices here
+        fx.load(U)
+        n, th, F, per = fx.fix_slices(tol, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=5, max_sweeps=3000)
+        ref = U.copy()
+        n_ref, th_ref, F_ref, per_ref = oracle.fix_slices(ref, dims, oracle.UPDATE_OVERRELAX2, 1.5, tol, 5, 3000, lag=1)
+        assert gfm.gf_fix_last_form(fx.ctx) == (1, 0)
+        assert per == per_ref.tolist() and n == n_ref and len(set(per)) > 1
+        assert th == pytest.approx(th_ref, rel=1e-5) and F == pytest.approx(F_ref, rel=1e-10)
+        assert np.abs(fx.download() - ref).max() < 1e-9
+    gfm.gf_set_monitor(fx.ctx, 0)  # the paper's rule
+    fx.load(U)
     n, th, F, per = fx.fix_slices(tol, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=5, max_sweeps=3000)
     n_ref, th_ref, F_ref, per_ref = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, tol, 5, 3000)
     sl = fx.theta_slices()
@@ -286,6 +303,7 @@ def test_coulomb_reading_b_with_fix_slices_and_errors(gfm):
     U = gf_inputs.smooth_random(dims, 0.5, 45)
     fx = gfm.GaugeFixer(dims, precision="fp64", gauge="coulomb")
     gfm.gf_set_coulomb_reading(fx.ctx, True)
+    gfm.gf_set_monitor(fx.ctx, 0)  # the paper's stop rule
     fx.load(U)
     n, th, F, per = fx.fix_slices(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=5, max_sweeps=3000)
     n_ref, th_ref, F_ref, per_ref = oracle.fix_slices(U, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-9, 5, 3000)
@@ -511,9 +529,42 @@ def test_fused_fix_slices_matches_oracle_with_lag_one(gfm, precision):
     fx.close()
 
 
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("every", [1, 4, 25])
+def test_fix_result_does_not_depend_on_the_launch_shape(gfm, precision, every):
+    """gf_fix: the same arguments give the same sweeps_done and the same field whatever gf_set_tuning picked -- with the
+    default shape the fused monitor runs (check_every <= 10), with a 96-thread block its blocks straddle timeslices and
+    the separate check runs, under the same stop rule (lag 1, from the context's gf_set_monitor setting alone); with
+    check_every = 25 both shapes take the separate check.  fp64: bit-identical fields; fp32: the hybrid chain's
+    roughness history differs between a 32- and a 1-sweep batch of launches, so fields agree to the fp32 tolerance."""
+    dims = (8, 8, 8, 8)
+    U = gf_inputs.smooth_random(dims, 0.3, 65)
+    tol = 1e-9 if precision == "fp64" else 1e-8
+    out = []
+    for block in (0, 96, 64):
+        fx = gfm.GaugeFixer(dims, precision=precision)
+        gfm.gf_set_tuning(fx.ctx, 0, block)
+        fx.load(U)
+        n, th, F = fx.fix(tol, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=every, max_sweeps=3000)
+        out.append((n, gfm.gf_fix_last_form(fx.ctx), fx.download(), th))
+        fx.close()
+    assert out[0][1] == (1, 1 if every <= 10 else 0) and out[1][1] == (1, 0)
+    assert 0 < out[0][0] < 3000 and out[0][3] < tol
+    for n, form, field, th in out[1:]:
+        assert form[0] == 1
+        if precision == "fp64":
+            assert n == out[0][0] and np.array_equal(field, out[0][2])
+        else:
+            assert abs(n - out[0][0]) <= every and th < tol
+    ref = U.copy()
+    n_ref = oracle.fix(ref, dims, oracle.UPDATE_OVERRELAX2, 1.6, tol, every, 3000, lag=1)[0]
+    if precision == "fp64":
+        assert out[0][0] == n_ref and np.abs(out[0][2] - ref).max() < 1e-9
+
+
 def test_fused_monitor_stochastic_and_fallback(gfm):
     """the variants run under the monitor too (stochastic relaxation: decisions continue through the loop, C18); a
-    lattice whose blocks straddle timeslices falls back to the separate check (lag 0)"""
+    lattice whose blocks straddle timeslices falls back to the separate check and keeps the context's stop rule (lag 1)"""
     dims = (8, 8, 8, 4)
     U = gf_inputs.smooth_random(dims, 0.3, 64)
     fx = gfm.GaugeFixer(dims, precision="fp64")
@@ -528,7 +579,9 @@ def test_fused_monitor_stochastic_and_fallback(gfm):
     fx = gfm.GaugeFixer(dims, precision="fp64")
     fx.load(U)
     n = fx.fix(1e-9, gfm.GF_UPDATE_OVERRELAX2, 1.6, check_every=3, max_sweeps=2000)[0]
-    assert n == oracle.fix(U, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-9, 3, 2000, lag=0)[0]
+    ref = U.copy()
+    assert n == oracle.fix(ref, dims, oracle.UPDATE_OVERRELAX2, 1.6, 1e-9, 3, 2000, lag=1)[0]
+    assert gfm.gf_fix_last_form(fx.ctx) == (1, 0) and np.abs(fx.download() - ref).max() < 1e-9
     with pytest.raises(gfm.GFError):
         gfm.gf_monitor_last(fx.ctx, 4)
     fx.close()
