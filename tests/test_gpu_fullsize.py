@@ -85,6 +85,46 @@ def test_32x4_fp32_every_link_more_seeds(gfm, seed, omega):
 
 
 @pytest.fixture(scope="module")
+def advanced32(field32):
+    """configs[2] advanced by the ORACLE by 10 and by 60 sweeps (the states the timed sweeps of bench.py work on are
+    these, not the random-gauge start), each rounded to fp32 -- what an fp32 context stores -- with the oracle's next
+    sweep from that rounded state"""
+    dims = (32, 32, 32, 32)
+    U = field32.copy()
+    out, done = {}, 0
+    for k in (10, 60):
+        oracle.overrelax(U, dims, 1.7, k - done)
+        done = k
+        start = U.astype(np.complex64).astype(np.complex128)
+        nxt = start.copy()
+        oracle.overrelax(nxt, dims, 1.7, 1)
+        out[k] = (start, nxt)
+    return out
+
+
+@pytest.mark.parametrize("k", [10, 60])
+@pytest.mark.parametrize("R", [18, 12])
+def test_32x4_fp32_steady_state_chain_every_link(gfm, advanced32, R, k):
+    """The fp32 per-link bound on the kernel path that bench.py spends its time in.  The first sweep of every API call
+    runs the site chain in double (gf_set_chain, hybrid default), so the one-sweep checks above never see the fp32 chain
+    at full size.  Here the field is the oracle's state after k sweeps and the sweep is run as sweep 1 of a call
+    (gf_begin_sweeps + gf_relax_half: no forced double chain, roughness flags clear): gf_chain_count must show that no
+    launch took the double chain, and every link must be within 5e-5 of the oracle's sweep from the same input."""
+    dims = (32, 32, 32, 32)
+    start, nxt = advanced32[k]
+    fx = gfm.GaugeFixer(dims, precision="fp32", reals_per_link=R)  # default chain, default launch shape
+    fx.load(start)
+    before = gfm.gf_chain_count(fx.ctx)[0]
+    gfm.gf_begin_sweeps(fx.ctx)
+    for parity in (0, 1):
+        gfm.gf_relax_half(fx.ctx, fx.U, gfm.GF_UPDATE_OVERRELAX2, 1.7, parity, 1, 0, 0, dims[3])
+    assert gfm.gf_chain_count(fx.ctx)[0] == before  # both half-sweeps ran the fp32 chain
+    err = np.abs(fx.download() - nxt).max()
+    fx.close()
+    assert err <= TOL_LINK["fp32"], (R, k, err)
+
+
+@pytest.fixture(scope="module")
 def oracle32_500(field32):
     """the headline config run to its end by the oracle: 500 sweeps at omega = 1.7 (about 40 s on 16 cores)"""
     dims = (32, 32, 32, 32)
