@@ -925,6 +925,14 @@ static int fix_fused(gf_ctx* c, void* U, int update, double param, double tol, i
     hs->any_active = active;
     hs->stop_sweep = -1;
     hs->stop_from = INT_MAX;
+    if (slices && active > 0 && active < Nt) {
+        // slices frozen before the first sweep: no sweep will ever deliver their share of F (the duty keeps a frozen
+        // slice's last values), so it is seeded here from the separate reduction
+        if ((rc = reduce_to_host(c, U, false, who)) != GF_OK) return rc;
+        const double raw = 3.0 * (coulomb ? 3.0 : 4.0) * 2.0 * (double)c->Hs; // undoes the per-slice normalisation
+        for (int t = 0; t < Nt; ++t)
+            if (h_from[t] != INT_MAX) h_theta_t[Nt + t] = c->h_out[2 + t] * raw;
+    }
     const bool fixed_already = slices ? active == 0 : hs->theta < tol;
     int done = 0;
     if (!fixed_already && max_sweeps > 0) {

@@ -529,6 +529,28 @@ def test_fused_fix_slices_matches_oracle_with_lag_one(gfm, precision):
     fx.close()
 
 
+def test_fused_monitor_F_counts_slices_frozen_before_the_first_sweep(gfm):
+    """gf_monitor_last after gf_fix_slices on a field with one timeslice already fixed at the start (its spatial links
+    are unit matrices: theta_t = 0): that slice is never swept, and the monitor's F must still contain its share"""
+    dims = (8, 8, 8, 6)
+    Vs = dims[0] * dims[1] * dims[2]
+    U = gf_inputs.smooth_random(dims, 0.5, 66)
+    U[2 * Vs:3 * Vs, :3] = np.eye(3)  # timeslice t = 2, mu = x, y, z
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge="coulomb")
+    fx.load(U)
+    assert fx.theta_slices()[2] == 0.0
+    n, th, F, per = fx.fix_slices(1e-30, gfm.GF_UPDATE_OVERRELAX2, 1.5, check_every=2, max_sweeps=6)
+    assert gfm.gf_fix_last_form(fx.ctx) == (1, 1) and n == 6 and per == [6, 6, 0, 6, 6, 6]
+    k, th_k, F_k, th_t = gfm.gf_monitor_last(fx.ctx, dims[3])
+    assert k == 4  # checks after sweeps 2 and 4; none at the last allowed sweep
+    ref = U.copy()
+    oracle.fix_slices(ref, dims, oracle.UPDATE_OVERRELAX2, 1.5, 1e-30, 2, 4, lag=1)
+    assert F_k == pytest.approx(oracle.functional(ref, dims, oracle.COULOMB), rel=1e-10)
+    np.testing.assert_allclose(th_t, oracle.theta_slices(ref, dims, oracle.COULOMB), rtol=1e-6, atol=1e-30)
+    assert th_t[2] == 0.0 and th_k == pytest.approx(oracle.theta(ref, dims, oracle.COULOMB), rel=1e-6)
+    fx.close()
+
+
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 @pytest.mark.parametrize("every", [1, 4, 25])
 def test_fix_result_does_not_depend_on_the_launch_shape(gfm, precision, every):
