@@ -336,9 +336,13 @@ int gf_monitor_last(gf_ctx* ctx, int* check_sweep, double* theta_host, double* F
  *   products; one rounding at the store) where the projected block has |k| below fix_threshold (default 0.15) in one of
  *   its three steps, where an accept test fell inside the SFU error band of its threshold, or where (i) is still too
  *   coarse -- 8e-5 of the sites at T = 1.4, none below T ~ 0.1.  Accept decisions: 1e-7 of the draws differ from an fp64
- *   evaluation; links: all within 5e-5 below T ~ 0.5, about 1e-6 of the sites of a 7 M-site lattice miss it at T = 1.4,
- *   where alpha = |k|/T inherits the fp32 rounding of K.  chain = 1: the double chain at every site (every link within
- *   5e-5; about -17 %).  chain = 0: plain fp32, no tiers.
+ *   evaluation.  Links, one half-sweep at a time against an fp64 evaluation of the same stored input: all within 5e-5
+ *   at every temperature (measured max 3e-5 on 7 M sites at T = 1.4).  Over a whole step the BLACK half-sweep reads RED
+ *   links that carry their fp32 storage rounding and a site with a small block amplifies it by 1/|k|: against an fp64
+ *   run of the whole step about 7e-6 of the sites of a 7 M-site lattice end beyond 5e-5 at T = 1.4 (max 1.3e-4), none
+ *   below T ~ 0.5.  chain = 1: the double chain at every site (about -17 %): the same per-half-sweep bound; it cannot
+ *   remove the whole-step tail, which sits in the stored input (measured 4e-6 of the sites, max 7.6e-5) -- only an fp64
+ *   context does.  chain = 0: plain fp32, no tiers.
  * A threshold of 0 keeps the current value.  Ignored by fp64 contexts.  GF_EINVAL: chain outside 0..2, a threshold < 0
  * or > 1e3.
  * gf_chain_count (each output may be NULL; synchronises the stream): half-sweep launches that ran the double chain and

@@ -295,6 +295,92 @@ def test_config5_48x3x64_coulomb_anneal_census(gfm, T, chain):
     torch.cuda.empty_cache()
 
 
+_HALF_REF = {}  # one temperature at a time: (input, RED reference, its trials, RED reference rounded, BLACK reference, its trials)
+
+
+def _half_sweep_reference(T):
+    """oracle side of test_config5_48x3x64_coulomb_anneal_half_sweeps, computed once per temperature: the fp32-rounded
+    48^3x64 input; the oracle's RED half-sweep of it; that result rounded to fp32 ON THE HOST; the oracle's BLACK
+    half-sweep continued from the rounded field"""
+    if T not in _HALF_REF:
+        _HALF_REF.clear()
+        gdims, dims = (24, 24, 24, 32), (48, 48, 48, 64)
+        V = int(np.prod(dims))
+        Nx, Ny, Nz, Nt = gdims
+        U = gf_inputs.smooth_random(gdims, 0.5, 5)
+        start = np.tile(U.reshape(Nt, Nz, Ny, Nx, 4, 3, 3), (2, 2, 2, 2, 1, 1, 1)).reshape(V, 4, 3, 3)
+        start = start.astype(np.complex64).astype(np.complex128)
+        red_ref = start.copy()
+        red_trials = np.zeros((V, 3), dtype=np.int32)
+        oracle.heatbath_half(red_ref, dims, T, 7, 0, 0, oracle.COULOMB, trials=red_trials)
+        mid = red_ref.astype(np.complex64).astype(np.complex128)
+        black_ref = mid.copy()
+        black_trials = np.zeros((V, 3), dtype=np.int32)
+        oracle.heatbath_half(black_ref, dims, T, 7, 0, 1, oracle.COULOMB, trials=black_trials)
+        _HALF_REF[T] = (start, red_ref, red_trials, mid, black_ref, black_trials)
+    return _HALF_REF[T]
+
+
+def _one_half_sweep(gfm, dims, chain, T, parity, field, ref, ref_trials):
+    """one heatbath half-sweep of `parity` on a FRESH context from `field`; returns (flipped draws, draws, per-link error
+    of the links whose updating site took the oracle's decisions)"""
+    import torch
+
+    V = int(np.prod(dims))
+    fx = gfm.GaugeFixer(dims, precision="fp32", gauge="coulomb")
+    gfm.gf_set_chain(fx.ctx, chain)
+    gfm.gf_set_coulomb_reading(fx.ctx, False)  # single half-sweeps run reading A
+    trials = torch.zeros(V * 3, dtype=torch.int32, device="cuda")
+    gfm.gf_set_trial_buffer(fx.ctx, trials)
+    fx.load(field)
+    gfm.gf_begin_sweeps(fx.ctx)
+    gfm.gf_anneal_half(fx.ctx, fx.U, T, parity, 0, 7, 0, dims[3])
+    got = fx.download()
+    got_trials = trials.cpu().numpy().reshape(V, 3)
+    fx.close()
+    del trials
+    torch.cuda.empty_cache()
+    s = np.arange(V)
+    c = [s % 48, (s // 48) % 48, (s // 48**2) % 48, s // 48**3]
+    active = ((c[0] + c[1] + c[2] + c[3]) & 1) == parity
+    assert got_trials[active].min() >= 1 and got_trials[~active].max() == 0
+    flipped = active & (got_trials != ref_trials).any(axis=1)
+    draws_flipped = int((got_trials[active] != ref_trials[active]).sum())
+    err = np.abs(got - ref).max(axis=(2, 3))  # (V, 4): link mu stored at site s
+    del got
+    # a flipped site f updated U_mu(f) and U_mu(f - mu): those links are not judged
+    stride = [1, 48, 48**2, 48**3]
+    for f in np.nonzero(flipped)[0]:
+        err[f, :] = 0.0
+        for mu in range(4):
+            x = int(c[mu][f])
+            back = f - stride[mu] if x > 0 else f + (dims[mu] - 1) * stride[mu]
+            err[back, mu] = 0.0
+    return draws_flipped, 3 * int(active.sum()), err
+
+
+@pytest.mark.parametrize("chain", [2, 1])  # gf_set_chain: default tiers, double chain at every site
+@pytest.mark.parametrize("T", [1.4, 0.7, 0.05])
+def test_config5_48x3x64_coulomb_anneal_half_sweeps(gfm, T, chain):
+    """The fp32 annealing sweep judged one half-sweep at a time on the full 48^3x64 lattice, so that the kernel's own
+    error is separated from what a whole step does to the storage rounding of its first half (a BLACK site with a small
+    projected block amplifies the fp32 rounding of the RED links by 1/|k|; no fp32 kernel can remove that).
+    (i) RED half-sweep from the fp32-rounded input against orc_heatbath_half(parity 0) of the same input.
+    (ii) a fresh context loaded with the ORACLE's RED result rounded to fp32 on the host, one BLACK half-sweep, against
+    orc_heatbath_half(parity 1) continued from that same rounded field.
+    In both: at most 1e-5 of the Kennedy-Pendleton trial counts differ (C14), and EVERY link updated by a site whose
+    decisions are the oracle's is within 5e-5 -- the maximum, no quantile, no ceiling above it."""
+    dims = (48, 48, 48, 64)
+    start, red_ref, red_trials, mid, black_ref, black_trials = _half_sweep_reference(T)
+    for name, parity, field, ref, ref_trials in (("RED", 0, start, red_ref, red_trials), ("BLACK", 1, mid, black_ref, black_trials)):
+        flips, draws, err = _one_half_sweep(gfm, dims, chain, T, parity, field, ref, ref_trials)
+        print(f"half-sweep T={T} chain={chain} {name}: {flips} of {draws} draws flipped; links max {err.max():.3e}, "
+              f"above 5e-5: {int((err > 5e-5).sum())}, above 2e-5: {int((err > 2e-5).sum())}")
+        assert flips <= 1e-5 * draws, (name, flips)
+        assert err.max() <= TOL_LINK["fp32"], (name, float(err.max()), int((err > TOL_LINK["fp32"]).sum()))
+        del err
+
+
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_config2_16x3x32_logs_every_100_sweeps(gfm, precision):
     """BASELINE.json configs[1]: 16^3x32, eps 0.3, seed 2, omega 1.7, 1000 sweeps, F and theta logged every 100
