@@ -16,7 +16,8 @@ Workloads (BASELINE.json configs; seeded synthetic fields, recipe in DESIGN.md "
 N > 1 (torchrun): by default every rank runs an independent replica of the workload on its own GPU ("replicas": the
 shape of production gauge fixing, ensembles of configurations; no data-path collective); --shard t runs ONE
 configuration cut into t-slabs over the ranks (paper_1209_4008_b200/slab.py: one face message up and one down per
-half-sweep and slab boundary, strong scaling).  value = site-updates of the whole job / max-over-ranks time.
+half-sweep and slab boundary, strong scaling -- never run on more than one GPU so far: unmeasured).
+value = site-updates of the whole job / max-over-ranks time.
 
 --impl reference times the fp64 CPU oracle (oracle/, as it stands) on the host cores on the same config.
 """
@@ -316,9 +317,19 @@ def time_e2e(gfm, w, hosts, sweeps, steps, warmup):
         gfm.gf_overrelax_host_batch(ctx, hosts, w["omega"], sweeps)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
+    # the same through the single-configuration call (gf_overrelax_host / _f32): nothing overlaps the copies -- the
+    # figure round 1 reported, kept so that the end-to-end numbers of the rounds stay comparable
+    one = gfm.gf_overrelax_host_f32 if hosts[0].element_size() == 4 else gfm.gf_overrelax_host
+    one(ctx, hosts[0], w["omega"], sweeps)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one(ctx, hosts[0], w["omega"], sweeps)
+    torch.cuda.synchronize()
+    dt_single = time.perf_counter() - t0
     gfm.gf_destroy(ctx)
     nbytes = hosts[0].numel() * hosts[0].element_size()
-    return dt, nbytes, nbytes + 16
+    return dt, nbytes, nbytes + 16, dt_single
 
 
 def time_oracle(w, U, sweeps, reps):
@@ -591,13 +602,18 @@ def main():
         hosts = [base.clone().pin_memory() for _ in range(nconf)]
         del base
         e_steps = max(1, min(steps, 3))
-        dt, h2d, d2h = time_e2e(gfm, w, hosts, sweeps, e_steps, 1)
+        dt, h2d, d2h, dt_single = time_e2e(gfm, w, hosts, sweeps, e_steps, 1)
         e2e = {"value": world * nconf * V * sweeps * e_steps / dt, "unit": "site-updates/s", "h2d_bytes_per_step": nconf * h2d,
                "d2h_bytes_per_step": nconf * d2h, "steps": e_steps, "ms_per_step": dt / e_steps * 1e3,
                "configurations_per_step": nconf, "ms_per_configuration": dt / e_steps / nconf * 1e3,
                "call": f"gf_overrelax_host_batch: {nconf} canonical configurations in pinned host memory in, the fixed fields + "
                        "F + theta out; upload of configuration i+1 and download of i-1 overlap the sweeps of i (three slots, "
-                       "three streams); element type = the context's precision"}
+                       "three streams); element type = the context's precision",
+               "single_configuration": {
+                   "value": world * V * sweeps * e_steps / dt_single, "unit": "site-updates/s",
+                   "ms_per_step": dt_single / e_steps * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                   "call": "gf_overrelax_host" + ("_f32" if w["precision"] == "fp32" else "") +
+                           ": ONE configuration per step, copies not overlapped with the sweeps (round 1's e2e figure)"}}
         del hosts
 
     also = []

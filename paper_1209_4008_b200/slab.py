@@ -69,6 +69,36 @@ class LocalRing:
         return max(values.values())
 
 
+class StreamRing(LocalRing):
+    """all slabs live in this process, EACH ON ITS OWN CUDA STREAM (engines with a `.stream`): the copy that stands for a
+    message runs on the receiver's stream behind an event the sender records after packing, so the interior launches of
+    one slab really do overlap the face traffic and the launches of the others, and only the events order them -- what
+    DistRing does across processes.  The sender then waits for the copy before it may reuse its send buffer."""
+
+    def __init__(self, engines: Dict[int, object]):
+        import torch
+
+        super().__init__(len(engines))
+        self.torch = torch
+        self.stream = {r: e.stream for r, e in engines.items()}
+
+    def start(self, msgs: Dict[int, object], direction: int, recv_like: Dict[int, object]):
+        torch = self.torch
+        out = {}
+        for src, buf in msgs.items():
+            dst = (src + direction) % self.n
+            packed = torch.cuda.Event()
+            packed.record(self.stream[src])
+            self.stream[dst].wait_event(packed)
+            with torch.cuda.stream(self.stream[dst]):
+                recv_like[dst].copy_(buf)
+            copied = torch.cuda.Event()
+            copied.record(self.stream[dst])
+            self.stream[src].wait_event(copied)
+            out[dst] = recv_like[dst]
+        return out
+
+
 class DistRing:
     """one slab per rank of an initialised torch.distributed group; messages are point-to-point sends"""
 
@@ -123,12 +153,14 @@ class DistRing:
 # the engine of one slab on the GPU: argument marshalling around the C ABI
 # ---------------------------------------------------------------------------------------------------------
 class GpuSlab:
-    def __init__(self, dims, t_begin: int, t_end: int, precision="fp64", gauge="landau", reals_per_link: int = 18):
+    def __init__(self, dims, t_begin: int, t_end: int, precision="fp64", gauge="landau", reals_per_link: int = 18,
+                 own_stream: bool = False):
         import torch
 
         import paper_1209_4008_b200 as gfm
 
         self.gfm, self.torch = gfm, torch
+        self.stream = torch.cuda.Stream() if own_stream else None  # None: whatever stream is current at each call
         self.dims = tuple(int(d) for d in dims)
         self.t_begin, self.t_end, self.Nt = int(t_begin), int(t_end), int(t_end - t_begin)
         prec = {"fp32": gfm.GF_FP32, "fp64": gfm.GF_FP64}[precision]
@@ -147,42 +179,58 @@ class GpuSlab:
     def new_face(self):
         return self.torch.empty(self.face_bytes, dtype=self.torch.uint8, device="cuda")
 
+    def _on_stream(self):
+        """context manager: the slab's own stream current (a no-op without one)"""
+        import contextlib
+
+        return self.torch.cuda.stream(self.stream) if self.stream is not None else contextlib.nullcontext()
+
     def load(self, U_canon_slab):
         """host numpy complex128 (Nt_local * Vs, 4, 3, 3): the owned slices in the canonical layout"""
         torch = self.torch
         dev = torch.from_numpy(U_canon_slab.view("float64").reshape(-1)).to("cuda")
         assert dev.numel() == self.Nt * self.Vs * 72
-        self.gfm.gf_pack(self.ctx, dev, self.U)
         torch.cuda.current_stream().synchronize()
+        with self._on_stream():
+            self.gfm.gf_pack(self.ctx, dev, self.U)
+            torch.cuda.current_stream().synchronize()
 
     def download(self):
         torch = self.torch
         dev = torch.empty(self.Nt * self.Vs * 72, dtype=torch.float64, device="cuda")
-        self.gfm.gf_unpack(self.ctx, self.U, dev)
+        with self._on_stream():
+            self.gfm.gf_unpack(self.ctx, self.U, dev)
+            torch.cuda.current_stream().synchronize()
         return dev.cpu().numpy().view("complex128").reshape(self.Nt * self.Vs, 4, 3, 3)
 
     # the five methods of an engine
     def pack_face(self, which: int, block_parity: int, buf):
-        self.gfm.gf_slab_pack_face(self.ctx, self.U, which, block_parity, buf)
+        with self._on_stream():
+            self.gfm.gf_slab_pack_face(self.ctx, self.U, which, block_parity, buf)
         return buf
 
     def unpack_face(self, which: int, block_parity: int, buf):
-        self.gfm.gf_slab_unpack_face(self.ctx, self.U, which, block_parity, buf)
+        with self._on_stream():
+            self.gfm.gf_slab_unpack_face(self.ctx, self.U, which, block_parity, buf)
 
     def half_sweep(self, kind, parity: int, sweep: int, t_first: int, t_count: int):
-        if kind[0] == "anneal":
-            self.gfm.gf_anneal_half(self.ctx, self.U, kind[1], parity, sweep, kind[2], t_first, t_count)
-        else:
-            self.gfm.gf_relax_half(self.ctx, self.U, kind[1], kind[2], parity, sweep, kind[3], t_first, t_count)
+        with self._on_stream():
+            if kind[0] == "anneal":
+                self.gfm.gf_anneal_half(self.ctx, self.U, kind[1], parity, sweep, kind[2], t_first, t_count)
+            else:
+                self.gfm.gf_relax_half(self.ctx, self.U, kind[1], kind[2], parity, sweep, kind[3], t_first, t_count)
 
     def begin(self):
-        self.gfm.gf_begin_sweeps(self.ctx)
+        with self._on_stream():
+            self.gfm.gf_begin_sweeps(self.ctx)
 
     def raw_sums(self):
-        return self.gfm.gf_raw_sums(self.ctx, self.U)
+        with self._on_stream():
+            return self.gfm.gf_raw_sums(self.ctx, self.U)
 
     def theta_slices(self):
-        return self.gfm.gf_theta_slices(self.ctx, self.U, self.Nt)
+        with self._on_stream():
+            return self.gfm.gf_theta_slices(self.ctx, self.U, self.Nt)
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -278,11 +326,17 @@ class SlabRunner:
         return done, th, F
 
 
-def local_slabs(dims, nslabs: int, precision="fp64", gauge="landau", reals_per_link: int = 18, overlap: bool = True):
-    """nslabs slab contexts of one configuration in this process (one GPU), wired into a :class:`SlabRunner`"""
+def local_slabs(dims, nslabs: int, precision="fp64", gauge="landau", reals_per_link: int = 18, overlap: bool = True,
+                streams: bool = False):
+    """nslabs slab contexts of one configuration in this process (one GPU), wired into a :class:`SlabRunner`.
+    streams = False: every launch and copy on the current stream (:class:`LocalRing`; the schedule's order only).
+    streams = True: one CUDA stream per slab, face copies ordered by events (:class:`StreamRing`): the interior launches
+    of a slab overlap the face traffic and the other slabs' launches, as they would across GPUs."""
     bounds = slab_bounds(dims[3], nslabs)
-    engines = {r: GpuSlab(dims, b[0], b[1], precision, gauge, reals_per_link) for r, b in enumerate(bounds)}
-    return SlabRunner(engines, LocalRing(nslabs), dims, gauge, overlap), bounds
+    engines = {r: GpuSlab(dims, b[0], b[1], precision, gauge, reals_per_link, own_stream=streams)
+               for r, b in enumerate(bounds)}
+    ring = StreamRing(engines) if streams else LocalRing(nslabs)
+    return SlabRunner(engines, ring, dims, gauge, overlap), bounds
 
 
 def dist_slab(dims, precision="fp64", gauge="landau", reals_per_link: int = 18, overlap: bool = True, group=None):

@@ -110,6 +110,40 @@ def test_slabs_other_formats_and_random_updates(gfm, precision, R):
         e.close()
 
 
+@pytest.mark.parametrize("nslabs", [2, 4])
+@pytest.mark.parametrize("gauge", ["landau", "coulomb"])
+def test_slabs_on_their_own_streams_bit_identical(gfm, nslabs, gauge):
+    """every slab on its own CUDA stream, the face copies ordered by events alone (StreamRing): interior launches,
+    face traffic and the other slabs' launches may now run in any order the events allow, so a missing dependency in
+    the schedule would show as a wrong link.  Relaxation, annealing and stochastic sweeps sharded = unsharded bit for
+    bit, repeated so that an ordering that only sometimes fails has several chances; F and theta from the raw sums."""
+    from paper_1209_4008_b200 import slab
+
+    dims = (16, 16, 16, 16)
+    U = gf_inputs.smooth_random(dims, 0.4, 75)
+    fx = gfm.GaugeFixer(dims, precision="fp64", gauge=gauge)
+    if gauge == "coulomb":
+        gfm.gf_set_coulomb_reading(fx.ctx, False)  # the slabs run reading A
+    fx.load(U)
+    fx.overrelax(1.7, 6)
+    fx.anneal(1.0, 0.2, 3, 11)
+    fx.relax(gfm.GF_UPDATE_STOCHASTIC, 0.6, 4, seed=5)
+    whole = fx.download()
+    for rep in range(3):
+        run, bounds = slab.local_slabs(dims, nslabs, "fp64", gauge, overlap=True, streams=True)
+        assert len({e.stream.cuda_stream for e in run.eng.values()}) == nslabs
+        _load(run, bounds, U, dims)
+        run.overrelax(1.7, 6)
+        run.anneal(1.0, 0.2, 3, 11)
+        run.overrelax(0.6, 4, update=gfm.GF_UPDATE_STOCHASTIC, seed=5)
+        assert np.array_equal(_gather(run, bounds), whole), (nslabs, rep)
+        F, th = run.functional_theta()
+        assert F == pytest.approx(fx.functional(), rel=1e-13) and th == pytest.approx(fx.theta(), rel=1e-11)
+        for e in run.eng.values():
+            e.close()
+    fx.close()
+
+
 def test_slab_fix_loop_and_errors(gfm):
     """the driver's Alg. 1 loop on slabs stops where gf_fix with the separate check stops (same theta to rounding);
     argument checks of the slab calls"""
