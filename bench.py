@@ -214,6 +214,8 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
     if barrier is not None:
         barrier()
     launches0 = gfm.gf_launch_count(fx.ctx)
+    fp32 = w["precision"] == "fp32"
+    dc0 = gfm.gf_chain_count(fx.ctx) if fp32 else (0, 0)  # synchronises; outside the timed region
     h0 = time.perf_counter()
     t0.record(stream)
     for k in range(steps):
@@ -229,6 +231,9 @@ def time_device(gfm, fx, w, sweeps, steps, warmup, stream, barrier=None, sampler
         barrier()
     total = t0.elapsed_time(t1) * 1e-3
     in_sweeps = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+    dc1 = gfm.gf_chain_count(fx.ctx) if fp32 else (0, 0)
+    # hybrid chain (fp32): launches / site updates of the TIMED region that ran in double
+    time_device.double_chain = (dc1[0] - dc0[0], dc1[1] - dc0[1])
     return total, in_sweeps, gfm.gf_launch_count(fx.ctx) - launches0, F, th, clocks
 
 
@@ -563,7 +568,7 @@ def main():
         fits = field_bytes_of(wl) <= L2_BYTES
         total, in_sw, launches, F, th, clocks = time_device(gfm, fx, wl, sweeps, steps, warmup, stream, bar, sampler)
         regs, spill = gfm.gf_kernel_info(fx.ctx, 1 if wl.get("anneal") else 0)
-        dc_launches, dc_sites = gfm.gf_chain_count(fx.ctx) if wl["precision"] == "fp32" else (0, 0)
+        dc_launches, dc_sites = time_device.double_chain  # over the timed region only
         fx.close()
         del fx
         torch.cuda.empty_cache()
@@ -627,7 +632,9 @@ def main():
                      "steps": a_steps, "ms_per_step": a["total"] / a_steps * 1e3,
                      "fits_l2": a["fits_l2"], "roofline": a["roofline"], "F": a["F"], "theta": a["theta"],
                      "regs_per_thread": a["regs"], "spill_bytes": a["spill"],
-                     "double_chain_launches": a["double_chain_launches"], "sites_redone_in_double": a["double_sites"]})
+                     "gpu_launches": a["launches"], "double_chain_launches": a["double_chain_launches"],
+                     "double_chain_fraction": a["double_chain_launches"] / max(1, 2 * sweeps * a_steps),
+                     "sites_redone_in_double": a["double_sites"]})
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -670,7 +677,8 @@ def main():
         "paper_context": "300 GFlops on GTX 580 (PAPER.md:13), another machine: context, not the target",
         "F": m["F"], "theta": m["theta"],
         "regs_per_thread": m["regs"], "spill_bytes": m["spill"],
-        "double_chain_launches": m["double_chain_launches"],
+        "double_chain_launches": m["double_chain_launches"],  # of the 2 * sweeps * steps half-sweep launches timed
+        "double_chain_fraction": m["double_chain_launches"] / max(1, 2 * sweeps * steps),
         "roofline": m["roofline"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
         "clocks": m["clocks"], "also": also,
     }
